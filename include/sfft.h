@@ -1,0 +1,184 @@
+/*
+ * sfft.h -- C ABI of libsfft: the SFFT (Saccadic Fast Fourier Transform) subtraction
+ * hot path on one NVIDIA B200 (sm_100a), FP64.
+ *
+ * What the library computes (BASELINE.json north_star; the paper only names the method:
+ * PAPER.md:29 "Saccadic Fast Fourier Transform (SFFT) method for difference imaging",
+ * PAPER.md:43 "flexible delta basis function", "[GPU] Apply SFFT subtraction"):
+ *
+ *     D = S - (R (*) K(x,y)) - B(x,y)
+ *
+ * K is an L x L delta-basis kernel whose coefficients vary as a 2-D polynomial of total
+ * degree DK over the frame, B a background polynomial of total degree DB.  The
+ * n = L*L*NK + NB coefficients (NK=(DK+1)(DK+2)/2, NB=(DB+1)(DB+2)/2) are the linear
+ * least-squares solution of  min || vec(m.S) - A c ||_2 ; column (t,u,v) of A is the
+ * image (x,y) -> T_t((x-u) mod nx, (y-v) mod ny),  T_t = xt^i yt^j (m.R),  column s is
+ * P_s = xt^p yt^q  (not masked);  xt = (2x+1-nx)/nx, yt = (2y+1-ny)/ny;  boundary
+ * conditions are circular at the native nx x ny (readings C2-C7).
+ *
+ * Steps:
+ *   a1  polynomial-weighted template images and their 2-D FFTs      (sfft_build_system)
+ *   a2  cross-correlations at kernel-offset pairs from the spectra   (sfft_build_system)
+ *   a3  gather into G = A^T A (n x n) and h = A^T b                  (sfft_build_system)
+ *   a4  FP64 Cholesky solve of the Jacobi-equilibrated system        (sfft_solve)
+ *   a5  FFT convolution with the solved kernel + fused subtraction   (sfft_subtract)
+ *   a6  batched: one template, many science images                  (sfft_set_template,
+ *                                                                     sfft_subtract_batch)
+ *
+ * Conventions
+ *   - images: row-major FP64, img[y*nx + x], 0 <= x < nx, 0 <= y < ny, DEVICE pointers
+ *     unless a parameter says "host"; inputs are never modified.
+ *   - mask: DEVICE ny*nx uint8 (non-zero = use pixel in the fit) or NULL = all ones.
+ *     The fit uses m.S and m.R; the subtraction uses the unmasked S and R.
+ *   - coefficient layout (output of the method), w = (L-1)/2:
+ *       coeffs[t*L*L + (v+w)*L + (u+w)] = a_{t,u,v},  t <-> (i,j) in the order
+ *       (0,0),(1,0),(0,1),(2,0),(1,1),(0,2),(3,0),...  (total degree ascending, then j);
+ *       coeffs[NK*L*L + s] = b_s in the same (p,q) order.
+ *     The kernel applied at SOURCE pixel (x',y') is K(u,v) = sum_t a_{t,u,v} xt(x')^i yt(y')^j.
+ *   - every call enqueues its kernels on the plan's CUDA stream and returns without
+ *     synchronising the device, except where stated.  No exceptions cross the boundary;
+ *     every function returns an sfft_status (or a plain value for the getters).
+ *   - the plan owns all workspaces (twiddles, spectra, lag tables, G, the factor).
+ *   - there is NO CPU fallback: without a CUDA device sfft_plan_create fails with
+ *     SFFT_ERR_CUDA.
+ */
+#ifndef SFFT_H
+#define SFFT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sfft_plan sfft_plan; /* opaque */
+
+typedef enum {
+    SFFT_OK = 0,
+    SFFT_ERR_INVALID_ARG = -1, /* bad size / NULL pointer / unsupported L or frame size       */
+    SFFT_ERR_ALLOC = -2,       /* host or device allocation failed                             */
+    SFFT_ERR_CUDA = -3,        /* a CUDA runtime call or kernel launch failed (no device etc.) */
+    SFFT_ERR_STATE = -4,       /* call order: solve before build, subtract before solve, ...   */
+    SFFT_ERR_NOT_SPD = -5      /* a pivot of the equilibrated matrix was <= 1e-12 (reading C9) */
+} sfft_status;
+
+/* Stage indices of sfft_get_timings (milliseconds of the most recent call of each stage). */
+enum {
+    SFFT_STAGE_A1_TEMPLATE = 0, /* weighted template images + forward FFTs           */
+    SFFT_STAGE_A1_SCIENCE = 1,  /* forward FFT of m.S                                */
+    SFFT_STAGE_A2_OMEGA = 2,    /* template-template lag tables (+Gamma)             */
+    SFFT_STAGE_A2_THETA = 3,    /* template-science lag tables (+Delta)              */
+    SFFT_STAGE_A3_GATHER = 4,   /* fill of G and h                                   */
+    SFFT_STAGE_A4_FACTOR = 5,   /* equilibration + Cholesky factorisation            */
+    SFFT_STAGE_A4_SOLVE = 6,    /* two triangular solves                             */
+    SFFT_STAGE_A5_SUBTRACT = 7, /* kernel spectrum synthesis, inverse FFTs, D        */
+    SFFT_NUM_STAGES = 8
+};
+
+/* Create a plan for nx x ny frames, L x L kernel (L odd, 1 <= L <= 21), polynomial degrees
+ * DK, DB (0 <= DK, DB <= 3).  Requires 2L-1 <= nx, ny <= 8192.  Frames are zero-padded
+ * internally to the next powers of two (>= 64); any nx, ny in range is supported,
+ * including 256, 1024 and 4088.  Allocates every workspace; uses the
+ * current CUDA device and the legacy default stream until sfft_plan_set_stream.
+ * Errors: INVALID_ARG, ALLOC, CUDA (no usable device). */
+sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int DB);
+
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream). */
+sfft_status sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
+
+/* Synchronises the plan's stream, frees everything.  NULL is accepted. */
+sfft_status sfft_plan_destroy(sfft_plan *plan);
+
+/* n = L*L*NK + NB (BASELINE.json north_star: unknown count).  0 for a NULL plan. */
+int sfft_num_unknowns(const sfft_plan *plan);
+
+/* Bytes of device memory the plan holds.  0 for a NULL plan. */
+size_t sfft_workspace_bytes(const sfft_plan *plan);
+
+/* ---- single pair ------------------------------------------------------------------ */
+
+/* a1-a3 for one (S, R, mask): afterwards the plan holds G and h.  The plan keeps the
+ * POINTERS S and R (not copies) for sfft_subtract: both must stay alive and unchanged
+ * until sfft_subtract has been enqueued and has run.  Errors: INVALID_ARG (NULL S/R), CUDA. */
+sfft_status sfft_build_system(sfft_plan *plan, const double *S, const double *R,
+                              const uint8_t *mask);
+
+/* a4: Jacobi equilibration, blocked Cholesky, two triangular solves.  Asynchronous: a
+ * failed pivot test is recorded on the device and reported by sfft_sync_status (or by the
+ * next sfft_subtract with a host coefficient read).  Errors: STATE, CUDA. */
+sfft_status sfft_solve(sfft_plan *plan);
+
+/* a5: D (device, ny*nx) = S - sum_t T_t (*) K_t - B using the solved coefficients;
+ * coeffs (device, n doubles) receives them, or NULL.  Errors: STATE, INVALID_ARG, CUDA. */
+sfft_status sfft_subtract(sfft_plan *plan, double *D, double *coeffs);
+
+/* Debug/verification variant of a5: subtract with coefficients the
+ * CALLER supplies (device, n doubles) instead of the solved ones.  Needs a prior
+ * sfft_build_system or sfft_set_template (+ S given here when S != NULL).  */
+sfft_status sfft_subtract_with(sfft_plan *plan, const double *S, const double *coeffs_in,
+                               double *D);
+
+/* ---- batched: one template, many science images (BASELINE.json configs[3]) ---------- */
+
+/* Template-side work, once: a1 (template), Omega, Gamma, Phi, the matrix part of a3 and
+ * the Cholesky factor of a4.  Keeps the pointer R (see sfft_build_system). */
+sfft_status sfft_set_template(sfft_plan *plan, const double *R, const uint8_t *mask);
+
+/* For b = 0..B-1: a1 (science), Theta, Delta, h, two triangular solves, a5.
+ * S, D: HOST arrays of B device pointers (ny*nx doubles each); coeffs: device B*n doubles
+ * or NULL.  mask is the one given to sfft_set_template.  Errors: STATE, INVALID_ARG, CUDA. */
+sfft_status sfft_subtract_batch(sfft_plan *plan, const double *const *S, int B,
+                                double *const *D, double *coeffs);
+
+/* ---- host-buffer convenience (the end-to-end call bench.py times as `e2e`) ---------- */
+
+/* Whole single-pair path from HOST buffers: copies S, R (and mask, may be NULL) to plan-owned
+ * device staging, runs a1-a5, copies D (ny*nx) and coeffs (n, may be NULL) back and
+ * SYNCHRONISES.  Returns NOT_SPD if the pivot test failed. */
+sfft_status sfft_difference_host(sfft_plan *plan, const double *S_host, const double *R_host,
+                                 const uint8_t *mask_host, double *D_host, double *coeffs_host);
+
+/* ---- introspection for tests and bench ------------------------------------------------ */
+
+/* Synchronises the stream and returns SFFT_ERR_NOT_SPD if the most recent factorisation
+ * failed its pivot test, SFFT_ERR_CUDA on a sticky CUDA error, else SFFT_OK. */
+sfft_status sfft_sync_status(sfft_plan *plan);
+
+/* Copies G (device, n*n, symmetric so row-major == column-major) and/or h (device, n);
+ * either may be NULL.  Errors: STATE (nothing built yet). */
+sfft_status sfft_get_system(const sfft_plan *plan, double *G, double *h);
+
+/* ms[0..n_stages) <- per-stage milliseconds (CUDA events on the plan's stream) of the most
+ * recent call of each stage; synchronises.  Timing is off until sfft_enable_timings(plan,1). */
+sfft_status sfft_enable_timings(sfft_plan *plan, int on);
+sfft_status sfft_get_timings(sfft_plan *plan, float *ms, int n_stages);
+
+/* Number of kernel launches this plan has enqueued since creation (bench: gpu_launches). */
+long long sfft_launch_count(const sfft_plan *plan);
+
+/* Plan-owned, NUL-terminated description of the most recent error ("" if none). */
+const char *sfft_last_error(const sfft_plan *plan);
+
+/* Library version string, e.g. "sfft-b200 0.1 (sm_100a)". */
+const char *sfft_version(void);
+
+/* Test hook: copies an internal device array to a HOST buffer (synchronises).
+ *   which = 0: template spectrum t=idx  (My x Hx complex128, column 0 = DC + i*Nyquist packed)
+ *           1: science spectrum
+ *           2: Omega lag table of pair idx ((4w+1)^2 doubles, [dv+2w][du+2w])
+ *           3: Theta lag table of t=idx (L*L doubles)
+ *           4: Gamma (NK*NB*L*L doubles), 5: Phi (NB*NB), 6: Delta (NB)
+ *           7: padded sizes {Mx, My} as two doubles
+ * Returns INVALID_ARG if nbytes is not the array's size. */
+sfft_status sfft_debug_read(sfft_plan *plan, int which, int idx, void *host_dst, size_t nbytes);
+
+/* FP64 rate probes used by bench.py to state the ALU roofline it divides by
+ * (DESIGN.md "peaks"): runs a register-resident DFMA (kind=0) or DMMA m8n8k4 (kind=1)
+ * loop on every SM for `iters` iterations and returns the achieved TFLOP/s in *tflops. */
+sfft_status sfft_probe_fp64(int kind, int iters, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFFT_H */

@@ -1,0 +1,153 @@
+// sfft_assemble.cu -- the polynomial terms of a2 and the gather a3
+// (BASELINE.json north_star (b)):
+//   Gamma_{t,s}[u,v] = X(T_t, P_s)[u,v],  P_s = xt^p yt^q (never masked, reading C7)
+//   Delta_s          = sum P_s (m.S)
+//   G[(t,u,v),(t',u',v')] = Omega_{tt'}[u-u', v-v'],  G[(t,u,v),s] = Gamma_{t,s}[u,v],  G[s,s'] = Phi_{ss'}
+//   h[(t,u,v)] = Theta_t[u,v],  h[s] = Delta_s
+// Gamma is separable: with the row moments mu_m[y] = sum_x xt^m (m.R)(x,y) from the a1 row pass,
+//   A_{i,p,u}[y] = sum_x xt^i xt((x+u) mod nx)^p (m.R)(x,y)
+//               = sum_k C(p,k) (2u/nx)^(p-k) mu_{i+k}[y]  +  (the |u| wrapped pixels, fixed up directly)
+//   Gamma_{(i,j),(p,q)}[u,v] = sum_y yt^j yt((y+v) mod ny)^q A_{i,p,u}[y].
+#include "sfft_internal.h"
+
+namespace sfft {
+
+__device__ __forceinline__ double ipw(double b, int e) { double r = 1.0; for (int k = 0; k < e; k++) r *= b; return r; }
+
+// one thread per (y, u, i, p)
+__global__ void gamma_rows_kernel(const double *__restrict__ mu, const double *__restrict__ R,
+                                  const uint8_t *__restrict__ mask, double *__restrict__ gamA, Geom g) {
+    const int L = g.L, w = g.w, ny = g.ny, nx = g.nx;
+    const long long total = (long long)(g.DK + 1) * (g.DB + 1) * L * ny;
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= total) return;
+    const int y = (int)(id % ny);
+    long long r = id / ny;
+    const int ui = (int)(r % L); r /= L;
+    const int pp = (int)(r % (g.DB + 1));
+    const int i = (int)(r / (g.DB + 1));
+    const int u = ui - w;
+    const double delta = 2.0 * u / (double)nx;
+    // binomial expansion of (xt + delta)^p
+    double acc = 0.0, binom = 1.0;
+    for (int k = 0; k <= pp; k++) {
+        acc += binom * ipw(delta, pp - k) * mu[(size_t)(i + k) * ny + y];
+        binom = binom * (pp - k) / (k + 1);
+    }
+    // wrapped pixels: xt((x+u) mod nx) = xt + delta -/+ 2
+    if (pp > 0 && u != 0) {
+        const int xa = u > 0 ? nx - u : 0, xb = u > 0 ? nx : -u;
+        for (int x = xa; x < xb; x++) {
+            const size_t o = (size_t)y * nx + x;
+            double v = R[o]; if (mask && !mask[o]) v = 0.0;
+            const double xt = (2.0 * x + 1.0 - nx) / nx;
+            const int xw = u > 0 ? x + u - nx : x + u + nx;
+            const double xtw = (2.0 * xw + 1.0 - nx) / nx;
+            acc += (ipw(xtw, pp) - ipw(xt + delta, pp)) * ipw(xt, i) * v;
+        }
+    }
+    gamA[id] = acc; // layout [i][p][u][y]
+}
+
+__device__ __forceinline__ double block_sum2(double v, double *sh) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+    __syncthreads();
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x == 0) for (int k = 0; k < (int)(blockDim.x >> 5); k++) r += sh[k];
+    return r;
+}
+
+// grid = (L*L, NB, NK); block 128
+__global__ void __launch_bounds__(128) gamma_cols_kernel(const double *__restrict__ gamA, double *__restrict__ gam, Geom g) {
+    __shared__ double sh[32];
+    const int L = g.L, w = g.w, ny = g.ny;
+    const int uv = blockIdx.x, s = blockIdx.y, t = blockIdx.z;
+    const int ui = uv % L, v = uv / L - w;
+    const int i = g.pi[t], j = g.pj[t], pp = g.pi[s], qq = g.pj[s];
+    const double *A = gamA + (((size_t)i * (g.DB + 1) + pp) * L + ui) * ny;
+    double acc = 0.0;
+    for (int y = threadIdx.x; y < ny; y += blockDim.x) {
+        int y2 = y + v; if (y2 >= ny) y2 -= ny; if (y2 < 0) y2 += ny;
+        const double yt = (2.0 * y + 1.0 - ny) / ny, yt2 = (2.0 * y2 + 1.0 - ny) / ny;
+        acc += ipw(yt, j) * ipw(yt2, qq) * A[y];
+    }
+    acc = block_sum2(acc, sh);
+    if (threadIdx.x == 0) gam[((size_t)t * g.NB + s) * L * L + uv] = acc;
+}
+
+// grid = NB; block 128:  Delta_s = sum_y yt^q muS_p[y]
+__global__ void __launch_bounds__(128) delta_kernel(const double *__restrict__ muS, double *__restrict__ delta, Geom g) {
+    __shared__ double sh[32];
+    const int s = blockIdx.x, pp = g.pi[s], qq = g.pj[s], ny = g.ny;
+    double acc = 0.0;
+    for (int y = threadIdx.x; y < ny; y += blockDim.x)
+        acc += ipw((2.0 * y + 1.0 - ny) / ny, qq) * muS[(size_t)pp * ny + y];
+    acc = block_sum2(acc, sh);
+    if (threadIdx.x == 0) delta[s] = acc;
+}
+
+__device__ __forceinline__ int pair_index(int t, int tp, int NK) { return t * NK - (t * (t - 1)) / 2 + (tp - t); }
+
+// one thread per entry of G (full matrix, both triangles)
+__global__ void gather_G_kernel(const double *__restrict__ lagO, const double *__restrict__ gam,
+                                const double *__restrict__ phi, double *__restrict__ G, Geom g) {
+    const int n = g.n, L = g.L, w = g.w, LL = L * L, NKLL = g.NK * LL, W2 = 4 * w + 1;
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (long long)n * n) return;
+    const int r = (int)(id / n), c = (int)(id % n);
+    double val;
+    if (r < NKLL && c < NKLL) {
+        const int t = r / LL, v = (r % LL) / L - w, u = (r % LL) % L - w;
+        const int tp = c / LL, vp = (c % LL) / L - w, up = (c % LL) % L - w;
+        if (t <= tp) val = lagO[(size_t)pair_index(t, tp, g.NK) * W2 * W2 + (v - vp + 2 * w) * W2 + (u - up + 2 * w)];
+        else val = lagO[(size_t)pair_index(tp, t, g.NK) * W2 * W2 + (vp - v + 2 * w) * W2 + (up - u + 2 * w)];
+    } else if (r < NKLL) {
+        val = gam[((size_t)(r / LL) * g.NB + (c - NKLL)) * LL + r % LL];
+    } else if (c < NKLL) {
+        val = gam[((size_t)(c / LL) * g.NB + (r - NKLL)) * LL + c % LL];
+    } else {
+        val = phi[(r - NKLL) * g.NB + (c - NKLL)];
+    }
+    G[id] = val;
+}
+
+__global__ void gather_h_kernel(const double *__restrict__ lagT, const double *__restrict__ delta, double *__restrict__ h, Geom g) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= g.n) return;
+    const int NKLL = g.NK * g.L * g.L;
+    h[r] = r < NKLL ? lagT[r] : delta[r - NKLL];
+}
+
+cudaError_t launch_gamma(sfft_plan *p) {
+    const Geom &g = p->g;
+    const long long total = (long long)(g.DK + 1) * (g.DB + 1) * g.L * g.ny;
+    gamma_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->stream>>>(p->muR, p->R, p->mask, p->gamA, g);
+    gamma_cols_kernel<<<dim3(g.L * g.L, g.NB, g.NK), 128, 0, p->stream>>>(p->gamA, p->gam, g);
+    p->launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_delta(sfft_plan *p) {
+    delta_kernel<<<p->g.NB, 128, 0, p->stream>>>(p->muS, p->delta, p->g);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gather_G(sfft_plan *p) {
+    const long long total = (long long)p->g.n * p->g.n;
+    gather_G_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->stream>>>(p->lagO, p->gam, p->phi, p->G, p->g);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gather_h(sfft_plan *p) {
+    gather_h_kernel<<<(p->g.n + 255) / 256, 256, 0, p->stream>>>(p->lagT, p->delta, p->h, p->g);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+} // namespace sfft

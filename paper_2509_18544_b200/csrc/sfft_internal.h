@@ -1,0 +1,112 @@
+// sfft_internal.h -- plan layout and kernel launchers shared by the .cu files of libsfft.
+// Not part of the C ABI (include/sfft.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/sfft.h"
+#include "sfft_fft.cuh"
+
+namespace sfft {
+
+constexpr int MAX_DEG = 3;                                   // DK, DB <= 3
+constexpr int MAX_NP = (MAX_DEG + 1) * (MAX_DEG + 2) / 2;    // 10 polynomial terms
+constexpr int MAX_L = 21;
+constexpr int MAX_PAIRS = MAX_NP * (MAX_NP + 1) / 2;         // 55 unordered template pairs
+constexpr double PIVOT_MIN = 1e-12;                          // reading C9
+
+// Geometry every kernel needs, passed by value.
+struct Geom {
+    int nx, ny;        // frame
+    int Mx, My;        // zero-padded power-of-two FFT sizes
+    int Hx;            // Mx/2: complex columns of a (packed) half spectrum
+    int log2Hx, log2My;
+    int L, w;          // kernel size, half width
+    int DK, DB, NK, NB, n;
+    int Nt;            // twiddle table length (max(Mx, My)); tw[k] = exp(-2 pi i k/Nt)
+    int pi[MAX_NP], pj[MAX_NP]; // t -> (i,j): total degree ascending, then j ascending
+};
+
+struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of one lag pass
+    int np;
+    int a[MAX_PAIRS], b[MAX_PAIRS];
+};
+
+} // namespace sfft
+
+struct sfft_plan {
+    sfft::Geom g;
+    cudaStream_t stream;
+    // device workspaces
+    sfft::cplx *tw;          // [Nt]
+    sfft::cplx *inter;       // [(DK+1)][ny][Hx] row-transformed intermediates (a1) / a5 intermediate
+    sfft::cplx *specT;       // [NK][My][Hx] spectra of the fit (masked) template images
+    sfft::cplx *specTo;      // [NK][My][Hx] spectra of the unmasked template images (== specT without mask)
+    sfft::cplx *specS;       // [My][Hx]
+    double *muR;             // [(DK+DB+1)][ny] row moments sum_x xt^m (m.R)
+    double *muS;             // [(DB+1)][ny]
+    sfft::cplx *Q;           // [np][2W+1][Hx+1] column-reduced products (stage 1 of a2)
+    double *lagO;            // [npairs][(4w+1)^2]
+    double *lagT;            // [NK][L*L]
+    double *bpart;           // [chunks][np][(2W+1)^2] wrap-correction partial sums
+    double *gamA;            // [(DK+1)][(DB+1)][L][ny] row sums for Gamma
+    double *gam;             // [NK][NB][L*L]
+    double *phi;             // [NB][NB]
+    double *delta;           // [NB]
+    double *G;               // [n][n]
+    double *h;               // [n]
+    double *Lf;              // [n][n] Cholesky factor of the equilibrated matrix (lower, row-major)
+    double *dscale;          // [n]   1/sqrt(G_ii)
+    double *ywork;           // [n]
+    double *coef;            // [n]   solved coefficients
+    sfft::cplx *E;           // [NK][L][Hx+1] kernel row tables for a5
+    int *flag;               // device: 1 = pivot test failed
+    int *flag_host;          // pinned mirror
+    // host staging for sfft_difference_host
+    double *stS, *stR, *stD; uint8_t *stM;
+    size_t bytes;
+    // state
+    const double *S, *R; const uint8_t *mask;
+    bool have_template, have_system, have_factor, have_solution;
+    int npairsO;
+    sfft::PairList plO, plT;
+    // timing
+    bool timing; cudaEvent_t ev0[SFFT_NUM_STAGES], ev1[SFFT_NUM_STAGES]; bool ev_used[SFFT_NUM_STAGES];
+    long long launches;
+    char err[256];
+};
+
+namespace sfft {
+
+// ---- a1 (sfft_fwd.cu) ---------------------------------------------------------------
+// rows: img (ny x nx real, optional mask) -> inter[i] (ny x Hx packed), i = 0..NI-1, weights xt^i;
+// also row moments mu[m][y] = sum_x xt^m (m.img), m = 0..NMOM-1.
+cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI,
+                           double *mu, int NMOM);
+// columns: inter[ii[k]] * yt^jj[k] -> spec[k] (My x Hx), k = 0..ns-1
+cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj);
+
+struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, rows_per_split; };
+void lagcol_config(const Geom &g, int np, int W, LagCfg *c);
+int border_chunks();
+// ---- a2, a3 (sfft_lags.cu, sfft_assemble.cu) ---------------------------------------------------------
+// lag tables of pair list pl over spectra base[s] = spec0 + s*My*Hx (s < nsA: template set, s == nsA: specS)
+cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag /*[np][(2W+1)^2]*/, bool science);
+cudaError_t launch_gamma(sfft_plan *p);   // muR, R, mask -> gam
+cudaError_t launch_delta(sfft_plan *p);   // muS -> delta
+cudaError_t launch_gather_G(sfft_plan *p);
+cudaError_t launch_gather_h(sfft_plan *p);
+
+// ---- a4 (sfft_solve.cu) ------------------------------------------------------------------
+cudaError_t launch_factor(sfft_plan *p);                      // G -> dscale, Lf, flag
+cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c); // c = D (L^-T (L^-1 (D h)))
+
+// ---- a5 (sfft_subtract.cu) ---------------------------------------------------------------
+cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D);
+
+// ---- probes (sfft_probe.cu) -------------------------------------------------------------------
+cudaError_t run_probe_fp64(int kind, int iters, double *tflops);
+
+inline int ilog2(int v) { int l = 0; while ((1 << l) < v) l++; return l; }
+
+} // namespace sfft
