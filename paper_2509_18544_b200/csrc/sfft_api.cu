@@ -1,0 +1,435 @@
+// sfft_api.cu -- the C ABI of include/sfft.h: plan life cycle, stage sequencing, introspection.
+// Every compute step is a kernel of this library (sfft_fwd/lags/assemble/solve/subtract.cu);
+// this file only validates, allocates, orders launches on the plan's stream and times them.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cmath>
+#include <new>
+#include "sfft_internal.h"
+
+using namespace sfft;
+
+namespace sfft {
+
+__global__ void twiddle_kernel(cplx *tw, int Nt) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= Nt) return;
+    double s, c;
+    sincospi(-2.0 * (double)k / (double)Nt, &s, &c);
+    tw[k] = mk(c, s);
+}
+
+static void poly_index(int t, int *i, int *j) { // total degree ascending, then j ascending (reading C4)
+    int d = 0;
+    while (t > d) { t -= d + 1; d++; }
+    *j = t; *i = d - t;
+}
+
+static int next_pow2(int v, int lo) { int m = lo; while (m < v) m <<= 1; return m; }
+
+// sum_x xt(x)^k, xt = (2x+1-n)/n: exactly 0 for odd k (pin P7), long double otherwise
+static double power_sum(int n, int k) {
+    if (k & 1) return 0.0;
+    long double acc = 0.0L;
+    for (int x = 0; x < n; x++) {
+        long double t = (2.0L * x + 1.0L - n) / n, p = 1.0L;
+        for (int e = 0; e < k; e++) p *= t;
+        acc += p;
+    }
+    return (double)acc;
+}
+
+} // namespace sfft
+
+static sfft_status fail(sfft_plan *p, sfft_status st, const char *what, cudaError_t e = cudaSuccess) {
+    if (p) {
+        if (e != cudaSuccess) snprintf(p->err, sizeof(p->err), "%s: %s", what, cudaGetErrorString(e));
+        else snprintf(p->err, sizeof(p->err), "%s", what);
+    }
+    return st;
+}
+
+#define CK(call, what)                                                          \
+    do {                                                                        \
+        cudaError_t e_ = (call);                                                \
+        if (e_ != cudaSuccess) return fail(p, SFFT_ERR_CUDA, what, e_);         \
+    } while (0)
+
+template <typename T> static cudaError_t dalloc(sfft_plan *p, T **ptr, size_t count) {
+    cudaError_t e = cudaMalloc((void **)ptr, count * sizeof(T));
+    if (e == cudaSuccess) p->bytes += count * sizeof(T);
+    return e;
+}
+
+struct StageTimer {
+    sfft_plan *p; int stage;
+    StageTimer(sfft_plan *p_, int s) : p(p_), stage(s) {
+        if (p->timing) { cudaEventRecord(p->ev0[stage], p->stream); p->ev_used[stage] = true; }
+    }
+    ~StageTimer() { if (p->timing) cudaEventRecord(p->ev1[stage], p->stream); }
+};
+
+static void free_plan(sfft_plan *p) {
+    if (!p) return;
+    void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
+                    p->Q, p->lagO, p->lagT, p->bpart, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale,
+                    p->ywork, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+    for (void *q : ptrs) if (q) cudaFree(q);
+    if (p->flag_host) cudaFreeHost(p->flag_host);
+    for (int s = 0; s < SFFT_NUM_STAGES; s++) {
+        if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
+        if (p->ev1[s]) cudaEventDestroy(p->ev1[s]);
+    }
+    delete p;
+}
+
+extern "C" {
+
+const char *sfft_version(void) { return "sfft-b200 0.1 (sm_100a)"; }
+
+sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int DB) {
+    if (!out) return SFFT_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (L < 1 || L > MAX_L || !(L & 1) || DK < 0 || DK > MAX_DEG || DB < 0 || DB > MAX_DEG) return SFFT_ERR_INVALID_ARG;
+    if (nx < 2 * L - 1 || ny < 2 * L - 1 || nx > 8192 || ny > 8192) return SFFT_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return SFFT_ERR_CUDA; }
+    sfft_plan *p = new (std::nothrow) sfft_plan();
+    if (!p) return SFFT_ERR_ALLOC;
+    memset(p, 0, sizeof(*p));
+    Geom &g = p->g;
+    g.nx = nx; g.ny = ny; g.L = L; g.w = (L - 1) / 2; g.DK = DK; g.DB = DB;
+    g.NK = (DK + 1) * (DK + 2) / 2; g.NB = (DB + 1) * (DB + 2) / 2; g.n = L * L * g.NK + g.NB;
+    g.Mx = next_pow2(nx, 64); g.My = next_pow2(ny, 64); g.Hx = g.Mx / 2;
+    g.log2Hx = ilog2(g.Hx); g.log2My = ilog2(g.My);
+    g.Nt = g.Mx > g.My ? g.Mx : g.My;
+    for (int t = 0; t < MAX_NP; t++) poly_index(t, &g.pi[t], &g.pj[t]);
+    // pair lists: Omega t <= t' ; Theta (t, science)
+    p->plO.np = 0;
+    for (int t = 0; t < g.NK; t++)
+        for (int tp = t; tp < g.NK; tp++) { p->plO.a[p->plO.np] = t; p->plO.b[p->plO.np] = tp; p->plO.np++; }
+    p->plT.np = g.NK;
+    for (int t = 0; t < g.NK; t++) { p->plT.a[t] = t; p->plT.b[t] = g.NK; }
+    p->npairsO = p->plO.np;
+
+    const size_t plane = (size_t)g.My * g.Hx;
+    const int W2 = 4 * g.w + 1, n = g.n;
+    LagCfg cO, cT; lagcol_config(g, p->plO.np, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.w, &cT);
+    const size_t qO = (size_t)cO.nsplit * p->plO.np * W2 * (g.Hx + 1), qT = (size_t)cT.nsplit * p->plT.np * L * (g.Hx + 1);
+    const size_t bO = (size_t)border_chunks() * p->plO.np * W2 * W2;
+    cudaError_t e = cudaSuccess;
+#define AL(ptr, cnt) if (e == cudaSuccess) e = dalloc(p, &ptr, (size_t)(cnt))
+    AL(p->tw, g.Nt);
+    AL(p->inter, (size_t)(DK + 1) * g.ny * g.Hx);
+    AL(p->specT, g.NK * plane);
+    AL(p->specS, plane);
+    AL(p->muR, (size_t)(DK + DB + 1) * ny);
+    AL(p->muS, (size_t)(DB + 1) * ny);
+    AL(p->Q, qO > qT ? qO : qT);
+    AL(p->lagO, (size_t)p->plO.np * W2 * W2);
+    AL(p->lagT, (size_t)g.NK * L * L);
+    AL(p->bpart, bO);
+    AL(p->gamA, (size_t)(DK + 1) * (DB + 1) * L * ny);
+    AL(p->gam, (size_t)g.NK * g.NB * L * L);
+    AL(p->phi, g.NB * g.NB);
+    AL(p->delta, g.NB);
+    AL(p->G, (size_t)n * n);
+    AL(p->h, n);
+    AL(p->Lf, (size_t)n * n);
+    AL(p->dscale, n);
+    AL(p->ywork, n);
+    AL(p->coef, n);
+    AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
+    AL(p->flag, 1);
+#undef AL
+    p->specTo = p->specT;
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&p->flag_host, sizeof(int));
+    if (e != cudaSuccess) {
+        const bool oom = (e == cudaErrorMemoryAllocation);
+        cudaGetLastError(); free_plan(p);
+        return oom ? SFFT_ERR_ALLOC : SFFT_ERR_CUDA;
+    }
+    *p->flag_host = 0;
+    for (int s = 0; s < SFFT_NUM_STAGES; s++) { cudaEventCreate(&p->ev0[s]); cudaEventCreate(&p->ev1[s]); }
+    p->stream = 0;
+    twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
+    // Phi (pin P7): closed form, mask independent
+    double phi[MAX_NP * MAX_NP];
+    for (int s = 0; s < g.NB; s++)
+        for (int s2 = 0; s2 < g.NB; s2++)
+            phi[s * g.NB + s2] = power_sum(nx, g.pi[s] + g.pi[s2]) * power_sum(ny, g.pj[s] + g.pj[s2]);
+    e = cudaMemcpy(p->phi, phi, sizeof(double) * g.NB * g.NB, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(p->flag, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { cudaGetLastError(); free_plan(p); return SFFT_ERR_CUDA; }
+    p->launches = 1;
+    *out = p;
+    return SFFT_OK;
+}
+
+sfft_status sfft_plan_set_stream(sfft_plan *p, void *cuda_stream) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    p->stream = (cudaStream_t)cuda_stream;
+    return SFFT_OK;
+}
+
+sfft_status sfft_plan_destroy(sfft_plan *p) {
+    if (!p) return SFFT_OK;
+    cudaStreamSynchronize(p->stream);
+    free_plan(p);
+    return SFFT_OK;
+}
+
+int sfft_num_unknowns(const sfft_plan *p) { return p ? p->g.n : 0; }
+size_t sfft_workspace_bytes(const sfft_plan *p) { return p ? p->bytes : 0; }
+long long sfft_launch_count(const sfft_plan *p) { return p ? p->launches : 0; }
+const char *sfft_last_error(const sfft_plan *p) { return p ? p->err : "null plan"; }
+
+} // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// stage sequencing
+// ------------------------------------------------------------------------------------------
+
+// a1 (template), Omega, Gamma, G.  Needs p->R, p->mask set.
+static sfft_status template_side(sfft_plan *p) {
+    const Geom &g = p->g;
+    {
+        StageTimer tm(p, SFFT_STAGE_A1_TEMPLATE);
+        if (p->mask && p->specTo == p->specT) { // the subtraction needs spectra of the UNMASKED template (C7)
+            CK(dalloc(p, &p->specTo, (size_t)g.NK * g.My * g.Hx), "alloc unmasked spectra");
+        }
+        if (p->mask) {
+            CK(launch_row_fwd(p, p->R, nullptr, p->inter, g.DK + 1, nullptr, 0), "row_fwd(R unmasked)");
+            CK(launch_col_fwd(p, p->inter, p->specTo, g.NK, g.pi, g.pj), "col_fwd(R unmasked)");
+        }
+        CK(launch_row_fwd(p, p->R, p->mask, p->inter, g.DK + 1, p->muR, g.DK + g.DB + 1), "row_fwd(R)");
+        CK(launch_col_fwd(p, p->inter, p->specT, g.NK, g.pi, g.pj), "col_fwd(R)");
+    }
+    {
+        StageTimer tm(p, SFFT_STAGE_A2_OMEGA);
+        CK(launch_lags(p, p->plO, 2 * g.w, p->lagO, false), "lags(Omega)");
+        CK(launch_gamma(p), "gamma");
+    }
+    {
+        StageTimer tm(p, SFFT_STAGE_A3_GATHER);
+        CK(launch_gather_G(p), "gather G");
+    }
+    return SFFT_OK;
+}
+
+// a1 (science), Theta, Delta, h.  Needs p->S (and p->R, p->mask of the template).
+static sfft_status science_side(sfft_plan *p) {
+    const Geom &g = p->g;
+    {
+        StageTimer tm(p, SFFT_STAGE_A1_SCIENCE);
+        const int i0 = 0, j0 = 0;
+        CK(launch_row_fwd(p, p->S, p->mask, p->inter, 1, p->muS, g.DB + 1), "row_fwd(S)");
+        CK(launch_col_fwd(p, p->inter, p->specS, 1, &i0, &j0), "col_fwd(S)");
+    }
+    {
+        StageTimer tm(p, SFFT_STAGE_A2_THETA);
+        CK(launch_lags(p, p->plT, g.w, p->lagT, true), "lags(Theta)");
+        CK(launch_delta(p), "delta");
+        CK(launch_gather_h(p), "gather h");
+    }
+    return SFFT_OK;
+}
+
+extern "C" {
+
+sfft_status sfft_build_system(sfft_plan *p, const double *S, const double *R, const uint8_t *mask) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!S || !R) return fail(p, SFFT_ERR_INVALID_ARG, "build_system: NULL image");
+    p->S = S; p->R = R; p->mask = mask;
+    p->have_template = p->have_system = p->have_factor = p->have_solution = false;
+    sfft_status st = template_side(p);
+    if (st != SFFT_OK) return st;
+    st = science_side(p);
+    if (st != SFFT_OK) return st;
+    p->have_template = true; p->have_system = true;
+    return SFFT_OK;
+}
+
+sfft_status sfft_solve(sfft_plan *p) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!p->have_system) return fail(p, SFFT_ERR_STATE, "solve before build_system");
+    if (!p->have_factor) {
+        StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
+        CK(launch_factor(p), "factor");
+        p->have_factor = true;
+    }
+    {
+        StageTimer tm(p, SFFT_STAGE_A4_SOLVE);
+        CK(launch_trisolve(p, p->h, p->coef), "trisolve");
+    }
+    p->have_solution = true;
+    return SFFT_OK;
+}
+
+sfft_status sfft_subtract(sfft_plan *p, double *D, double *coeffs) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!p->have_solution) return fail(p, SFFT_ERR_STATE, "subtract before solve");
+    if (!D) return fail(p, SFFT_ERR_INVALID_ARG, "subtract: NULL D");
+    {
+        StageTimer tm(p, SFFT_STAGE_A5_SUBTRACT);
+        CK(launch_subtract(p, p->S, p->R, p->coef, D), "subtract");
+    }
+    if (coeffs) CK(cudaMemcpyAsync(coeffs, p->coef, sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream), "copy coeffs");
+    return SFFT_OK;
+}
+
+sfft_status sfft_subtract_with(sfft_plan *p, const double *S, const double *coeffs_in, double *D) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!p->have_template) return fail(p, SFFT_ERR_STATE, "subtract_with before build_system/set_template");
+    if (!coeffs_in || !D) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_with: NULL pointer");
+    const double *Suse = S ? S : p->S;
+    if (!Suse) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_with: no science image");
+    StageTimer tm(p, SFFT_STAGE_A5_SUBTRACT);
+    CK(launch_subtract(p, Suse, p->R, coeffs_in, D), "subtract_with");
+    return SFFT_OK;
+}
+
+sfft_status sfft_set_template(sfft_plan *p, const double *R, const uint8_t *mask) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!R) return fail(p, SFFT_ERR_INVALID_ARG, "set_template: NULL image");
+    p->R = R; p->mask = mask; p->S = nullptr;
+    p->have_template = p->have_system = p->have_factor = p->have_solution = false;
+    sfft_status st = template_side(p);
+    if (st != SFFT_OK) return st;
+    {
+        StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
+        CK(launch_factor(p), "factor");
+    }
+    p->have_template = true; p->have_factor = true;
+    return SFFT_OK;
+}
+
+sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, double *const *D, double *coeffs) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!p->have_template || !p->have_factor) return fail(p, SFFT_ERR_STATE, "subtract_batch before set_template");
+    if (!S || !D || B < 1) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: bad arguments");
+    for (int b = 0; b < B; b++) if (!S[b] || !D[b]) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: NULL image");
+    for (int b = 0; b < B; b++) {
+        p->S = S[b];
+        sfft_status st = science_side(p);
+        if (st != SFFT_OK) return st;
+        p->have_system = true;
+        {
+            StageTimer tm(p, SFFT_STAGE_A4_SOLVE);
+            CK(launch_trisolve(p, p->h, p->coef), "trisolve");
+        }
+        p->have_solution = true;
+        {
+            StageTimer tm(p, SFFT_STAGE_A5_SUBTRACT);
+            CK(launch_subtract(p, p->S, p->R, p->coef, D[b]), "subtract");
+        }
+        if (coeffs)
+            CK(cudaMemcpyAsync(coeffs + (size_t)b * p->g.n, p->coef, sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream), "copy coeffs");
+    }
+    return SFFT_OK;
+}
+
+sfft_status sfft_sync_status(sfft_plan *p) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(p->stream), "sync");
+    if (p->have_factor) {
+        CK(cudaMemcpy(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost), "read flag");
+        if (*p->flag_host) return fail(p, SFFT_ERR_NOT_SPD, "pivot <= 1e-12: matrix not positive definite");
+    }
+    return SFFT_OK;
+}
+
+sfft_status sfft_difference_host(sfft_plan *p, const double *S_host, const double *R_host, const uint8_t *mask_host,
+                                 double *D_host, double *coeffs_host) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!S_host || !R_host || !D_host) return fail(p, SFFT_ERR_INVALID_ARG, "difference_host: NULL buffer");
+    const size_t npix = (size_t)p->g.nx * p->g.ny;
+    if (!p->stS) {
+        CK(dalloc(p, &p->stS, npix), "alloc staging"); CK(dalloc(p, &p->stR, npix), "alloc staging");
+        CK(dalloc(p, &p->stD, npix), "alloc staging");
+    }
+    if (mask_host && !p->stM) CK(dalloc(p, &p->stM, npix), "alloc staging");
+    CK(cudaMemcpyAsync(p->stS, S_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->stream), "H2D S");
+    CK(cudaMemcpyAsync(p->stR, R_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->stream), "H2D R");
+    if (mask_host) CK(cudaMemcpyAsync(p->stM, mask_host, npix, cudaMemcpyHostToDevice, p->stream), "H2D mask");
+    sfft_status st = sfft_build_system(p, p->stS, p->stR, mask_host ? p->stM : nullptr);
+    if (st == SFFT_OK) st = sfft_solve(p);
+    if (st == SFFT_OK) st = sfft_subtract(p, p->stD, nullptr);
+    if (st != SFFT_OK) return st;
+    CK(cudaMemcpyAsync(D_host, p->stD, npix * sizeof(double), cudaMemcpyDeviceToHost, p->stream), "D2H D");
+    if (coeffs_host) CK(cudaMemcpyAsync(coeffs_host, p->coef, sizeof(double) * p->g.n, cudaMemcpyDeviceToHost, p->stream), "D2H coeffs");
+    return sfft_sync_status(p);
+}
+
+} // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// introspection
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+sfft_status sfft_get_system(const sfft_plan *pc, double *G, double *h) {
+    sfft_plan *p = const_cast<sfft_plan *>(pc);
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!p->have_template) return fail(p, SFFT_ERR_STATE, "get_system: nothing built yet");
+    const size_t n = p->g.n;
+    if (G) CK(cudaMemcpyAsync(G, p->G, n * n * sizeof(double), cudaMemcpyDeviceToDevice, p->stream), "copy G");
+    if (h) {
+        if (!p->have_system) return fail(p, SFFT_ERR_STATE, "get_system: no right-hand side yet");
+        CK(cudaMemcpyAsync(h, p->h, n * sizeof(double), cudaMemcpyDeviceToDevice, p->stream), "copy h");
+    }
+    return SFFT_OK;
+}
+
+sfft_status sfft_enable_timings(sfft_plan *p, int on) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    p->timing = on != 0;
+    for (int s = 0; s < SFFT_NUM_STAGES; s++) p->ev_used[s] = false;
+    return SFFT_OK;
+}
+
+sfft_status sfft_get_timings(sfft_plan *p, float *ms, int n_stages) {
+    if (!p || !ms || n_stages < 0) return SFFT_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(p->stream), "sync");
+    for (int s = 0; s < n_stages; s++) {
+        ms[s] = 0.0f;
+        if (s < SFFT_NUM_STAGES && p->ev_used[s]) {
+            float t = 0.0f;
+            if (cudaEventElapsedTime(&t, p->ev0[s], p->ev1[s]) == cudaSuccess) ms[s] = t; else cudaGetLastError();
+        }
+    }
+    return SFFT_OK;
+}
+
+sfft_status sfft_debug_read(sfft_plan *p, int which, int idx, void *host_dst, size_t nbytes) {
+    if (!p || !host_dst) return SFFT_ERR_INVALID_ARG;
+    const Geom &g = p->g;
+    const size_t plane = (size_t)g.My * g.Hx * sizeof(cplx);
+    const int W2 = 4 * g.w + 1, LL = g.L * g.L;
+    const void *src = nullptr; size_t sz = 0;
+    double dims[2] = {(double)g.Mx, (double)g.My};
+    switch (which) {
+    case 0: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->specT + (size_t)idx * g.My * g.Hx; sz = plane; break;
+    case 1: src = p->specS; sz = plane; break;
+    case 2: if (idx < 0 || idx >= p->npairsO) return SFFT_ERR_INVALID_ARG; src = p->lagO + (size_t)idx * W2 * W2; sz = sizeof(double) * W2 * W2; break;
+    case 3: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->lagT + (size_t)idx * LL; sz = sizeof(double) * LL; break;
+    case 4: src = p->gam; sz = sizeof(double) * g.NK * g.NB * LL; break;
+    case 5: src = p->phi; sz = sizeof(double) * g.NB * g.NB; break;
+    case 6: src = p->delta; sz = sizeof(double) * g.NB; break;
+    case 7: if (nbytes != sizeof(dims)) return SFFT_ERR_INVALID_ARG; memcpy(host_dst, dims, sizeof(dims)); return SFFT_OK;
+    default: return SFFT_ERR_INVALID_ARG;
+    }
+    if (nbytes != sz) return fail(p, SFFT_ERR_INVALID_ARG, "debug_read: size mismatch");
+    CK(cudaStreamSynchronize(p->stream), "sync");
+    CK(cudaMemcpy(host_dst, src, sz, cudaMemcpyDeviceToHost), "debug copy");
+    return SFFT_OK;
+}
+
+sfft_status sfft_probe_fp64(int kind, int iters, double *tflops) {
+    if (!tflops || iters < 1 || kind < 0 || kind > 1) return SFFT_ERR_INVALID_ARG;
+    return run_probe_fp64(kind, iters, tflops) == cudaSuccess ? SFFT_OK : SFFT_ERR_CUDA;
+}
+
+} // extern "C"

@@ -60,8 +60,9 @@ __global__ void __launch_bounds__(256) potrf_kernel(double *__restrict__ Lf, int
 
 // panel: rows below the diagonal block, X L_kk^T = A.  grid = ceil(rows/64), block 64 (one row each)
 __global__ void __launch_bounds__(CB) trsm_kernel(double *__restrict__ Lf, int n, int k0, int bs) {
-    __shared__ double l[CB][CB + 1];
-    __shared__ double x[CB][CB + 1];
+    extern __shared__ __align__(16) double dsm[];
+    double (*l)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm);
+    double (*x)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm + CB * (CB + 1));
     const int r0 = k0 + bs + blockIdx.x * CB;
     for (int e = threadIdx.x; e < bs * bs; e += blockDim.x) l[e / bs][e % bs] = Lf[(size_t)(k0 + e / bs) * n + k0 + e % bs];
     for (int e = threadIdx.x; e < CB * bs; e += blockDim.x) {
@@ -90,8 +91,9 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
 // trailing update: for block rows bi >= bj > kb:  A[bi][bj] -= X_bi X_bj^T,  X = panel columns k0..k0+bs.
 // grid = ntile*(ntile+1)/2 lower-triangular tile pairs; block 256 = 8 warps, warp tile 16 x 32.
 __global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int n, int k0, int bs, int t0 /*first trailing row*/) {
-    __shared__ double As[CB][CLD];
-    __shared__ double Bs[CB][CLD];
+    extern __shared__ __align__(16) double dsm[];
+    double (*As)[CLD] = reinterpret_cast<double (*)[CLD]>(dsm);
+    double (*Bs)[CLD] = reinterpret_cast<double (*)[CLD]>(dsm + CB * CLD);
     // linear index -> (bi, bj), bj <= bi
     int idx = blockIdx.x, bi = 0;
     while (idx > bi) { idx -= bi + 1; bi++; }
@@ -215,6 +217,9 @@ cudaError_t launch_factor(sfft_plan *p) {
     equil_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p->G, p->dscale, p->Lf, n);
     p->launches += 2;
     const int nblk = (n + CB - 1) / CB;
+    const size_t sm_trsm = 2 * CB * (CB + 1) * sizeof(double), sm_syrk = 2 * CB * CLD * sizeof(double);
+    cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_trsm);
+    cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
         potrf_kernel<<<1, 256, 0, st>>>(p->Lf, n, k0, bs, p->flag);
@@ -222,8 +227,8 @@ cudaError_t launch_factor(sfft_plan *p) {
         const int rem = n - k0 - bs;
         if (rem > 0) {
             const int nt = (rem + CB - 1) / CB;
-            trsm_kernel<<<nt, CB, 0, st>>>(p->Lf, n, k0, bs);
-            syrk_kernel<<<nt * (nt + 1) / 2, 256, 0, st>>>(p->Lf, n, k0, bs, k0 + bs);
+            trsm_kernel<<<nt, CB, sm_trsm, st>>>(p->Lf, n, k0, bs);
+            syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs);
             p->launches += 2;
         }
     }

@@ -1,0 +1,249 @@
+"""ctypes binding of libsfft.so (include/sfft.h) -- argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; torch is used for device
+memory and streams, nothing else.  There is no CPU fallback: a missing library or a
+missing CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import torch
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libsfft.so"
+
+OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_STATE, ERR_NOT_SPD = 0, -1, -2, -3, -4, -5
+STAGES = ("a1_template", "a1_science", "a2_omega", "a2_theta", "a3_gather", "a4_factor",
+          "a4_solve", "a5_subtract")
+_STATUS = {0: "OK", -1: "INVALID_ARG", -2: "ALLOC", -3: "CUDA", -4: "STATE", -5: "NOT_SPD"}
+
+# every symbol include/sfft.h declares (tests check the library exports all of them)
+SYMBOLS = (
+    "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
+    "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_with",
+    "sfft_set_template", "sfft_subtract_batch", "sfft_difference_host", "sfft_sync_status",
+    "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_launch_count",
+    "sfft_last_error", "sfft_version", "sfft_debug_read", "sfft_probe_fp64",
+)
+
+
+class SfftError(RuntimeError):
+    def __init__(self, code, where, detail=""):
+        super().__init__(f"{where}: SFFT_ERR_{_STATUS.get(code, code)} {detail}".strip())
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libsfft.so (built by paper_2509_18544_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise FileNotFoundError(
+            f"{LIB_PATH} not found: run `python -m paper_2509_18544_b200.build` (no CPU fallback exists)")
+    lib = ctypes.CDLL(str(LIB_PATH))
+    vp, ci, dp = ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p
+    lib.sfft_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci]
+    lib.sfft_plan_set_stream.argtypes = [vp, vp]
+    lib.sfft_plan_destroy.argtypes = [vp]
+    lib.sfft_num_unknowns.argtypes = [vp]
+    lib.sfft_workspace_bytes.argtypes = [vp]
+    lib.sfft_workspace_bytes.restype = ctypes.c_size_t
+    lib.sfft_build_system.argtypes = [vp, dp, dp, dp]
+    lib.sfft_solve.argtypes = [vp]
+    lib.sfft_subtract.argtypes = [vp, dp, dp]
+    lib.sfft_subtract_with.argtypes = [vp, dp, dp, dp]
+    lib.sfft_set_template.argtypes = [vp, dp, dp]
+    lib.sfft_subtract_batch.argtypes = [vp, ctypes.POINTER(vp), ci, ctypes.POINTER(vp), dp]
+    lib.sfft_difference_host.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.sfft_sync_status.argtypes = [vp]
+    lib.sfft_get_system.argtypes = [vp, dp, dp]
+    lib.sfft_enable_timings.argtypes = [vp, ci]
+    lib.sfft_get_timings.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ci]
+    lib.sfft_launch_count.argtypes = [vp]
+    lib.sfft_launch_count.restype = ctypes.c_longlong
+    lib.sfft_last_error.argtypes = [vp]
+    lib.sfft_last_error.restype = ctypes.c_char_p
+    lib.sfft_version.restype = ctypes.c_char_p
+    lib.sfft_debug_read.argtypes = [vp, ci, ci, vp, ctypes.c_size_t]
+    lib.sfft_probe_fp64.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
+    _lib = lib
+    return lib
+
+
+def version() -> str:
+    return load_library().sfft_version().decode()
+
+
+def probe_fp64(kind: int, iters: int = 4096) -> float:
+    """Measured FP64 rate in TFLOP/s: kind 0 = DFMA, 1 = DMMA m8n8k4."""
+    out = ctypes.c_double()
+    rc = load_library().sfft_probe_fp64(kind, iters, ctypes.byref(out))
+    if rc:
+        raise SfftError(rc, "sfft_probe_fp64")
+    return out.value
+
+
+def _dev_f64(t, shape, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name}: need a contiguous CUDA float64 tensor")
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+    return t.data_ptr()
+
+
+def _dev_mask(m, shape):
+    if m is None:
+        return None
+    if not (isinstance(m, torch.Tensor) and m.is_cuda and m.dtype == torch.uint8 and m.is_contiguous()):
+        raise TypeError("mask: need a contiguous CUDA uint8 tensor")
+    if tuple(m.shape) != tuple(shape):
+        raise ValueError("mask: shape mismatch")
+    return m.data_ptr()
+
+
+class SfftPlan:
+    """sfft_plan_create(nx, ny, L, DK, DB) and the calls on it; same names as the C ABI."""
+
+    def __init__(self, nx, ny, L, DK, DB, stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("libsfft needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._lib = load_library()
+        self._h = ctypes.c_void_p()
+        rc = self._lib.sfft_plan_create(ctypes.byref(self._h), nx, ny, L, DK, DB)
+        if rc:
+            self._h = None
+            raise SfftError(rc, "sfft_plan_create")
+        self.nx, self.ny, self.L, self.DK, self.DB = nx, ny, L, DK, DB
+        self.shape = (ny, nx)
+        self.n = self._lib.sfft_num_unknowns(self._h)
+        self._keep = []
+        self.set_stream(stream if stream is not None else torch.cuda.current_stream())
+
+    # -- life cycle ---------------------------------------------------------------------
+    def set_stream(self, stream):
+        self._stream = stream
+        self._ck(self._lib.sfft_plan_set_stream(self._h, ctypes.c_void_p(stream.cuda_stream)), "sfft_plan_set_stream")
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.sfft_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def _ck(self, rc, where):
+        if rc:
+            raise SfftError(rc, where, self._lib.sfft_last_error(self._h).decode())
+
+    @property
+    def workspace_bytes(self):
+        return self._lib.sfft_workspace_bytes(self._h)
+
+    @property
+    def launch_count(self):
+        return self._lib.sfft_launch_count(self._h)
+
+    # -- single pair ----------------------------------------------------------------------
+    def build_system(self, S, R, mask=None):
+        sp, rp, mp = _dev_f64(S, self.shape, "S"), _dev_f64(R, self.shape, "R"), _dev_mask(mask, self.shape)
+        self._keep = [S, R, mask]  # the plan keeps the pointers until subtract
+        self._ck(self._lib.sfft_build_system(self._h, sp, rp, mp), "sfft_build_system")
+
+    def solve(self):
+        self._ck(self._lib.sfft_solve(self._h), "sfft_solve")
+
+    def subtract(self, D=None, coeffs=None):
+        if D is None:
+            D = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        if coeffs is None:
+            coeffs = torch.empty(self.n, dtype=torch.float64, device="cuda")
+        self._ck(self._lib.sfft_subtract(self._h, _dev_f64(D, self.shape, "D"), _dev_f64(coeffs, (self.n,), "coeffs")),
+                 "sfft_subtract")
+        return D, coeffs
+
+    def subtract_with(self, coeffs_in, S=None, D=None):
+        if D is None:
+            D = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        sp = _dev_f64(S, self.shape, "S") if S is not None else None
+        self._ck(self._lib.sfft_subtract_with(self._h, sp, _dev_f64(coeffs_in, (self.n,), "coeffs_in"),
+                                              _dev_f64(D, self.shape, "D")), "sfft_subtract_with")
+        return D
+
+    # -- batched --------------------------------------------------------------------------
+    def set_template(self, R, mask=None):
+        rp, mp = _dev_f64(R, self.shape, "R"), _dev_mask(mask, self.shape)
+        self._keep = [R, mask]
+        self._ck(self._lib.sfft_set_template(self._h, rp, mp), "sfft_set_template")
+
+    def subtract_batch(self, S_list, D_list=None, coeffs=None):
+        B = len(S_list)
+        if D_list is None:
+            D_list = [torch.empty(self.shape, dtype=torch.float64, device="cuda") for _ in range(B)]
+        if coeffs is None:
+            coeffs = torch.empty((B, self.n), dtype=torch.float64, device="cuda")
+        Sp = (ctypes.c_void_p * B)(*[_dev_f64(s, self.shape, "S[b]") for s in S_list])
+        Dp = (ctypes.c_void_p * B)(*[_dev_f64(d, self.shape, "D[b]") for d in D_list])
+        self._ck(self._lib.sfft_subtract_batch(self._h, Sp, B, Dp, _dev_f64(coeffs, (B, self.n), "coeffs")),
+                 "sfft_subtract_batch")
+        return D_list, coeffs
+
+    # -- host buffers (end to end) ----------------------------------------------------------
+    def difference_host(self, S_host, R_host, mask_host=None, D_host=None, coeffs_host=None):
+        """S_host, R_host: CPU float64 tensors (pinned for full copy speed).  Synchronises."""
+        for t, nm in ((S_host, "S_host"), (R_host, "R_host")):
+            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != self.shape:
+                raise TypeError(f"{nm}: need a contiguous CPU float64 tensor of shape {self.shape}")
+        if D_host is None:
+            D_host = torch.empty(self.shape, dtype=torch.float64).pin_memory()
+        if coeffs_host is None:
+            coeffs_host = torch.empty(self.n, dtype=torch.float64)
+        mp = mask_host.data_ptr() if mask_host is not None else None
+        self._ck(self._lib.sfft_difference_host(self._h, S_host.data_ptr(), R_host.data_ptr(), mp,
+                                                D_host.data_ptr(), coeffs_host.data_ptr()), "sfft_difference_host")
+        return D_host, coeffs_host
+
+    # -- introspection ---------------------------------------------------------------------
+    def sync_status(self):
+        self._ck(self._lib.sfft_sync_status(self._h), "sfft_sync_status")
+
+    def get_system(self, want_h=True):
+        G = torch.empty((self.n, self.n), dtype=torch.float64, device="cuda")
+        h = torch.empty(self.n, dtype=torch.float64, device="cuda") if want_h else None
+        self._ck(self._lib.sfft_get_system(self._h, G.data_ptr(), h.data_ptr() if want_h else None), "sfft_get_system")
+        return G, h
+
+    def enable_timings(self, on=True):
+        self._ck(self._lib.sfft_enable_timings(self._h, 1 if on else 0), "sfft_enable_timings")
+
+    def get_timings(self):
+        ms = (ctypes.c_float * len(STAGES))()
+        self._ck(self._lib.sfft_get_timings(self._h, ms, len(STAGES)), "sfft_get_timings")
+        return dict(zip(STAGES, [float(v) for v in ms]))
+
+    def debug_read(self, which, idx=0):
+        import numpy as np
+        dims = np.zeros(2)
+        self._ck(self._lib.sfft_debug_read(self._h, 7, 0, dims.ctypes.data_as(ctypes.c_void_p), 16), "sfft_debug_read")
+        Mx, My = int(dims[0]), int(dims[1])
+        if which == 7:
+            return Mx, My
+        w, L = (self.L - 1) // 2, self.L
+        NK, NB = (self.DK + 1) * (self.DK + 2) // 2, (self.DB + 1) * (self.DB + 2) // 2
+        shapes = {0: ((My, Mx // 2), np.complex128), 1: ((My, Mx // 2), np.complex128),
+                  2: ((4 * w + 1, 4 * w + 1), np.float64), 3: ((L, L), np.float64),
+                  4: ((NK, NB, L, L), np.float64), 5: ((NB, NB), np.float64), 6: ((NB,), np.float64)}
+        shp, dt = shapes[which]
+        out = np.zeros(shp, dtype=dt)
+        self._ck(self._lib.sfft_debug_read(self._h, which, idx, out.ctypes.data_as(ctypes.c_void_p), out.nbytes),
+                 "sfft_debug_read")
+        return out
