@@ -103,8 +103,12 @@ __global__ void gather_G_kernel(const double *__restrict__ lagO, const double *_
     if (r < NKLL && c < NKLL) {
         const int t = r / LL, v = (r % LL) / L - w, u = (r % LL) % L - w;
         const int tp = c / LL, vp = (c % LL) / L - w, up = (c % LL) % L - w;
-        if (t <= tp) val = lagO[(size_t)pair_index(t, tp, g.NK) * W2 * W2 + (v - vp + 2 * w) * W2 + (u - up + 2 * w)];
-        else val = lagO[(size_t)pair_index(tp, t, g.NK) * W2 * W2 + (vp - v + 2 * w) * W2 + (up - u + 2 * w)];
+        // X(b,a)[d] = X(a,b)[-d] (pin P11): every entry and its transpose read the SAME table slot, so G is
+        // symmetric bit for bit (for t == t' the slot with the lexicographically non-negative lag is used)
+        int dv = v - vp, du = u - up;
+        const bool flip = t > tp || (t == tp && (dv < 0 || (dv == 0 && du < 0)));
+        if (flip) { dv = -dv; du = -du; }
+        val = lagO[(size_t)pair_index(flip ? tp : t, flip ? t : tp, g.NK) * W2 * W2 + (dv + 2 * w) * W2 + (du + 2 * w)];
     } else if (r < NKLL) {
         val = gam[((size_t)(r / LL) * g.NB + (c - NKLL)) * LL + r % LL];
     } else if (c < NKLL) {

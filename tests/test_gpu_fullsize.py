@@ -1,0 +1,122 @@
+"""GPU parity at BASELINE.json's full sizes (4088 x 4088), in the launch configuration bench.py
+times.  configs[2] is compared element by element with the full oracle; configs[3] (batch) and
+configs[4] (n = 4416) on sampled outputs the oracle computes one by one (system entries by direct
+pixel summation, difference-image pixels by real-space convolution), on the solver alone against
+the oracle's textbook Cholesky of the same matrix, and on the normal-equation invariant P8."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2509_18544_b200 import SfftPlan, starfield
+from test_gpu_parity import TOL_C, TOL_D, TOL_G, TOL_H, assert_coeffs, assert_system, dev
+
+pytestmark = pytest.mark.gpu
+
+
+def sampled_system_check(S, R, L, DK, DB, G, h, rng, nsamp):
+    n = G.shape[0]
+    work = np.empty(3 * S.size)
+    diag = {}
+
+    def gdiag(i):
+        if i not in diag:
+            diag[i] = oracle.system_entry(S, R, None, L, DK, DB, i, i, work)
+        return diag[i]
+
+    nS = np.linalg.norm(S)
+    # spread over kernel-kernel, kernel-background, background-background blocks and the diagonal
+    pairs = [(int(rng.integers(n)), int(rng.integers(n))) for _ in range(nsamp)]
+    pairs += [(n - 1, n - 1), (0, n - 1), (n - 2, 0), (0, 0), (n // 2, n // 2)]
+    for r, c in pairs:
+        ref = oracle.system_entry(S, R, None, L, DK, DB, r, c, work)
+        assert abs(G[r, c] - ref) <= TOL_G * np.sqrt(gdiag(r) * gdiag(c)), (r, c)
+    for r in [int(rng.integers(n)) for _ in range(nsamp // 2)] + [0, n - 1]:
+        ref = oracle.system_entry(S, R, None, L, DK, DB, r, -1, work)
+        assert abs(h[r] - ref) <= TOL_H * np.sqrt(gdiag(r)) * nS, r
+
+
+def sampled_D_check(S, R, L, DK, DB, c, D, rng, noise_rms, nsamp=400):
+    ny, nx = S.shape
+    w = (L - 1) // 2
+    xs = rng.integers(0, nx, nsamp); ys = rng.integers(0, ny, nsamp)
+    # force the frame border and corners in (native-grid wrap path)
+    xs[:8] = [0, nx - 1, 0, nx - 1, w - 1, nx - w, nx // 2, 3]
+    ys[:8] = [0, 0, ny - 1, ny - 1, ny // 2, 5, ny - 1, w]
+    ref = oracle.subtract_at(S, R, L, DK, DB, c, xs, ys)
+    assert np.max(np.abs(D[ys, xs] - ref)) <= TOL_D * noise_rms
+
+
+def normal_equation_residual(S, R, L, DK, DB, D):
+    """Pin P8 on the GPU output: A^T D = 0, via numpy FFT cross-correlations (a property check)."""
+    ny, nx = S.shape
+    w = (L - 1) // 2
+    FD = np.fft.rfft2(D)
+    worst = 0.0
+    for t in range((DK + 1) * (DK + 2) // 2):
+        i, j = oracle.poly_index(t)
+        T = oracle.weighted_image(R, None, i, j)
+        X = np.fft.irfft2(np.conj(np.fft.rfft2(T)) * FD, s=D.shape)
+        lags = np.concatenate([X[:w + 1, :w + 1].ravel(), X[:w + 1, -w:].ravel(), X[-w:, :w + 1].ravel(), X[-w:, -w:].ravel()])
+        worst = max(worst, np.max(np.abs(lags)) / (np.linalg.norm(T) * np.linalg.norm(S)))
+    return worst
+
+
+def test_config2_full_roman_size():
+    cfg = starfield.make_pair(2)
+    S, R, L, DK, DB = cfg["S"], cfg["R"], cfg["L"], cfg["DK"], cfg["DB"]
+    p = SfftPlan(4088, 4088, L, DK, DB)
+    dS, dR = dev(S), dev(R)
+    p.build_system(dS, dR)
+    G, h = p.get_system()
+    p.solve()
+    D, c = p.subtract()
+    p.sync_status()
+    G, h, c, D = G.cpu().numpy(), h.cpu().numpy(), c.cpu().numpy(), D.cpu().numpy()
+    G0, h0 = oracle.build_system(S, R, None, L, DK, DB)
+    assert_system(G, h, G0, h0, S)
+    c0 = oracle.solve(G0, h0)
+    assert_coeffs(c, c0, L * L * 6)
+    D0 = oracle.subtract(S, R, L, DK, DB, c0)
+    assert np.max(np.abs(D - D0)) <= TOL_D * cfg["noise_rms"]
+    assert normal_equation_residual(S, R, L, DK, DB, D) <= 1e-12
+    # configs[3] at full size: the same template against 3 science images, template work once
+    p.set_template(dR)
+    Ss = [S if b == 0 else starfield.make_batch_science(cfg, b) for b in range(3)]
+    Ds, cs = p.subtract_batch([dS] + [dev(s) for s in Ss[1:]])
+    p.sync_status()
+    cs = cs.cpu().numpy()
+    assert np.array_equal(cs[0], c) and np.array_equal(Ds[0].cpu().numpy(), D)
+    rng = np.random.default_rng(77)
+    for b in (1, 2):
+        Db = Ds[b].cpu().numpy()
+        sampled_D_check(Ss[b], R, L, DK, DB, cs[b], Db, rng, cfg["noise_rms"])
+        assert normal_equation_residual(Ss[b], R, L, DK, DB, Db) <= 1e-12
+        work = np.empty(3 * S.size)
+        hb = np.array([oracle.system_entry(Ss[b], R, None, L, DK, DB, r, -1, work) for r in (0, 60, 300, 731)])
+        # c solves G c = h_b: check four rows of the normal equations with the oracle's G and direct-sum h
+        assert np.all(np.abs(G0[[0, 60, 300, 731]] @ cs[b] - hb) <= 1e-9 * np.sqrt(np.diag(G0)[[0, 60, 300, 731]]) * np.linalg.norm(Ss[b]))
+    p.destroy()
+
+
+def test_config4_large_kernel():
+    cfg = starfield.make_pair(4)
+    S, R, L, DK, DB = cfg["S"], cfg["R"], cfg["L"], cfg["DK"], cfg["DB"]
+    p = SfftPlan(4088, 4088, L, DK, DB)
+    assert p.n == 4416
+    dS, dR = dev(S), dev(R)
+    p.build_system(dS, dR)
+    G, h = p.get_system()
+    p.solve()
+    D, c = p.subtract()
+    p.sync_status()
+    G, h, c, D = G.cpu().numpy(), h.cpu().numpy(), c.cpu().numpy(), D.cpu().numpy()
+    assert np.array_equal(G, G.T)
+    rng = np.random.default_rng(99)
+    sampled_system_check(S, R, L, DK, DB, G, h, rng, nsamp=40)
+    # the solver alone: oracle's textbook Cholesky on the same matrix
+    c0 = oracle.solve(G, h)
+    assert_coeffs(c, c0, L * L * 10)
+    sampled_D_check(S, R, L, DK, DB, c, D, rng, cfg["noise_rms"], nsamp=300)
+    assert normal_equation_residual(S, R, L, DK, DB, D) <= 1e-12
+    p.destroy()

@@ -1,0 +1,190 @@
+"""GPU parity: libsfft (through the C ABI binding) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json north_star's, in the norm-wise form of
+DESIGN.md readings C12/C13:
+   G:  |dG_ij| <= 1e-10 sqrt(G_ii G_jj);   h: |dh_i| <= 1e-10 sqrt(G_ii) ||m.S||_2
+   c:  max|da| <= 1e-8 max|a| (kernel block), max|db| <= 1e-8 max|b| (background block)
+   D:  max|dD| <= 1e-6 * noise RMS of the science image
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2509_18544_b200 import SfftError, SfftPlan, starfield
+
+pytestmark = pytest.mark.gpu
+
+TOL_G, TOL_H, TOL_C, TOL_D = 1e-10, 1e-10, 1e-8, 1e-6
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(S, R, mask, L, DK, DB):
+    ny, nx = S.shape
+    p = SfftPlan(nx, ny, L, DK, DB)
+    dS, dR = dev(S), dev(R)
+    dM = dev(mask) if mask is not None else None
+    p.build_system(dS, dR, dM)
+    G, h = p.get_system()
+    p.solve()
+    D, c = p.subtract()
+    p.sync_status()
+    return p, G.cpu().numpy(), h.cpu().numpy(), c.cpu().numpy(), D.cpu().numpy()
+
+
+def assert_system(G, h, G0, h0, Sf):
+    d = np.sqrt(np.diag(G0))
+    assert np.all(np.abs(G - G0) <= TOL_G * np.outer(d, d)), np.max(np.abs(G - G0) / np.outer(d, d))
+    assert np.all(np.abs(h - h0) <= TOL_H * d * np.linalg.norm(Sf)), np.max(np.abs(h - h0) / (d * np.linalg.norm(Sf)))
+    assert np.array_equal(G, G.T)
+
+
+def assert_coeffs(c, c0, nker):
+    assert np.max(np.abs(c - c0)[:nker]) <= TOL_C * np.max(np.abs(c0[:nker]))
+    assert np.max(np.abs(c - c0)[nker:]) <= TOL_C * np.max(np.abs(c0[nker:]))
+
+
+def full_parity(S, R, mask, L, DK, DB, noise_rms):
+    p, G, h, c, D = run_gpu(S, R, mask, L, DK, DB)
+    G0, h0 = oracle.build_system(S, R, mask, L, DK, DB)
+    Sf = S * mask if mask is not None else S
+    assert_system(G, h, G0, h0, Sf)
+    c0 = oracle.solve(G0, h0)
+    nker = L * L * (DK + 1) * (DK + 2) // 2
+    assert_coeffs(c, c0, nker)
+    D0 = oracle.subtract(S, R, L, DK, DB, c0)
+    assert np.max(np.abs(D - D0)) <= TOL_D * noise_rms
+    # convolution alone (oracle coefficients through the GPU subtract), reading C13
+    D1 = p.subtract_with(dev(c0)).cpu().numpy()
+    assert np.max(np.abs(D1 - D0)) <= TOL_D * noise_rms
+    p.destroy()
+    return c, D
+
+
+# sizes spanning several FFT tiles and ragged tails: powers of two (no padding), non powers of two
+# (zero padding + native-grid wrap corrections), nx != ny, odd sizes, every polynomial degree.
+@pytest.mark.parametrize("nx,ny,L,DK,DB,masked", [
+    (128, 64, 5, 1, 1, False),
+    (100, 72, 5, 1, 1, False),
+    (100, 72, 5, 2, 2, True),
+    (61, 67, 7, 0, 0, False),
+    (90, 130, 3, 3, 3, False),
+    (200, 120, 9, 1, 2, True),
+    (64, 64, 1, 2, 1, False),
+    (257, 129, 5, 2, 0, False),
+])
+def test_parity_small(nx, ny, L, DK, DB, masked):
+    S, R = starfield.random_pair(nx, ny, seed=nx * 7 + ny)
+    mask = None
+    if masked:
+        rng = np.random.default_rng(5)
+        mask = (rng.random((ny, nx)) > 0.05).astype(np.uint8)
+        yy, xx = np.mgrid[:ny, :nx]
+        mask[(yy - ny // 3) ** 2 + (xx - nx // 2) ** 2 < 36] = 0  # a masked disc
+    full_parity(S, R, mask, L, DK, DB, noise_rms=20.0)
+
+
+def test_minimum_frame_size():
+    L = 5
+    S, R = starfield.random_pair(2 * L - 1, 2 * L - 1, seed=3)
+    full_parity(S, R, None, L, 0, 0, noise_rms=20.0)
+
+
+def test_config0_tiny():
+    c = starfield.make_pair(0)
+    full_parity(c["S"], c["R"], None, c["L"], c["DK"], c["DB"], c["noise_rms"])
+
+
+def test_config1_mid():
+    c = starfield.make_pair(1)
+    full_parity(c["S"], c["R"], None, c["L"], c["DK"], c["DB"], c["noise_rms"])
+
+
+def test_config2_recipe_reduced_non_pow2():
+    """configs[2]'s recipe (elliptical PSFs, deeper template, transients) at 511 x 389."""
+    c = starfield.make_pair(2, nx=511, ny=389, n_stars=1000)
+    full_parity(c["S"], c["R"], None, 11, 2, 2, c["noise_rms"])
+
+
+def test_P2_identity_on_gpu():
+    _, R = starfield.random_pair(96, 80, seed=11)
+    p, G, h, c, D = run_gpu(R, R, None, 5, 1, 1)
+    e = np.zeros_like(c); e[2 * 5 + 2] = 1.0
+    assert np.max(np.abs(c - e)) < 1e-9
+    assert np.max(np.abs(D)) < 1e-8
+
+
+def test_P5_pure_shift_on_gpu():
+    _, R = starfield.random_pair(100, 72, seed=12)
+    S = np.roll(R, (2, -1), axis=(0, 1))  # S(x,y) = R(x+1, y-2): delta at (u,v) = (-1, 2)
+    p, G, h, c, D = run_gpu(S, R, None, 5, 0, 0)
+    k = c[:25].reshape(5, 5)
+    assert abs(k[2 + 2, 2 - 1] - 1.0) < 1e-9 and np.abs(D).max() < 1e-8
+
+
+def test_not_spd_is_reported():
+    R = np.full((64, 64), 3.0)
+    S, _ = starfield.random_pair(64, 64, seed=1)
+    p = SfftPlan(64, 64, 3, 1, 0)
+    p.build_system(dev(S), dev(R))
+    p.solve()
+    with pytest.raises(SfftError) as ei:
+        p.sync_status()
+    assert ei.value.code == -5
+    with pytest.raises(oracle.OracleError):
+        G0, h0 = oracle.build_system(S, R, None, 3, 1, 0)
+        oracle.solve(G0, h0)
+
+
+def test_state_and_argument_errors():
+    with pytest.raises(SfftError):
+        SfftPlan(64, 64, 4, 0, 0)       # even L
+    with pytest.raises(SfftError):
+        SfftPlan(8, 64, 5, 0, 0)        # nx < 2L-1
+    with pytest.raises(SfftError):
+        SfftPlan(64, 64, 3, 4, 0)       # DK out of range
+    p = SfftPlan(64, 64, 3, 0, 0)
+    with pytest.raises(SfftError) as ei:
+        p.solve()
+    assert ei.value.code == -4
+    with pytest.raises(SfftError):
+        p.subtract()
+    with pytest.raises(SfftError):
+        p.subtract_batch([torch.zeros(64, 64, dtype=torch.float64, device="cuda")])
+    with pytest.raises(TypeError):
+        p.build_system(torch.zeros(64, 64), torch.zeros(64, 64))
+
+
+def test_batched_matches_single_and_oracle():
+    """configs[3]'s structure at reduced size: one template, B science images; template-side work
+    once.  Each image must match the single-pair path bit for bit and the oracle to tolerance."""
+    t = starfield.make_pair(3, nx=300, ny=260, n_stars=600)
+    B, L, DK, DB = 3, 11, 2, 2
+    Ss = [t["S"]] + [starfield.make_batch_science(t, b) for b in range(1, B)]
+    p = SfftPlan(300, 260, L, DK, DB)
+    dR = dev(t["R"]); dSs = [dev(s) for s in Ss]
+    p.set_template(dR)
+    Ds, cs = p.subtract_batch(dSs)
+    p.sync_status()
+    cs = cs.cpu().numpy()
+    for b in range(B):
+        p1, G, h, c, D = run_gpu(Ss[b], t["R"], None, L, DK, DB)
+        assert np.array_equal(c, cs[b]) and np.array_equal(D, Ds[b].cpu().numpy())
+        G0, h0 = oracle.build_system(Ss[b], t["R"], None, L, DK, DB)
+        c0 = oracle.solve(G0, h0)
+        assert_coeffs(cs[b], c0, L * L * 6)
+        D0 = oracle.subtract(Ss[b], t["R"], L, DK, DB, c0)
+        assert np.max(np.abs(Ds[b].cpu().numpy() - D0)) <= TOL_D * t["noise_rms"]
+    # P10: linearity in S for a fixed template
+    p.subtract_batch([dSs[0] + dSs[1]], coeffs=(c12 := torch.empty((1, p.n), dtype=torch.float64, device="cuda")))
+    p.sync_status()
+    assert np.max(np.abs(c12.cpu().numpy()[0] - cs[0] - cs[1])) <= 1e-9 * np.max(np.abs(cs[0]))
+
+
+def test_difference_host_matches_device_path():
+    c = starfield.make_pair(0)
+    p, G, h, cd, D = run_gpu(c["S"], c["R"], None, c["L"], c["DK"], c["DB"])
+    Dh, ch = p.difference_host(torch.from_numpy(c["S"]).pin_memory(), torch.from_numpy(c["R"]).pin_memory())
+    assert np.array_equal(Dh.numpy(), D) and np.array_equal(ch.numpy(), cd)
