@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- SFFT difference images/s at 4088^2 (L=11, DK=2), and % of HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (sfft_build_system,
+sfft_solve, sfft_subtract) over ONE synthetic 4088 x 4088 science/template pair, L=11, DK=2, DB=2
+(BASELINE.json configs[2], the configuration `metric` is quoted on).  Nothing is reused between
+steps.  `value` is timed with the inputs resident in HBM; `e2e` is the same metric through
+sfft_difference_host with pinned HOST buffers (H2D of S and R, D2H of D and the coefficients inside
+the timed region).  N > 1: replicas only -- every rank runs the same
+independent problem on its own GPU, no data-path collective; value = N / max-over-ranks step time.
+
+Extra objects on the JSON line: `roofline` (dominant kernel, timed live with CUDA events through
+the library's per-launch timers on the plan's stream), `path_roofline` (the metric's "% of HBM
+roofline": 34 r of algorithmic bytes over the a1+a2+a3+a5 time), `stages_ms`, `kernels_ms`,
+`batched` (configs[3]: template-side work once, per-science-image throughput), `cpu_baseline`
+(the oracle on this box's host cores, bounded sample), `clocks`.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the same config and metric.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "sfft_difference_images_per_sec_4088sq_L11_DK2"
+UNIT = "images/s"
+WORKLOAD = dict(workload="BASELINE.json configs[2]: single 4088x4088 fp64 pair, 60k stars, L=11, DK=2, DB=2 (n=732)",
+                nx=4088, ny=4088, L=11, DK=2, DB=2, n=732)
+NOMINAL_HBM_GBS = 7700.0
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            d = json.loads(f.read_text())
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def algorithmic_bytes(nx, ny, DK, NK):
+    """SURVEY.md 8(d) / DESIGN.md: bytes the canonical 2-D-FFT formulation must move, in units of
+    r = nx*ny*8 (one FP64 image; a half spectrum is ~r).  Per kernel and per stage group."""
+    r = nx * ny * 8.0
+    k = {
+        "row_fwd_R": (1 + (DK + 1)) * r,        # read R, write DK+1 row-transformed intermediates
+        "col_fwd_R": ((DK + 1) + NK) * r,       # read them, write NK spectra
+        "row_fwd_S": 2 * r, "col_fwd_S": 2 * r,
+        "lagcol_omega": NK * r,                 # NK template spectra, once
+        "lagcol_theta": (NK + 1) * r,           # + the science spectrum
+        "col_inv": (NK + 1) * r,                # NK spectra in, one intermediate out
+        "row_inv": 3 * r,                       # intermediate + S in, D out
+    }
+    path = (1 + 2 * (DK + 1) + NK) * r + 4 * r + (NK + 1) * r + (NK + 4) * r   # 13 + 4 + 7 + 10 = 34 r at DK=2
+    return k, path
+
+
+class ClockSampler:
+    """Samples SM clock, power and throttle reasons of one GPU every 100 ms (NVML) while running."""
+
+    def __init__(self, index):
+        self.index, self.samples, self.reasons, self._stop, self._t = index, [], set(), threading.Event(), None
+        self.max_mhz, self.ok = None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def _loop(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append((int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)),
+                                     nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0))
+                try:
+                    bits = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for b, nm in names.items():
+                    if bits & b:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        if self.ok:
+            self._t = threading.Thread(target=self._loop, daemon=True)
+            self._t.start()
+
+    def stop(self):
+        if self._t:
+            self._stop.set()
+            self._t.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        mhz = sorted(s[0] for s in self.samples)
+        return {"sm_mhz": mhz[len(mhz) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "power_w_max": round(max(s[1] for s in self.samples), 1), "samples": len(mhz)}
+
+
+# ------------------------------------------------------------------------------------------
+# the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------
+def oracle_step(S, R, crop, L, DK, DB):
+    """The oracle's whole path (direct-sum build_system, textbook Cholesky, real-space subtract) on
+    the top-left crop x crop corner of the pair.  Returns seconds of (build, solve, subtract)."""
+    import oracle
+    s = np.ascontiguousarray(S[:crop, :crop])
+    r = np.ascontiguousarray(R[:crop, :crop])
+    t0 = time.perf_counter()
+    G, h = oracle.build_system(s, r, None, L, DK, DB)
+    t1 = time.perf_counter()
+    c = oracle.solve(G, h)
+    t2 = time.perf_counter()
+    oracle.subtract(s, r, L, DK, DB, c)
+    t3 = time.perf_counter()
+    return t1 - t0, t2 - t1, t3 - t2
+
+
+def oracle_full_frame_seconds(tb, ts, tsub, crop, nx, ny):
+    """build and subtract are sums over pixels (linear in the pixel count), the solve is not."""
+    scale = (nx * ny) / float(crop * crop)
+    return (tb + tsub) * scale + ts
+
+
+def pick_crop(S, R, L, DK, DB, budget_s, nsteps):
+    """Largest crop in {2044, 1022, 511} whose nsteps oracle passes fit budget_s (calibrated on 511)."""
+    tb, ts, tsub = oracle_step(S, R, 511, L, DK, DB)
+    per_pix = (tb + tsub) / (511.0 * 511.0)
+    for crop in (2044, 1022):
+        if nsteps * (per_pix * crop * crop + ts) <= budget_s:
+            return crop
+    return 511
+
+
+def cpu_baseline(S, R, cfg, budget_s=25.0):
+    import oracle
+    crop = pick_crop(S, R, cfg["L"], cfg["DK"], cfg["DB"], budget_s, 1)
+    tb, ts, tsub = oracle_step(S, R, crop, cfg["L"], cfg["DK"], cfg["DB"])
+    full = oracle_full_frame_seconds(tb, ts, tsub, crop, cfg["nx"], cfg["ny"])
+    return {"value": 1.0 / full, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"oracle build_system+solve+subtract on the top-left {crop}x{crop} crop of the same pair "
+                      f"({tb + ts + tsub:.2f} s); pixel-linear stages scaled by {cfg['nx'] * cfg['ny'] / crop / crop:.1f} "
+                      f"to 4088x4088, Cholesky (n={cfg['n']}) unscaled",
+            "seconds_sample": round(tb + ts + tsub, 3), "seconds_full_frame_est": round(full, 2)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config/metric; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    import oracle
+    from paper_2509_18544_b200 import starfield
+    cfg = dict(WORKLOAD)
+    pair = starfield.make_pair(2)
+    S, R = pair["S"], pair["R"]
+    crop = pick_crop(S, R, cfg["L"], cfg["DK"], cfg["DB"], 150.0, args.steps + args.warmup)
+    for _ in range(args.warmup):
+        oracle_step(S, R, crop, cfg["L"], cfg["DK"], cfg["DB"])
+    tot, raw = 0.0, 0.0
+    for _ in range(args.steps):
+        tb, ts, tsub = oracle_step(S, R, crop, cfg["L"], cfg["DK"], cfg["DB"])
+        tot += oracle_full_frame_seconds(tb, ts, tsub, crop, cfg["nx"], cfg["ny"])
+        raw += tb + ts + tsub
+    sec = tot / args.steps
+    val = 1.0 / sec
+    sample = (f"each step = oracle build_system+solve+subtract on the top-left {crop}x{crop} crop "
+              f"({raw / args.steps:.2f} s measured), pixel-linear stages scaled to 4088x4088")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(cfg, l2="n/a (CPU)"),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2509_18544_b200 import SfftPlan, sfft, starfield
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libsfft has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = dict(WORKLOAD)
+    nx, ny, L, DK, DB = cfg["nx"], cfg["ny"], cfg["L"], cfg["DK"], cfg["DB"]
+    NK = (DK + 1) * (DK + 2) // 2
+    pair = starfield.make_pair(2)                      # same seeded pair on every replica
+    S_np, R_np = pair["S"], pair["R"]
+    dS, dR = torch.from_numpy(S_np).cuda(), torch.from_numpy(R_np).cuda()
+    D = torch.empty_like(dS)
+    coeffs = torch.empty(cfg["n"], dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    plan = SfftPlan(nx, ny, L, DK, DB, stream=stream)
+
+    def step():
+        plan.build_system(dS, dR)
+        plan.solve()
+        plan.subtract(D, coeffs)
+
+    # ---- headline: K steps, device-resident inputs --------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        step()
+    plan.sync_status()
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    n0 = plan.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = plan.launch_count - n0
+    plan.sync_status()
+
+    # ---- e2e: host buffers through sfft_difference_host ---------------------------------------
+    hS, hR = torch.from_numpy(S_np).pin_memory(), torch.from_numpy(R_np).pin_memory()
+    hD = torch.empty((ny, nx), dtype=torch.float64).pin_memory()
+    hc = torch.empty(cfg["n"], dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        plan.difference_host(hS, hR, None, hD, hc)
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(stream)
+    for _ in range(args.steps):
+        plan.difference_host(hS, hR, None, hD, hc)
+    f1.record(stream)
+    barrier()
+    ms_e2e = f0.elapsed_time(f1)
+    clk = clocks.stop()
+
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_step = ms_total / args.steps
+    value = world * 1e3 / ms_step
+    e2e_value = world * 1e3 / (ms_e2e / args.steps)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(cfg, parallelism=f"replicas x{world}" if world > 1 else "single GPU",
+                           l2="inputs larger than L2: S, R 134 MB each, ~5 GB streamed per step vs 126 MB L2; no flush"),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(2 * nx * ny * 8),
+                    "d2h_bytes_per_step": int(nx * ny * 8 + cfg["n"] * 8), "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": int(launches), "clocks": clk, "library": sfft.version(),
+            "workspace_gb": round(plan.workspace_bytes / 1e9, 3)}
+
+    if rank == 0:
+        line.update(detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch))
+        if world == 1:
+            line["cpu_baseline"] = cpu_baseline(S_np, R_np, cfg)
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
+    """Per-stage and per-kernel times (live, CUDA events on the plan's stream), the rooflines, the
+    batched variant and the measured FP64 rates.  Runs after the headline region, on rank 0."""
+    from paper_2509_18544_b200 import sfft, starfield
+    nx, ny, DK = cfg["nx"], cfg["ny"], cfg["DK"]
+    peak, peak_src = measured_peaks()
+    kbytes, path_bytes = algorithmic_bytes(nx, ny, DK, NK)
+    K = max(3, min(args.steps, 10))
+
+    # per stage
+    stages = {}
+    for _ in range(K):
+        plan.enable_timings(1)
+        step()
+        for k, v in plan.get_timings().items():
+            stages.setdefault(k, []).append(v)
+    stages = {k: float(np.median(v)) for k, v in stages.items()}
+    # per kernel launch
+    ksum, kcnt = {}, {}
+    for _ in range(K):
+        plan.enable_timings(2)
+        step()
+        per = {}
+        for name, ms in plan.kernel_timings():
+            per[name] = per.get(name, 0.0) + ms
+            kcnt[name] = kcnt.get(name, 0) + 1
+        for name, ms in per.items():
+            ksum.setdefault(name, []).append(ms)
+    plan.enable_timings(0)
+    kernels = {k: float(np.median(v)) for k, v in ksum.items()}          # ms per step, all launches of that kernel
+    kcnt = {k: v // K for k, v in kcnt.items()}
+
+    out = {"stages_ms": {k: round(v, 4) for k, v in stages.items()},
+           "kernels_ms": {k: round(v, 4) for k, v in sorted(kernels.items(), key=lambda kv: -kv[1])},
+           "kernel_launches_per_step": kcnt}
+
+    # dominant kernel among those that stream images/spectra
+    hbm_kernels = {k: v for k, v in kernels.items() if k in kbytes}
+    dom = max(hbm_kernels, key=hbm_kernels.get)
+    per_launch_ms = kernels[dom] / kcnt[dom]
+    ach = kbytes[dom] / (per_launch_ms * 1e-3) / 1e9
+    out["roofline"] = {"kernel": dom, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
+                       "frac": round(ach / peak, 4), "traffic": None, "peak_source": peak_src,
+                       "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": round(per_launch_ms, 4),
+                       "share_of_step": round(kernels[dom] / sum(kernels.values()), 3)}
+    t_path = sum(stages[k] for k in ("a1_template", "a1_science", "a2_omega", "a2_theta", "a3_gather", "a5_subtract"))
+    out["path_roofline"] = {"what": "a1+a2+a3+a5 (BASELINE.json target: >= 0.60)", "algorithmic_bytes": path_bytes,
+                            "ms": round(t_path, 4), "achieved_gbs": round(path_bytes / t_path / 1e6, 1),
+                            "frac_of_measured": round(path_bytes / t_path / 1e6 / peak, 4),
+                            "frac_of_nominal_7.7TBs": round(path_bytes / t_path / 1e6 / NOMINAL_HBM_GBS, 4),
+                            "a4_ms": round(stages["a4_factor"] + stages["a4_solve"], 4)}
+    # FP64 rates of this box (the ALU roofline of a2 and a4)
+    try:
+        out["fp64_probe_tflops"] = {"dfma": round(sfft.probe_fp64(0), 2), "dmma_m8n8k4": round(sfft.probe_fp64(1), 2)}
+    except Exception as e:  # pragma: no cover
+        out["fp64_probe_tflops"] = {"error": str(e)}
+
+    # batched variant (BASELINE.json configs[3]): template once, B science images
+    B = args.batch
+    if B > 0:
+        tmpl = dict(pair)
+        Ss = [dS] + [torch.from_numpy(starfield.make_batch_science(tmpl, b)).cuda() for b in range(1, min(B, 4))]
+        S_list = [Ss[b % len(Ss)] for b in range(B)]          # B launches over 4 distinct seeded images
+        D_list = [torch.empty_like(dS) for _ in range(min(B, 4))]
+        D_arg = [D_list[b % len(D_list)] for b in range(B)]
+        cb = torch.empty((B, cfg["n"]), dtype=torch.float64, device="cuda")
+        stream = torch.cuda.current_stream()
+        for _ in range(2):
+            plan.set_template(dR)
+            plan.subtract_batch(S_list[:2], D_arg[:2], cb[:2].contiguous())
+        torch.cuda.synchronize()
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        e[0].record(stream)
+        plan.set_template(dR)
+        e[1].record(stream)
+        plan.subtract_batch(S_list, D_arg, cb)
+        e[2].record(stream)
+        torch.cuda.synchronize()
+        plan.sync_status()
+        t_t, t_b = e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
+        r = nx * ny * 8.0
+        per_img_bytes = (4 + (NK + 1) + (NK + 4)) * r + (13 + NK) * r / B
+        out["batched"] = {"workload": f"BASELINE.json configs[3]: one template, B={B} science images "
+                                      f"({len(Ss)} distinct seeded images cycled)",
+                          "B": B, "template_ms": round(t_t, 3), "per_image_ms": round(t_b / B, 4),
+                          "images_per_s": round(B * 1e3 / (t_t + t_b), 1),
+                          "frac_of_measured_hbm": round(per_img_bytes / ((t_t + t_b) / B) / 1e6 / peak, 4)}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=32, help="science images of the batched (configs[3]) extra; 0 = skip")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -149,10 +149,18 @@ sfft_status sfft_sync_status(sfft_plan *plan);
  * either may be NULL.  Errors: STATE (nothing built yet). */
 sfft_status sfft_get_system(const sfft_plan *plan, double *G, double *h);
 
-/* ms[0..n_stages) <- per-stage milliseconds (CUDA events on the plan's stream) of the most
- * recent call of each stage; synchronises.  Timing is off until sfft_enable_timings(plan,1). */
+/* Timing mode: 0 = off (default), 1 = per stage, 2 = per kernel launch.  Resets what was recorded.
+ * sfft_get_timings: ms[0..n_stages) <- per-stage milliseconds (CUDA events on the plan's
+ * stream) of the most recent call of each stage; synchronises.  */
 sfft_status sfft_enable_timings(sfft_plan *plan, int on);
 sfft_status sfft_get_timings(sfft_plan *plan, float *ms, int n_stages);
+
+/* Mode 2: every kernel launch since sfft_enable_timings(plan, 2) is bracketed by a CUDA event
+ * pair on the plan's stream (at most 512 are kept).  sfft_kernel_timing_count returns how many
+ * were recorded; sfft_kernel_timing_get gives launch i's kernel name (static string, library
+ * owned) and its milliseconds (synchronises on that launch).  Errors: INVALID_ARG, CUDA. */
+int sfft_kernel_timing_count(const sfft_plan *plan);
+sfft_status sfft_kernel_timing_get(sfft_plan *plan, int i, const char **name, float *ms);
 
 /* Number of kernel launches this plan has enqueued since creation (bench: gpu_launches). */
 long long sfft_launch_count(const sfft_plan *plan);

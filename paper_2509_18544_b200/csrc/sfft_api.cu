@@ -81,6 +81,8 @@ static void free_plan(sfft_plan *p) {
         if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
         if (p->ev1[s]) cudaEventDestroy(p->ev1[s]);
     }
+    for (int k = 0; k < MAX_KREC; k++)
+        if (p->krec[k].e0) { cudaEventDestroy(p->krec[k].e0); cudaEventDestroy(p->krec[k].e1); }
     delete p;
 }
 
@@ -385,8 +387,20 @@ sfft_status sfft_get_system(const sfft_plan *pc, double *G, double *h) {
 
 sfft_status sfft_enable_timings(sfft_plan *p, int on) {
     if (!p) return SFFT_ERR_INVALID_ARG;
-    p->timing = on != 0;
+    p->timing = on == 1;
+    p->ktiming = on == 2;
+    p->nkrec = 0;
     for (int s = 0; s < SFFT_NUM_STAGES; s++) p->ev_used[s] = false;
+    return SFFT_OK;
+}
+
+int sfft_kernel_timing_count(const sfft_plan *p) { return p ? p->nkrec : 0; }
+
+sfft_status sfft_kernel_timing_get(sfft_plan *p, int i, const char **name, float *ms) {
+    if (!p || !name || !ms || i < 0 || i >= p->nkrec) return SFFT_ERR_INVALID_ARG;
+    CK(cudaEventSynchronize(p->krec[i].e1), "sync");
+    *name = p->krec[i].name; *ms = 0.0f;
+    CK(cudaEventElapsedTime(ms, p->krec[i].e0, p->krec[i].e1), "elapsed");
     return SFFT_OK;
 }
 

@@ -156,8 +156,7 @@ cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask,
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    row_fwd_kernel<<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, NI > 1 ? "row_fwd_R" : "row_fwd_S"); row_fwd_kernel<<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw); }
     return cudaGetLastError();
 }
 
@@ -173,8 +172,7 @@ cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, 
     }
     ColJobs jobs; jobs.ns = ns;
     for (int k = 0; k < ns; k++) { jobs.ii[k] = ii[k]; jobs.jj[k] = jj[k]; }
-    col_fwd_kernel<<<ns * (g.Hx / C), threads, smem, p->stream>>>(inter, spec, jobs, C, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, ns > 1 ? "col_fwd_R" : "col_fwd_S"); col_fwd_kernel<<<ns * (g.Hx / C), threads, smem, p->stream>>>(inter, spec, jobs, C, g, p->tw); }
     return cudaGetLastError();
 }
 

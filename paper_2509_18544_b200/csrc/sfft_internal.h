@@ -27,6 +27,9 @@ struct Geom {
     int pi[MAX_NP], pj[MAX_NP]; // t -> (i,j): total degree ascending, then j ascending
 };
 
+constexpr int MAX_KREC = 512;  // per-launch timing records kept between two sfft_enable_timings calls
+struct KRec { const char *name; cudaEvent_t e0, e1; };
+
 struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of one lag pass
     int np;
     int a[MAX_PAIRS], b[MAX_PAIRS];
@@ -72,6 +75,8 @@ struct sfft_plan {
     sfft::PairList plO, plT;
     // timing
     bool timing; cudaEvent_t ev0[SFFT_NUM_STAGES], ev1[SFFT_NUM_STAGES]; bool ev_used[SFFT_NUM_STAGES];
+    // per-launch timing (sfft_enable_timings(plan, 2)): one event pair per kernel launch, in launch order
+    bool ktiming; int nkrec; sfft::KRec krec[sfft::MAX_KREC];
     long long launches;
     char err[256];
 };
@@ -106,6 +111,21 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
 
 // ---- probes (sfft_probe.cu) -------------------------------------------------------------------
 cudaError_t run_probe_fp64(int kind, int iters, double *tflops);
+
+// RAII around ONE kernel launch: counts it and, in per-launch timing mode, brackets it with events.
+struct KLaunch {
+    sfft_plan *p; KRec *r;
+    KLaunch(sfft_plan *p_, const char *name) : p(p_), r(nullptr) {
+        p->launches++;
+        if (p->ktiming && p->nkrec < MAX_KREC) {
+            r = &p->krec[p->nkrec];
+            if (!r->e0) { cudaEventCreate(&r->e0); cudaEventCreate(&r->e1); }
+            r->name = name; p->nkrec++;
+            cudaEventRecord(r->e0, p->stream);
+        }
+    }
+    ~KLaunch() { if (r) cudaEventRecord(r->e1, p->stream); }
+};
 
 inline int ilog2(int v) { int l = 0; while ((1 << l) < v) l++; return l; }
 

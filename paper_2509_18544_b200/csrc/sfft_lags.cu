@@ -325,14 +325,13 @@ void lagcol_config(const Geom &g, int np, int W, LagCfg *c) {
 }
 
 template <int WB>
-static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const PairList &pl, int W, const LagCfg &c) {
+static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const PairList &pl, int W, const LagCfg &c, bool science) {
     const Geom &g = p->g;
     const size_t smem = (size_t)LC_NST * LC_RT * (ns * c.KXC + WB) * sizeof(cplx);
     cudaError_t e = cudaFuncSetAttribute(lagcol_kernel<WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
     if (e != cudaSuccess) return e;
     dim3 grid(c.nkb, c.ngr, c.nsplit);
-    lagcol_kernel<WB><<<grid, c.npg * c.KXC, smem, p->stream>>>(ss, ns, pl, c.npg, c.KXC, W, c.rows_per_split, p->Q, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega"); lagcol_kernel<WB><<<grid, c.npg * c.KXC, smem, p->stream>>>(ss, ns, pl, c.npg, c.KXC, W, c.rows_per_split, p->Q, g, p->tw); }
     return cudaGetLastError();
 }
 
@@ -347,25 +346,23 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     LagCfg c; lagcol_config(g, pl.np, W, &c);
     const int nsplit = c.nsplit;
     cudaError_t e;
-    if (c.WB == 3) e = run_lagcol<3>(p, ss, ns, pl, W, c);
-    else if (c.WB == 5) e = run_lagcol<5>(p, ss, ns, pl, W, c);
-    else if (c.WB == 6) e = run_lagcol<6>(p, ss, ns, pl, W, c);
-    else if (c.WB == 10) e = run_lagcol<10>(p, ss, ns, pl, W, c);
-    else e = run_lagcol<20>(p, ss, ns, pl, W, c);
+    if (c.WB == 3) e = run_lagcol<3>(p, ss, ns, pl, W, c, science);
+    else if (c.WB == 5) e = run_lagcol<5>(p, ss, ns, pl, W, c, science);
+    else if (c.WB == 6) e = run_lagcol<6>(p, ss, ns, pl, W, c, science);
+    else if (c.WB == 10) e = run_lagcol<10>(p, ss, ns, pl, W, c, science);
+    else e = run_lagcol<20>(p, ss, ns, pl, W, c, science);
     if (e != cudaSuccess) return e;
-    lagedge_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(ss, pl, W, nsplit, p->Q, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, science ? "lagedge_theta" : "lagedge_omega"); lagedge_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(ss, pl, W, nsplit, p->Q, g, p->tw); }
     int nchunk = 0;
     double *bpart = p->bpart;
     if (g.Mx != g.nx || g.My != g.ny) {
         nchunk = border_chunks();
         dim3 bg(2 * W + 1, 2 * W + 1, nchunk);
+        KLaunch kl(p, science ? "border_theta" : "border_omega");
         if (science) border_kernel<true><<<bg, 256, 0, p->stream>>>(p->R, p->S, p->mask, W, nchunk, bpart, pl.np, g);
         else border_kernel<false><<<bg, 256, 0, p->stream>>>(p->R, p->S, p->mask, W, nchunk, bpart, pl.np, g);
-        p->launches++;
     }
-    lagrow_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega"); lagrow_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw); }
     return cudaGetLastError();
 }
 

@@ -212,24 +212,21 @@ cudaError_t launch_factor(sfft_plan *p) {
     const int n = p->g.n;
     cudaStream_t st = p->stream;
     cudaMemsetAsync(p->flag, 0, sizeof(int), st);
-    equil_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(p->G, p->dscale, n, p->flag);
+    { KLaunch kl(p, "equil_diag"); equil_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(p->G, p->dscale, n, p->flag); }
     const long long total = (long long)n * n;
-    equil_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p->G, p->dscale, p->Lf, n);
-    p->launches += 2;
+    { KLaunch kl(p, "equil_scale"); equil_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p->G, p->dscale, p->Lf, n); }
     const int nblk = (n + CB - 1) / CB;
     const size_t sm_trsm = 2 * CB * (CB + 1) * sizeof(double), sm_syrk = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_trsm);
     cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
-        potrf_kernel<<<1, 256, 0, st>>>(p->Lf, n, k0, bs, p->flag);
-        p->launches++;
+        { KLaunch kl(p, "potrf"); potrf_kernel<<<1, 256, 0, st>>>(p->Lf, n, k0, bs, p->flag); }
         const int rem = n - k0 - bs;
         if (rem > 0) {
             const int nt = (rem + CB - 1) / CB;
-            trsm_kernel<<<nt, CB, sm_trsm, st>>>(p->Lf, n, k0, bs);
-            syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs);
-            p->launches += 2;
+            { KLaunch kl(p, "trsm"); trsm_kernel<<<nt, CB, sm_trsm, st>>>(p->Lf, n, k0, bs); }
+            { KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs); }
         }
     }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
@@ -237,8 +234,7 @@ cudaError_t launch_factor(sfft_plan *p) {
 }
 
 cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c) {
-    trisolve_kernel<<<1, 1024, 0, p->stream>>>(p->Lf, p->dscale, h, p->ywork, c, p->g.n);
-    p->launches++;
+    { KLaunch kl(p, "trisolve"); trisolve_kernel<<<1, 1024, 0, p->stream>>>(p->Lf, p->dscale, h, p->ywork, c, p->g.n); }
     return cudaGetLastError();
 }
 

@@ -235,8 +235,7 @@ int col_cfg(const Geom &g, int *threads, size_t *smem); // sfft_fwd.cu
 cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D) {
     const Geom &g = p->g;
     cudaStream_t st = p->stream;
-    ktab_kernel<<<dim3((g.Hx + 1 + 127) / 128, g.w + 1, g.NK), 128, 0, st>>>(coef, p->E, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, "ktab"); ktab_kernel<<<dim3((g.Hx + 1 + 127) / 128, g.w + 1, g.NK), 128, 0, st>>>(coef, p->E, g, p->tw); }
     int threads; size_t smem;
     const int C = col_cfg(g, &threads, &smem);
     smem += (size_t)g.NK * g.L * (C + 1) * sizeof(cplx);
@@ -247,17 +246,15 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw); }
     const int T = g.Hx >> 4;
     int RPB = 256 / T; if (RPB < 1) RPB = 1;
     const size_t rsmem = (size_t)RPB * padded_len(g.Hx) * sizeof(cplx);
-    row_inv_kernel<<<(g.ny + RPB - 1) / RPB, RPB * T, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
-    p->launches++;
+    { KLaunch kl(p, "row_inv"); row_inv_kernel<<<(g.ny + RPB - 1) / RPB, RPB * T, rsmem, st>>>(p->inter, S, coef, D, g, p->tw); }
     if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
         const long long nb = 2LL * g.w * g.nx + 2LL * g.w * (g.ny - 2 * g.w);
+        KLaunch kl(p, "wrapfix");
         wrapfix_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(R, coef, D, g);
-        p->launches++;
     }
     return cudaGetLastError();
 }

@@ -24,7 +24,8 @@ SYMBOLS = (
     "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
     "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_with",
     "sfft_set_template", "sfft_subtract_batch", "sfft_difference_host", "sfft_sync_status",
-    "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_launch_count",
+    "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
+    "sfft_kernel_timing_get", "sfft_launch_count",
     "sfft_last_error", "sfft_version", "sfft_debug_read", "sfft_probe_fp64",
 )
 
@@ -65,6 +66,8 @@ def load_library():
     lib.sfft_get_system.argtypes = [vp, dp, dp]
     lib.sfft_enable_timings.argtypes = [vp, ci]
     lib.sfft_get_timings.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ci]
+    lib.sfft_kernel_timing_count.argtypes = [vp]
+    lib.sfft_kernel_timing_get.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(ctypes.c_float)]
     lib.sfft_launch_count.argtypes = [vp]
     lib.sfft_launch_count.restype = ctypes.c_longlong
     lib.sfft_last_error.argtypes = [vp]
@@ -223,7 +226,18 @@ class SfftPlan:
         return G, h
 
     def enable_timings(self, on=True):
-        self._ck(self._lib.sfft_enable_timings(self._h, 1 if on else 0), "sfft_enable_timings")
+        """on: False/0 = off, True/1 = per stage, 2 = per kernel launch."""
+        self._ck(self._lib.sfft_enable_timings(self._h, int(on)), "sfft_enable_timings")
+
+    def kernel_timings(self):
+        """[(kernel name, ms), ...] of every launch since enable_timings(2), in launch order."""
+        out = []
+        name, ms = ctypes.c_char_p(), ctypes.c_float()
+        for i in range(self._lib.sfft_kernel_timing_count(self._h)):
+            self._ck(self._lib.sfft_kernel_timing_get(self._h, i, ctypes.byref(name), ctypes.byref(ms)),
+                     "sfft_kernel_timing_get")
+            out.append((name.value.decode(), float(ms.value)))
+        return out
 
     def get_timings(self):
         ms = (ctypes.c_float * len(STAGES))()
