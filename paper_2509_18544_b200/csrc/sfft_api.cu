@@ -73,7 +73,7 @@ struct StageTimer {
 static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
-                    p->Q, p->lagO, p->lagT, p->bpart, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale,
+                    p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale,
                     p->ywork, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->flag_host) cudaFreeHost(p->flag_host);
@@ -132,6 +132,11 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->lagO, (size_t)p->plO.np * W2 * W2);
     AL(p->lagT, (size_t)g.NK * L * L);
     AL(p->bpart, bO);
+    AL(p->SB, border_strip_doubles(g, 2 * g.w > 0 ? 2 * g.w : 1));
+    {
+        const size_t lpO = border_lp_doubles(g, 2 * g.w, DK + 1), lpT = border_lp_doubles(g, g.w, 1);
+        AL(p->LP, (lpO > lpT ? lpO : lpT) + 1);
+    }
     AL(p->gamA, (size_t)(DK + 1) * (DB + 1) * L * ny);
     AL(p->gam, (size_t)g.NK * g.NB * L * L);
     AL(p->phi, g.NB * g.NB);

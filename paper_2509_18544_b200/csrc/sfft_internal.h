@@ -51,7 +51,9 @@ struct sfft_plan {
     sfft::cplx *Q;           // [np][2W+1][Hx+1] column-reduced products (stage 1 of a2)
     double *lagO;            // [npairs][(4w+1)^2]
     double *lagT;            // [NK][L*L]
-    double *bpart;           // [chunks][np][(2W+1)^2] wrap-correction partial sums
+    double *bpart;           // [np][(2W+1)^2] native-grid wrap corrections X_N - X_M
+    double *SB;              // [2 images][4 sides][W][max(nx,ny)] border strips of m.R, m.S (sfft_border.cu)
+    double *LP;              // [chunk][4][W][W][2W+1][DK+1][DK+1|1] line-pair linear correlations
     double *gamA;            // [(DK+1)][(DB+1)][L][ny] row sums for Gamma
     double *gam;             // [NK][NB][L*L]
     double *phi;             // [NB][NB]
@@ -94,6 +96,10 @@ cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, 
 struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, rows_per_split; };
 void lagcol_config(const Geom &g, int np, int W, LagCfg *c);
 int border_chunks();
+int border_linpair_chunks();
+size_t border_lp_doubles(const Geom &g, int W, int EB);
+size_t border_strip_doubles(const Geom &g, int W);
+cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science, double *bpart);
 // ---- a2, a3 (sfft_lags.cu, sfft_assemble.cu) ---------------------------------------------------------
 // lag tables of pair list pl over spectra base[s] = spec0 + s*My*Hx (s < nsA: template set, s == nsA: specS)
 cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag /*[np][(2W+1)^2]*/, bool science);

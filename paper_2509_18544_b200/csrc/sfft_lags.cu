@@ -16,7 +16,7 @@
 //   lagcol_kernel  stage 1: Q[p][dv][kx] = sum_ky conj(A)B e^{2 pi i ky dv/My}, thread = (pair, kx),
 //                  rows streamed through a cp.async shared-memory pipeline shared by all pairs
 //   lagedge_kernel the packed column kx = 0 (DC + i Nyquist) untangled -> Q[.][.][0], Q[.][.][Hx]
-//   border_kernel  the wrap corrections by direct summation over the frame border
+//   (sfft_border.cu) the wrap corrections X_N - X_M from border strips
 //   lagrow_kernel  stage 2: lag[p][dv][du] = 1/(Mx My) sum_kx g Re(Q e^{2 pi i kx du/Mx}) + border
 #include "sfft_internal.h"
 
@@ -163,107 +163,6 @@ __global__ void __launch_bounds__(256) lagedge_kernel(SpecSet ss, PairList pl, i
         }
 }
 
-// ---------------------------------------------------------------- wrap corrections
-// grid = (2W+1 [du], 2W+1 [dv], nchunk); block 256.  SCI: b = m.S (pairs = t); else b = T_t' (pairs t<=t').
-// bpart[chunk][pair][dvIdx*(2W+1)+duIdx]
-template <bool SCI>
-__global__ void __launch_bounds__(256) border_kernel(const double *__restrict__ R, const double *__restrict__ S,
-                                                    const uint8_t *__restrict__ mask, int W, int nchunk,
-                                                    double *__restrict__ bpart, int np, Geom g) {
-    __shared__ double sh[32];
-    const int du = (int)blockIdx.x - W, dv = (int)blockIdx.y - W;
-    const int nx = g.nx, ny = g.ny, adu = abs(du), adv = abs(dv);
-    // region A: rows whose y+dv leaves the frame (adv rows, all x); region B: other rows, x+du outside
-    const long long nA = (long long)adv * nx, nB = (long long)(ny - adv) * adu, ntot = nA + nB;
-    const long long per = (ntot + nchunk - 1) / nchunk;
-    const long long i0 = per * blockIdx.z, i1 = min(ntot, i0 + per);
-    constexpr int NACC = SCI ? MAX_NP : MAX_PAIRS;
-    double acc[NACC];
-#pragma unroll
-    for (int k = 0; k < NACC; k++) acc[k] = 0.0;
-    const double inx = 1.0 / nx, iny = 1.0 / ny;
-    const double *Bimg = SCI ? S : R;
-    for (long long idx = i0 + threadIdx.x; idx < i1; idx += blockDim.x) {
-        int x, y;
-        if (idx < nA) {
-            const int ry = (int)(idx / nx); x = (int)(idx - (long long)ry * nx);
-            y = dv > 0 ? ny - adv + ry : ry;
-        } else {
-            const long long k = idx - nA;
-            const int ry = (int)(k / adu), rx = (int)(k - (long long)ry * adu);
-            y = dv > 0 ? ry : ry + adv;           // rows with y+dv inside
-            x = du > 0 ? nx - adu + rx : rx;
-        }
-        const size_t o = (size_t)y * nx + x;
-        double a = R[o]; if (mask && !mask[o]) a = 0.0;
-        int xN = x + du; if (xN >= nx) xN -= nx; if (xN < 0) xN += nx;
-        int yN = y + dv; if (yN >= ny) yN -= ny; if (yN < 0) yN += ny;
-        const int xM = (x + du + g.Mx) & (g.Mx - 1), yM = (y + dv + g.My) & (g.My - 1);
-        const size_t oN = (size_t)yN * nx + xN;
-        double bN = Bimg[oN]; if (mask && !mask[oN]) bN = 0.0;
-        double bM = 0.0;
-        const bool inM = xM < nx && yM < ny;
-        if (inM) { const size_t oM = (size_t)yM * nx + xM; bM = Bimg[oM]; if (mask && !mask[oM]) bM = 0.0; }
-        const double xa = (2.0 * x + 1.0 - nx) * inx, ya = (2.0 * y + 1.0 - ny) * iny;
-        double xpa[MAX_DEG + 1], ypa[MAX_DEG + 1];
-        xpa[0] = 1.0; ypa[0] = 1.0;
-#pragma unroll
-        for (int k = 1; k <= MAX_DEG; k++) { xpa[k] = xpa[k - 1] * xa; ypa[k] = ypa[k - 1] * ya; }
-        if (SCI) {
-            const double d = a * (bN - bM);
-#pragma unroll
-            for (int t = 0; t < MAX_NP; t++)
-                if (t < g.NK) {
-                    double wx = 1.0, wy = 1.0;
-#pragma unroll
-                    for (int k = 1; k <= MAX_DEG; k++) { if (g.pi[t] == k) wx = xpa[k]; if (g.pj[t] == k) wy = ypa[k]; }
-                    acc[t] = fma(wx * wy, d, acc[t]);
-                }
-        } else {
-            const double xb = (2.0 * xN + 1.0 - nx) * inx, yb = (2.0 * yN + 1.0 - ny) * iny;
-            const double xc = (2.0 * xM + 1.0 - nx) * inx, yc = (2.0 * yM + 1.0 - ny) * iny;
-            double xpb[MAX_DEG + 1], ypb[MAX_DEG + 1], xpc[MAX_DEG + 1], ypc[MAX_DEG + 1];
-            xpb[0] = ypb[0] = xpc[0] = ypc[0] = 1.0;
-#pragma unroll
-            for (int k = 1; k <= MAX_DEG; k++) {
-                xpb[k] = xpb[k - 1] * xb; ypb[k] = ypb[k - 1] * yb; xpc[k] = xpc[k - 1] * xc; ypc[k] = ypc[k - 1] * yc;
-            }
-            double wa[MAX_NP], wd[MAX_NP]; // wa[t] = T_t(x,y);  wd[t'] = T_t'(N-wrapped) - T_t'(M-wrapped)
-#pragma unroll
-            for (int t = 0; t < MAX_NP; t++) {
-                double ax = 1.0, ay = 1.0, bx = 1.0, by = 1.0, cx = 1.0, cy = 1.0;
-#pragma unroll
-                for (int k = 1; k <= MAX_DEG; k++) {
-                    if (g.pi[t] == k) { ax = xpa[k]; bx = xpb[k]; cx = xpc[k]; }
-                    if (g.pj[t] == k) { ay = ypa[k]; by = ypb[k]; cy = ypc[k]; }
-                }
-                wa[t] = ax * ay * a;
-                wd[t] = bx * by * bN - cx * cy * bM;
-            }
-#pragma unroll
-            for (int t = 0; t < MAX_NP; t++)
-#pragma unroll
-                for (int tp = t; tp < MAX_NP; tp++)
-                    if (tp < g.NK) { // static slot t*MAX_NP - t(t-1)/2 + tp - t
-                        const int slot = t * MAX_NP - (t * (t - 1)) / 2 + (tp - t);
-                        acc[slot] = fma(wa[t], wd[tp], acc[slot]);
-                    }
-        }
-    }
-    const int nl = (2 * W + 1) * (2 * W + 1);
-    // actual pair order: t ascending, tp = t..NK-1 (SCI: pair k = t)
-    int k = 0;
-    for (int t = 0; t < g.NK; t++)
-        for (int tp = t; tp < (SCI ? t + 1 : g.NK); tp++, k++) {
-            const int slot = SCI ? t : t * MAX_NP - (t * (t - 1)) / 2 + (tp - t);
-            double v = 0.0;
-#pragma unroll
-            for (int q = 0; q < NACC; q++) if (q == slot) v = acc[q];
-            v = block_sum(v, sh);
-            if (threadIdx.x == 0) bpart[((size_t)blockIdx.z * np + k) * nl + blockIdx.y * (2 * W + 1) + blockIdx.x] = v;
-        }
-}
-
 // ---------------------------------------------------------------- stage 2
 // grid = (np, 2W+1 [dv]); block 256.
 __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q, int np, int W, int nsplit,
@@ -335,7 +234,7 @@ static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const Pai
     return cudaGetLastError();
 }
 
-int border_chunks() { return 8; }
+int border_chunks() { return 1; }
 
 cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bool science) {
     const Geom &g = p->g;
@@ -357,10 +256,8 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     double *bpart = p->bpart;
     if (g.Mx != g.nx || g.My != g.ny) {
         nchunk = border_chunks();
-        dim3 bg(2 * W + 1, 2 * W + 1, nchunk);
-        KLaunch kl(p, science ? "border_theta" : "border_omega");
-        if (science) border_kernel<true><<<bg, 256, 0, p->stream>>>(p->R, p->S, p->mask, W, nchunk, bpart, pl.np, g);
-        else border_kernel<false><<<bg, 256, 0, p->stream>>>(p->R, p->S, p->mask, W, nchunk, bpart, pl.np, g);
+        if (W > 0) { e = launch_border(p, pl, W, science, bpart); if (e != cudaSuccess) return e; }
+        else nchunk = 0;
     }
     { KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega"); lagrow_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw); }
     return cudaGetLastError();
