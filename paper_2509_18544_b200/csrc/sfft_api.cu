@@ -73,8 +73,8 @@ struct StageTimer {
 static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
-                    p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale,
-                    p->ywork, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
+                    p->ywork, p->zwork, p->sflags, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->flag_host) cudaFreeHost(p->flag_host);
     for (int s = 0; s < SFFT_NUM_STAGES; s++) {
@@ -145,7 +145,10 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->h, n);
     AL(p->Lf, (size_t)n * n);
     AL(p->dscale, n);
+    AL(p->Linv, (size_t)((n + 63) / 64) * 64 * 64);
     AL(p->ywork, n);
+    AL(p->zwork, n);
+    AL(p->sflags, 2 * ((n + 63) / 64));
     AL(p->coef, n);
     AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
     AL(p->flag, 1);
@@ -168,6 +171,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
             phi[s * g.NB + s2] = power_sum(nx, g.pi[s] + g.pi[s2]) * power_sum(ny, g.pj[s] + g.pj[s2]);
     e = cudaMemcpy(p->phi, phi, sizeof(double) * g.NB * g.NB, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemset(p->flag, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(p->sflags, 0, sizeof(int) * 2 * ((n + 63) / 64));
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { cudaGetLastError(); free_plan(p); return SFFT_ERR_CUDA; }
     p->launches = 1;

@@ -62,7 +62,9 @@ struct sfft_plan {
     double *h;               // [n]
     double *Lf;              // [n][n] Cholesky factor of the equilibrated matrix (lower, row-major)
     double *dscale;          // [n]   1/sqrt(G_ii)
-    double *ywork;           // [n]
+    double *Linv;            // [nblk][64][64] inverses of the factor's diagonal blocks
+    double *ywork, *zwork;   // [n] forward / backward substitution vectors
+    int *sflags; int solve_epoch; // [2*nblk] block-done flags of the cooperative triangular solve
     double *coef;            // [n]   solved coefficients
     sfft::cplx *E;           // [NK][L][Hx+1] kernel row tables for a5
     int *flag;               // device: 1 = pivot test failed

@@ -27,60 +27,96 @@ __global__ void equil_scale_kernel(const double *__restrict__ G, const double *_
     Lf[id] = c <= r ? dscale[r] * G[id] * dscale[c] : 0.0;
 }
 
-// diagonal block k0..k0+bs: unblocked right-looking Cholesky in shared memory
-__global__ void __launch_bounds__(256) potrf_kernel(double *__restrict__ Lf, int n, int k0, int bs, int *flag) {
-    __shared__ double a[CB][CB + 1];
-    for (int e = threadIdx.x; e < bs * bs; e += blockDim.x) {
-        const int r = e / bs, c = e % bs;
-        a[r][c] = Lf[(size_t)(k0 + r) * n + k0 + c];
+// Fused panel step: every CTA factors the diagonal block k0..k0+bs redundantly (thread (r, cq) keeps
+// a[r][c], c = cq mod 4, in 16 registers; one barrier per column, through which the current column is
+// shared), CTA 0 writes L_kk back, and CTA b then solves its own 64 rows below the block,
+// X L_kk^T = A, by a register-resident right-looking substitution (4 lanes per row, shuffles only).
+// No FP64 division or sqrt on the dependent chain: inv = rsqrt(pivot), L_jj = pivot * inv.
+// grid = max(1, row tiles below); block 256; static smem.
+__global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ Lf, int n, int k0, int bs, int *flag) {
+    __shared__ double l[CB][CB + 1];
+    __shared__ double col[2][CB];
+    __shared__ double rd[CB];
+    const int tid = threadIdx.x, r = tid >> 2, cq = tid & 3, lane = tid & 31;
+    const int r0 = k0 + bs + blockIdx.x * CB;
+    const bool have_rows = r0 < n;
+    double areg[16], xr[16];
+#pragma unroll
+    for (int q = 0; q < 16; q++) {
+        const int c = 4 * q + cq;
+        double v = (r == c) ? 1.0 : 0.0;                         // identity padding for a short last block
+        if (r < bs && c < bs) v = (c <= r) ? Lf[(size_t)(k0 + r) * n + k0 + c] : 0.0;
+        areg[q] = v;
+        xr[q] = (have_rows && r0 + r < n && c < bs) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
     }
-    for (int j = 0; j < bs; j++) {
+#pragma unroll
+    for (int j = 0; j < CB; j++) {
+        double *cj = col[j & 1];
+        if (cq == (j & 3) && r >= j) cj[r] = areg[j >> 2];
         __syncthreads();
-        if (threadIdx.x == 0) {
-            double s = a[j][j];
-            if (!(s > PIVOT_MIN)) { *flag = 1; s = 1.0; }
-            a[j][j] = sqrt(s);
+        double piv = cj[j];
+        if (!(piv > PIVOT_MIN)) { if (tid == 0 && blockIdx.x == 0) *flag = 1; piv = 1.0; }
+        const double inv = rsqrt(piv);
+        const double lr = (r == j) ? piv * inv : cj[r] * inv;
+        if (tid == 0) rd[j] = inv;
+        if (cq == (j & 3) && r >= j) areg[j >> 2] = lr;
+        if (r > j) {
+#pragma unroll
+            for (int q = j >> 2; q < 16; q++) {
+                const int c = 4 * q + cq;
+                if (c > j && c <= r) areg[q] = fma(-lr, cj[c] * inv, areg[q]);
+            }
         }
-        __syncthreads();
-        const double d = 1.0 / a[j][j];
-        for (int r = j + 1 + threadIdx.x; r < bs; r += blockDim.x) a[r][j] *= d;
-        __syncthreads();
-        const int m = bs - j - 1;
-        for (int e = threadIdx.x; e < m * m; e += blockDim.x) {
-            const int r = j + 1 + e / m, c = j + 1 + e % m;
-            if (c <= r) a[r][c] -= a[r][j] * a[c][j];
-        }
+    }
+#pragma unroll
+    for (int q = 0; q < 16; q++) {
+        const int c = 4 * q + cq;
+        l[r][c] = c <= r ? areg[q] : 0.0;
+        if (blockIdx.x == 0 && r < bs && c <= r) Lf[(size_t)(k0 + r) * n + k0 + c] = areg[q];
     }
     __syncthreads();
-    for (int e = threadIdx.x; e < bs * bs; e += blockDim.x) {
-        const int r = e / bs, c = e % bs;
-        if (c <= r) Lf[(size_t)(k0 + r) * n + k0 + c] = a[r][c];
+    if (!have_rows) return;
+    // x_j = x_j / l_jj, then x_c -= x_j l_cj for c > j; lanes 4g..4g+3 hold row r
+#pragma unroll
+    for (int j = 0; j < CB; j++) {
+        double xj = xr[j >> 2] * rd[j];
+        xj = __shfl_sync(0xffffffffu, xj, (lane & ~3) | (j & 3));
+        if (cq == (j & 3)) xr[j >> 2] = xj;
+#pragma unroll
+        for (int q = j >> 2; q < 16; q++) {
+            const int c = 4 * q + cq;
+            if (c > j) xr[q] = fma(-xj, l[c][j], xr[q]);
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < 16; q++) {
+        const int c = 4 * q + cq;
+        if (r0 + r < n && c < bs) Lf[(size_t)(r0 + r) * n + k0 + c] = xr[q];
     }
 }
 
-// panel: rows below the diagonal block, X L_kk^T = A.  grid = ceil(rows/64), block 64 (one row each)
-__global__ void __launch_bounds__(CB) trsm_kernel(double *__restrict__ Lf, int n, int k0, int bs) {
+// Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves:
+// Linv[b][i][c], thread c solves column c of  L X = I  by forward substitution.  grid = nblk; block 64.
+__global__ void __launch_bounds__(CB) trinv_kernel(const double *__restrict__ Lf, double *__restrict__ Linv, int n) {
     extern __shared__ __align__(16) double dsm[];
     double (*l)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm);
     double (*x)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm + CB * (CB + 1));
-    const int r0 = k0 + bs + blockIdx.x * CB;
-    for (int e = threadIdx.x; e < bs * bs; e += blockDim.x) l[e / bs][e % bs] = Lf[(size_t)(k0 + e / bs) * n + k0 + e % bs];
-    for (int e = threadIdx.x; e < CB * bs; e += blockDim.x) {
-        const int r = e / bs, c = e % bs;
-        x[r][c] = (r0 + r < n) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
+    const int k0 = blockIdx.x * CB, bs = min(CB, n - k0), c = threadIdx.x;
+    for (int e = threadIdx.x; e < CB * CB; e += CB) {
+        const int r = e >> 6, cc = e & 63;
+        l[r][cc] = (r < bs && cc <= r) ? Lf[(size_t)(k0 + r) * n + k0 + cc] : (r == cc ? 1.0 : 0.0);
     }
     __syncthreads();
-    const int r = threadIdx.x;
-    for (int j = 0; j < bs; j++) {
-        double s = x[r][j];
-        for (int m = 0; m < j; m++) s = fma(-x[r][m], l[j][m], s);
-        x[r][j] = s / l[j][j];
+    for (int i = 0; i < CB; i++) {
+        double s0 = (i == c) ? 1.0 : 0.0, s1 = 0.0;
+        int m = c;
+        for (; m + 1 < i; m += 2) { s0 = fma(-l[i][m], x[m][c], s0); s1 = fma(-l[i][m + 1], x[m + 1][c], s1); }
+        if (m < i) s0 = fma(-l[i][m], x[m][c], s0);
+        x[i][c] = i >= c ? (s0 + s1) / l[i][i] : 0.0;
     }
     __syncthreads();
-    for (int e = threadIdx.x; e < CB * bs; e += blockDim.x) {
-        const int rr = e / bs, c = e % bs;
-        if (r0 + rr < n) Lf[(size_t)(r0 + rr) * n + k0 + c] = x[rr][c];
-    }
+    double *dst = Linv + (size_t)blockIdx.x * CB * CB;
+    for (int e = threadIdx.x; e < CB * CB; e += CB) dst[e] = x[e >> 6][e & 63];
 }
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
@@ -137,75 +173,106 @@ __global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int 
         }
 }
 
-// ---- triangular solves, single CTA of 1024 threads (32 warps), block 64 ---------------------------
-// forward (left-looking): y_blk = L_kk^-1 ( (D h)_blk - L[blk, 0:k0] y[0:k0] )
-// backward:               z_blk = L_kk^-T ( y_blk - L[k0+bs:, blk]^T z[k0+bs:] ),  c = D z
-__global__ void __launch_bounds__(1024) trisolve_kernel(const double *__restrict__ Lf, const double *__restrict__ dscale,
-                                                       const double *__restrict__ h, double *__restrict__ y,
-                                                       double *__restrict__ c, int n) {
+// ---- triangular solves: one CTA per 64-row block, all co-resident (cooperative launch) -------------
+// c = D L^-T L^-1 D h.  Forward: CTA b accumulates L[b, kb] y_kb for kb = 0..b-1 as soon as block kb
+// publishes y_kb (flag in global memory), then solves its diagonal block and publishes y_b; backward the
+// same from the last block up with L^T.  The critical path is the chain of 64 x 64 diagonal solves; the
+// off-diagonal products of the waiting CTAs run beside it.  flags[0..nblk) forward, [nblk..2 nblk) backward,
+// compared against `epoch` (incremented per call, so no reset is needed).
+__device__ __forceinline__ void wait_flag(const int *f, int epoch) {
+    if (threadIdx.x == 0) {
+        while (*((volatile const int *)f) != epoch) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict__ Lf, const double *__restrict__ Linv,
+                                                      const double *__restrict__ dscale,
+                                                      const double *__restrict__ h, double *__restrict__ y,
+                                                      double *__restrict__ z, double *__restrict__ c, int n,
+                                                      int *flags, int epoch) {
+    __shared__ double Ld[CB][CB + 1];
+    __shared__ double vec[CB];
     __shared__ double blk[CB];
-    __shared__ double part[16][CB];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    const int nblk = (n + CB - 1) / CB;
-    // ---------------- forward
-    for (int kb = 0; kb < nblk; kb++) {
-        const int k0 = kb * CB, bs = min(CB, n - k0);
-        for (int r = warp; r < bs; r += nw) {
-            const double *row = Lf + (size_t)(k0 + r) * n;
-            double s = 0.0;
-            for (int j = lane; j < k0; j += 32) s = fma(row[j], y[j], s);
+    __shared__ double part[4][CB];
+    const int b = blockIdx.x, nblk = gridDim.x;
+    const int k0 = b * CB, bs = min(CB, n - k0);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    for (int e = tid; e < CB * CB; e += 256) Ld[e >> 6][e & 63] = Linv[(size_t)b * CB * CB + e]; // inverse of L_bb
+    // ---------------- forward: rows of this block, 8 rows per warp, lanes over the 64 columns of block kb
+    double acc[8];
 #pragma unroll
-            for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
-            if (lane == 0) blk[r] = dscale[k0 + r] * h[k0 + r] - s;
+    for (int q = 0; q < 8; q++) acc[q] = 0.0;
+    for (int kb = 0; kb < b; kb++) {
+        double l0[8], l1[8];
+#pragma unroll
+        for (int q = 0; q < 8; q++) { // L is final: load before waiting for y_kb
+            const int r = warp * 8 + q;
+            const double *row = Lf + (size_t)(k0 + r) * n + kb * CB;
+            l0[q] = r < bs ? row[lane] : 0.0; l1[q] = r < bs ? row[lane + 32] : 0.0;
         }
+        wait_flag(flags + kb, epoch);
+        const double y0 = __ldcg(y + kb * CB + lane), y1 = __ldcg(y + kb * CB + lane + 32);
+#pragma unroll
+        for (int q = 0; q < 8; q++) acc[q] = fma(l0[q], y0, fma(l1[q], y1, acc[q]));
+    }
+#pragma unroll
+    for (int q = 0; q < 8; q++) {
+        double s = acc[q];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+        const int r = warp * 8 + q;
+        if (lane == 0) blk[r] = r < bs ? dscale[k0 + r] * h[k0 + r] - s : 0.0;
+    }
+    __syncthreads();
+    {   // y_b = Linv_b * rhs: thread (r = tid/4, cq = tid%4) sums the columns c = cq mod 4
+        const int r = tid >> 2, cq = tid & 3;
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < 16; q++) t = fma(Ld[r][4 * q + cq], blk[4 * q + cq], t);
+        t += __shfl_xor_sync(0xffffffffu, t, 1);
+        t += __shfl_xor_sync(0xffffffffu, t, 2);
         __syncthreads();
-        if (warp == 0) {
-            // sequential substitution inside the block, lanes over the rows being updated
-            for (int j = 0; j < bs; j++) {
-                const double xj = blk[j] / Lf[(size_t)(k0 + j) * n + k0 + j];
-                __syncwarp();
-                if (lane == 0) blk[j] = xj;
-                for (int r = j + 1 + lane; r < bs; r += 32) blk[r] -= Lf[(size_t)(k0 + r) * n + k0 + j] * xj;
-                __syncwarp();
-            }
+        if (cq == 0) { blk[r] = t; if (r < bs) y[k0 + r] = t; }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) atomicExch(flags + b, epoch);
+    }
+    // ---------------- backward: columns of this block; thread -> (col = tid % 64, slice = tid / 64)
+    const int col = tid & (CB - 1), slice = tid >> 6;
+    double s = 0.0;
+    for (int kb = nblk - 1; kb > b; kb--) {
+        const int i0 = kb * CB, ibs = min(CB, n - i0);
+        double lv[16];
+#pragma unroll
+        for (int q = 0; q < 16; q++) {
+            const int i = slice + 4 * q;
+            lv[q] = (i < ibs && col < bs) ? Lf[(size_t)(i0 + i) * n + k0 + col] : 0.0;
         }
+        wait_flag(flags + nblk + kb, epoch);
+        if (tid < CB) vec[tid] = tid < ibs ? __ldcg(z + i0 + tid) : 0.0;
         __syncthreads();
-        for (int r = threadIdx.x; r < bs; r += blockDim.x) y[k0 + r] = blk[r];
+#pragma unroll
+        for (int q = 0; q < 16; q++) s = fma(lv[q], vec[slice + 4 * q], s);
         __syncthreads();
     }
-    // ---------------- backward
-    for (int kb = nblk - 1; kb >= 0; kb--) {
-        const int k0 = kb * CB, bs = min(CB, n - k0), t0 = k0 + bs;
-        // s[col] = sum_{i >= t0} L[i][k0+col] z[i]: thread -> (col = tid % 64, slice = tid / 64)
-        {
-            const int col = threadIdx.x & (CB - 1), slice = threadIdx.x >> 6; // 16 slices
-            double s = 0.0;
-            if (col < bs)
-                for (int i = t0 + slice; i < n; i += 16) s = fma(Lf[(size_t)i * n + k0 + col], c[i], s);
-            part[slice][col] = s;
-        }
-        __syncthreads();
-        if (threadIdx.x < bs) {
-            double s = 0.0;
+    part[slice][col] = s;
+    __syncthreads();
+    if (tid < CB) blk[tid] = blk[tid] - (part[0][tid] + part[1][tid] + part[2][tid] + part[3][tid]);
+    __syncthreads();
+    {   // z_b = Linv_b^T * rhs
+        const int cc = tid >> 2, cq = tid & 3;
+        double t = 0.0;
 #pragma unroll
-            for (int k = 0; k < 16; k++) s += part[k][threadIdx.x];
-            blk[threadIdx.x] = y[k0 + threadIdx.x] - s;
-        }
+        for (int q = 0; q < 16; q++) t = fma(Ld[4 * q + cq][cc], blk[4 * q + cq], t);
+        t += __shfl_xor_sync(0xffffffffu, t, 1);
+        t += __shfl_xor_sync(0xffffffffu, t, 2);
+        if (cq == 0 && cc < bs) { z[k0 + cc] = t; c[k0 + cc] = t * dscale[k0 + cc]; }
+        __threadfence();
         __syncthreads();
-        if (warp == 0) {
-            for (int j = bs - 1; j >= 0; j--) {
-                const double xj = blk[j] / Lf[(size_t)(k0 + j) * n + k0 + j];
-                __syncwarp();
-                if (lane == 0) blk[j] = xj;
-                for (int r = lane; r < j; r += 32) blk[r] -= Lf[(size_t)(k0 + j) * n + k0 + r] * xj;
-                __syncwarp();
-            }
-        }
-        __syncthreads();
-        for (int r = threadIdx.x; r < bs; r += blockDim.x) c[k0 + r] = blk[r]; // z, unscaled, read by later blocks
-        __syncthreads();
+        if (tid == 0) atomicExch(flags + nblk + b, epoch);
     }
-    for (int r = threadIdx.x; r < n; r += blockDim.x) c[r] *= dscale[r];
 }
 
 cudaError_t launch_factor(sfft_plan *p) {
@@ -216,26 +283,29 @@ cudaError_t launch_factor(sfft_plan *p) {
     const long long total = (long long)n * n;
     { KLaunch kl(p, "equil_scale"); equil_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p->G, p->dscale, p->Lf, n); }
     const int nblk = (n + CB - 1) / CB;
-    const size_t sm_trsm = 2 * CB * (CB + 1) * sizeof(double), sm_syrk = 2 * CB * CLD * sizeof(double);
-    cudaFuncSetAttribute(trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_trsm);
+    const size_t sm_syrk = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
+    cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * CB * (CB + 1) * sizeof(double)));
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
-        { KLaunch kl(p, "potrf"); potrf_kernel<<<1, 256, 0, st>>>(p->Lf, n, k0, bs, p->flag); }
-        const int rem = n - k0 - bs;
-        if (rem > 0) {
-            const int nt = (rem + CB - 1) / CB;
-            { KLaunch kl(p, "trsm"); trsm_kernel<<<nt, CB, sm_trsm, st>>>(p->Lf, n, k0, bs); }
-            { KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs); }
-        }
+        const int rem = n - k0 - bs, nt = (rem + CB - 1) / CB;
+        { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, 0, st>>>(p->Lf, n, k0, bs, p->flag); }
+        if (rem > 0) { KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs); }
     }
+    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, CB, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Lf, p->Linv, n); }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     return cudaGetLastError();
 }
 
 cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c) {
-    { KLaunch kl(p, "trisolve"); trisolve_kernel<<<1, 1024, 0, p->stream>>>(p->Lf, p->dscale, h, p->ywork, c, p->g.n); }
-    return cudaGetLastError();
+    const int n = p->g.n, nblk = (n + CB - 1) / CB;
+    p->solve_epoch++;
+    const double *Lf = p->Lf, *Li = p->Linv, *ds = p->dscale;
+    double *y = p->ywork, *z = p->zwork;
+    int *flags = p->sflags, epoch = p->solve_epoch, nn = n;
+    void *args[] = {(void *)&Lf, (void *)&Li, (void *)&ds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&flags, (void *)&epoch};
+    KLaunch kl(p, "trisolve");
+    return cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, p->stream);
 }
 
 } // namespace sfft
