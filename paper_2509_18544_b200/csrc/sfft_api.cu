@@ -117,7 +117,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
 
     const size_t plane = (size_t)g.My * g.Hx;
     const int W2 = 4 * g.w + 1, n = g.n;
-    LagCfg cO, cT; lagcol_config(g, p->plO.np, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.w, &cT);
+    LagCfg cO, cT; lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.NK + 1, g.w, &cT);
     const size_t qO = (size_t)cO.nsplit * p->plO.np * W2 * (g.Hx + 1), qT = (size_t)cT.nsplit * p->plT.np * L * (g.Hx + 1);
     const size_t bO = (size_t)border_chunks() * p->plO.np * W2 * W2;
     cudaError_t e = cudaSuccess;

@@ -95,8 +95,8 @@ cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask,
 // columns: inter[ii[k]] * yt^jj[k] -> spec[k] (My x Hx), k = 0..ns-1
 cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj);
 
-struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, rows_per_split; };
-void lagcol_config(const Geom &g, int np, int W, LagCfg *c);
+struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split; };
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c);
 int border_chunks();
 int border_linpair_chunks();
 size_t border_lp_doubles(const Geom &g, int W, int EB);

@@ -31,49 +31,68 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
-constexpr int LC_RT = 8;   // rows per pipeline stage
-constexpr int LC_NST = 3;  // stages
+constexpr int LC_NA = 16;  // decimation factor: ky = b + (My/16) a, a = 0..15
+constexpr int LC_NST = 3;  // cp.async pipeline stages
 
-// grid = (kx blocks, pair groups, ky splits); block = npg * KXC threads (npg = pairs per group).
-// dynamic smem: LC_NST * LC_RT * (ns*KXC + WB) cplx
-template <int WB>
-__global__ void __launch_bounds__(WB > 10 ? 288 : 512)
-lagcol_kernel(SpecSet ss, int ns, PairList pl, int npg, int KXC, int W, int rows_per_split, cplx *__restrict__ Q,
-              Geom g, const cplx *__restrict__ tw) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx *tile = reinterpret_cast<cplx *>(smem_raw);
-    const int Hx = g.Hx, My = g.My;
-    const int stage_elems = LC_RT * (ns * KXC + WB);
+// Stage 1, output-pruned inverse DFT along ky by decimation:
+//   Q[dv] = sum_ky P[ky] e^{2 pi i ky dv/My},  P = conj(A) B,  ky = b + Tb a  (Tb = My/16)
+//         = sum_b e^{2 pi i b dv/My} F_b[dv mod 16],   F_b[m] = sum_a P[b + Tb a] e^{2 pi i a m/16}.
+// A thread owns (pair, kx): per b it forms the 16 products, runs one register-resident 16-point DFT
+// and folds the outputs it needs (DLO <= dv <= DHI) into its accumulators with one complex
+// multiply-add each: ~19 FP64 instructions per spectrum element and pair instead of 4 + 4(2W+1)/2... of the
+// direct sum.  The rows {b + Tb a} of all spectra of the CTA's kx chunk and the W phase factors of b
+// arrive through a cp.async shared-memory pipeline shared by all pairs.
+// grid = (kx blocks, pair groups, b splits * halves); block = npg * KXC threads.
+// dynamic smem: LC_NST * (16 * ns * KXC + WB) cplx
+template <int DLO, int DHI>
+__device__ __forceinline__ void lag_fold(const cplx *x, const cplx *ph, cplx *acc) {
+#pragma unroll
+    for (int d = DLO; d <= DHI; d++) {
+        const cplx v = x[((d % 16) + 16) % 16];
+        cplx &a = acc[d - DLO];
+        if (d == 0) { a.x += v.x; a.y += v.y; }
+        else {
+            const cplx e = ph[(d > 0 ? d : -d) - 1];       // exp(-i phi |d|): cos = e.x, sin = -e.y
+            const double c = e.x, sn = d > 0 ? -e.y : e.y;  // multiply by exp(+i phi d)
+            a.x = fma(v.x, c, a.x); a.x = fma(-v.y, sn, a.x);
+            a.y = fma(v.x, sn, a.y); a.y = fma(v.y, c, a.y);
+        }
+    }
+}
+
+template <int DLO, int DHI, int WB>
+__device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const PairList &pl, int npg, int KXC, int W, int nbs,
+                                            int zsplit, cplx *__restrict__ Q, const Geom &g, const cplx *__restrict__ tw,
+                                            cplx *tile) {
+    const int Hx = g.Hx, My = g.My, Tb = My / LC_NA;
+    const int row_elems = ns * KXC, stage_elems = LC_NA * row_elems + WB;
     const int kx0 = blockIdx.x * KXC;
     const int pl0 = blockIdx.y * npg;
-    const int r0 = blockIdx.z * rows_per_split;
-    const int r1 = min(My, r0 + rows_per_split);
-    const int nIt = (r1 - r0 + LC_RT - 1) / LC_RT;
+    const int b0 = zsplit * nbs, b1 = min(Tb, b0 + nbs);
+    const int nIt = max(0, b1 - b0);
     const int lp = threadIdx.x / KXC, lane = threadIdx.x - lp * KXC;
     const int p = pl0 + lp;
     const bool active = (p < pl.np) && (lp < npg);
     const int sa = active ? pl.a[p] : 0, sb = active ? pl.b[p] : 0;
     const int twsy = g.Nt / My;
-
-    double a0r = 0.0, a0i = 0.0;
-    double s1[WB], s2[WB], s3[WB], s4[WB];
+    constexpr int NACC = DHI - DLO + 1;
+    cplx acc[NACC];
 #pragma unroll
-    for (int d = 0; d < WB; d++) { s1[d] = 0.0; s2[d] = 0.0; s3[d] = 0.0; s4[d] = 0.0; }
+    for (int d = 0; d < NACC; d++) acc[d] = mk(0.0, 0.0);
 
     auto issue = [&](int it) {
         if (it < nIt) {
             cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
-            const int per_row = ns * KXC + WB;
+            const int b = b0 + it;
             for (int e = threadIdx.x; e < stage_elems; e += blockDim.x) {
-                const int r = e / per_row, o = e - r * per_row;
-                int ky = r0 + it * LC_RT + r; if (ky >= r1) ky = r1 - 1;
                 const cplx *src;
-                if (o < ns * KXC) {
+                if (e < LC_NA * row_elems) {
+                    const int a = e / row_elems, o = e - a * row_elems;
                     const int s = o / KXC; int kx = kx0 + (o - s * KXC); if (kx >= Hx) kx = Hx - 1;
-                    src = ss.p[s] + (size_t)ky * Hx + kx;
+                    src = ss.p[s] + (size_t)(b + Tb * a) * Hx + kx;
                 } else {
-                    const int d = o - ns * KXC + 1;
-                    src = tw + (size_t)((ky * d) & (My - 1)) * twsy;
+                    const int d = e - LC_NA * row_elems + 1;
+                    src = tw + (size_t)((b * d) & (My - 1)) * twsy;
                 }
                 cp_async16(st + e, src);
             }
@@ -88,35 +107,40 @@ lagcol_kernel(SpecSet ss, int ns, PairList pl, int npg, int KXC, int W, int rows
         __syncthreads();
         if (active) {
             const cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
-            const int nr = min(LC_RT, r1 - r0 - it * LC_RT);
-            for (int r = 0; r < nr; r++) {
-                const cplx *row = st + r * (ns * KXC + WB);
-                const cplx A = row[sa * KXC + lane], B = row[sb * KXC + lane];
-                const double pr = A.x * B.x + A.y * B.y, pi = A.x * B.y - A.y * B.x;
-                a0r += pr; a0i += pi;
-                const cplx *ph = row + ns * KXC;
+            cplx x[LC_NA];
 #pragma unroll
-                for (int d = 0; d < WB; d++) {
-                    const cplx e = ph[d];            // exp(-i phi): cos = e.x, sin = -e.y
-                    s1[d] = fma(pr, e.x, s1[d]); s2[d] = fma(pi, e.y, s2[d]);
-                    s3[d] = fma(pr, e.y, s3[d]); s4[d] = fma(pi, e.x, s4[d]);
-                }
+            for (int a = 0; a < LC_NA; a++) {
+                const cplx A = st[a * row_elems + sa * KXC + lane], B = st[a * row_elems + sb * KXC + lane];
+                x[a] = cmulc(A, B);
             }
+            dft16<1>(x);
+            lag_fold<DLO, DHI>(x, st + LC_NA * row_elems, acc);
         }
         __syncthreads();
     }
-    // Q[+d] = (S1 - S2) + i(S3 + S4),  Q[-d] = (S1 + S2) + i(S4 - S3)  with sin = -e.y folded in:
-    // s2 = -sum pi*sin, s3 = -sum pr*sin
     const int kx = kx0 + lane;
     if (active && kx < Hx) {
-        cplx *q = Q + ((size_t)(blockIdx.z * pl.np + p) * (2 * W + 1)) * (Hx + 1) + kx;
-        q[(size_t)W * (Hx + 1)] = mk(a0r, a0i);
+        cplx *q = Q + ((size_t)(zsplit * pl.np + p) * (2 * W + 1)) * (Hx + 1) + kx;
 #pragma unroll
-        for (int d = 0; d < WB; d++)
-            if (d < W) {
-                q[(size_t)(W + d + 1) * (Hx + 1)] = mk(s1[d] + s2[d], s4[d] - s3[d]);
-                q[(size_t)(W - d - 1) * (Hx + 1)] = mk(s1[d] - s2[d], s4[d] + s3[d]);
-            }
+        for (int d = DLO; d <= DHI; d++)
+            if (d >= -W && d <= W) q[(size_t)(W + d) * (Hx + 1)] = acc[d - DLO];
+    }
+}
+
+// WB <= 10: one thread folds all 2 WB + 1 lags.  WB = 20: the lag range is split in two halves
+// (blockIdx.z parity) to keep the accumulators in registers; both halves write disjoint rows of Q.
+template <int WB>
+__global__ void __launch_bounds__(192, WB > 10 ? 1 : 2)
+lagcol_kernel(SpecSet ss, int ns, PairList pl, int npg, int KXC, int W, int nbs, cplx *__restrict__ Q, Geom g,
+              const cplx *__restrict__ tw) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx *tile = reinterpret_cast<cplx *>(smem_raw);
+    if (WB > 10) {
+        const int half = blockIdx.z & 1, zs = blockIdx.z >> 1;
+        if (half == 0) lagcol_body<0, WB, WB>(ss, ns, pl, npg, KXC, W, nbs, zs, Q, g, tw, tile);
+        else lagcol_body<-WB, -1, WB>(ss, ns, pl, npg, KXC, W, nbs, zs, Q, g, tw, tile);
+    } else {
+        lagcol_body<-WB, WB, WB>(ss, ns, pl, npg, KXC, W, nbs, blockIdx.z, Q, g, tw, tile);
     }
 }
 
@@ -207,29 +231,41 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
 }
 
 // ---------------------------------------------------------------- host side
-// Launch shape of stage 1 (also used by the plan to size Q).
-void lagcol_config(const Geom &g, int np, int W, LagCfg *c) {
+// Launch shape of stage 1 (also used by the plan to size Q): pick the kx chunk and the b split that
+// minimise  waves * (work per CTA)  on 148 SMs x CTAs per SM, preferring wide chunks and few splits.
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c) {
     const int WB = W <= 3 ? 3 : W <= 5 ? 5 : W <= 6 ? 6 : W <= 10 ? 10 : 20;
-    const int maxthreads = WB > 10 ? 288 : 512;
-    int KXC = maxthreads / np, npg = np;
-    if (KXC < 8) { KXC = 8; npg = maxthreads / KXC; }   // split the pairs into groups, keep 128-byte runs
-    if (KXC > 32) KXC = 32;
-    if (WB <= 10 && np * 14 <= maxthreads && np * 16 > 256 && g.Hx >= 1024) KXC = 14; // Hx=2048: 147 CTAs on 148 SMs
-    if (KXC > g.Hx) KXC = g.Hx;
-    const int nkb = (g.Hx + KXC - 1) / KXC, ngr = (np + npg - 1) / npg;
-    int nsplit = 1;
-    while (nkb * ngr * nsplit < 148 && nsplit < 8 && g.My / (nsplit * 2) >= 64) nsplit *= 2;
-    c->WB = WB; c->KXC = KXC; c->npg = npg; c->nkb = nkb; c->ngr = ngr; c->nsplit = nsplit;
-    c->rows_per_split = (g.My + nsplit - 1) / nsplit;
+    const int halves = WB > 10 ? 2 : 1, per_sm = WB > 10 ? 1 : 2, maxthreads = 192;
+    const int Tb = g.My / LC_NA;
+    double best = 1e300; int bK = 4, bS = 1, bG = np;
+    for (int KXC = 4; KXC <= 32; KXC++) {
+        if (KXC > g.Hx) break;
+        if ((size_t)LC_NST * (LC_NA * ns * KXC + WB) * sizeof(cplx) > (size_t)(per_sm == 2 ? 100 : 200) * 1024) break;
+        int npg = maxthreads / KXC; if (npg > np) npg = np; if (npg < 1) continue;
+        const int ngr = (np + npg - 1) / npg, nkb = (g.Hx + KXC - 1) / KXC;
+        for (int nsplit = 1; nsplit <= 16; nsplit *= 2) {
+            if (Tb / nsplit < 4 && nsplit > 1) break;
+            const long long ncta = (long long)nkb * ngr * nsplit * halves, slots = 148LL * per_sm;
+            const long long waves = (ncta + slots - 1) / slots;
+            // a CTA with few threads keeps the FP64 pipes idle: charge it as if it had at least 160
+            const int thr = npg * KXC < 160 ? 160 : npg * KXC;
+            double cost = (double)waves * thr * ((Tb + nsplit - 1) / nsplit + 6);
+            cost *= 1.0 + 0.01 * nsplit + (KXC < 8 ? 0.03 * (8 - KXC) : 0.0);
+            if (cost < best) { best = cost; bK = KXC; bS = nsplit; bG = npg; }
+        }
+    }
+    c->WB = WB; c->KXC = bK; c->npg = bG; c->nkb = (g.Hx + bK - 1) / bK; c->ngr = (np + bG - 1) / bG;
+    c->nsplit = bS; c->halves = halves;
+    c->rows_per_split = (Tb + bS - 1) / bS; // in units of b
 }
 
 template <int WB>
 static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const PairList &pl, int W, const LagCfg &c, bool science) {
     const Geom &g = p->g;
-    const size_t smem = (size_t)LC_NST * LC_RT * (ns * c.KXC + WB) * sizeof(cplx);
-    cudaError_t e = cudaFuncSetAttribute(lagcol_kernel<WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    const size_t smem = (size_t)LC_NST * (LC_NA * ns * c.KXC + WB) * sizeof(cplx);
+    cudaError_t e = cudaFuncSetAttribute(lagcol_kernel<WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) return e;
-    dim3 grid(c.nkb, c.ngr, c.nsplit);
+    dim3 grid(c.nkb, c.ngr, c.nsplit * c.halves);
     { KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega"); lagcol_kernel<WB><<<grid, c.npg * c.KXC, smem, p->stream>>>(ss, ns, pl, c.npg, c.KXC, W, c.rows_per_split, p->Q, g, p->tw); }
     return cudaGetLastError();
 }
@@ -242,7 +278,7 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     for (int t = 0; t < g.NK; t++) ss.p[t] = p->specT + (size_t)t * g.My * g.Hx;
     ss.p[g.NK] = p->specS;
     const int ns = science ? g.NK + 1 : g.NK;
-    LagCfg c; lagcol_config(g, pl.np, W, &c);
+    LagCfg c; lagcol_config(g, pl.np, ns, W, &c);
     const int nsplit = c.nsplit;
     cudaError_t e;
     if (c.WB == 3) e = run_lagcol<3>(p, ss, ns, pl, W, c, science);
