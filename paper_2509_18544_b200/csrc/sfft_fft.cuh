@@ -127,6 +127,82 @@ template <int R> SFFT_HD void twiddle_powers(cplx *x, cplx w1) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Generic form: E values per thread (E = 8 or 16), T = N/E threads per transform.  Canonical layout:
+// thread j holds elements j + q*T, q = 0..E-1.  Shared-memory indices are padded by one element per E
+// (phys = i + i/E) so that the stride-E scatter of the first pass is bank-conflict free.
+// ---------------------------------------------------------------------------------------------
+template <int E> SFFT_HD int padE(int i) { return i + i / E; }
+template <int E> SFFT_HD int padded_lenE(int N) { return N + N / E; }
+
+// One Stockham pass of radix R (R divides E) on the canonical registers of thread j.
+//   Ns = product of the radices of earlier passes (log2Ns given), tw[k] = exp(-2 pi i k/Nt).
+// STORE: results go to shared memory s (padded) at their autosort positions; otherwise (last pass)
+// they stay canonical in v.
+template <int E, int R, int DIR, bool STORE>
+SFFT_HD void fft_passE(cplx *v, cplx *s, int j, int T, int log2Ns, const cplx *tw, int Nt) {
+    constexpr int NBF = E / R; // butterflies per thread
+    constexpr int LOG2R = (R == 16) ? 4 : (R == 8) ? 3 : (R == 4) ? 2 : 1;
+    const int Ns = 1 << log2Ns;
+#pragma unroll
+    for (int b = 0; b < NBF; b++) {
+        cplx x[R];
+#pragma unroll
+        for (int m = 0; m < R; m++) x[m] = v[b + m * NBF];
+        const int jb = j + b * T;
+        const int k = jb & (Ns - 1);
+        if (log2Ns > 0) {
+            cplx w1 = tw[(size_t)k * (Nt >> (log2Ns + LOG2R))];
+            if (DIR > 0) w1.y = -w1.y;
+            twiddle_powers<R>(x, w1);
+        }
+        dftR<R, DIR>(x);
+        if (STORE) {
+            const int base = ((jb >> log2Ns) << (log2Ns + LOG2R)) + k;
+#pragma unroll
+            for (int m = 0; m < R; m++) s[padE<E>(base + (m << log2Ns))] = x[m];
+        } else {
+#pragma unroll
+            for (int m = 0; m < R; m++) v[b + m * NBF] = x[m];
+        }
+    }
+}
+
+template <int E> SFFT_HD void fft_load_canonicalE(cplx *v, const cplx *s, int j, int T) {
+#pragma unroll
+    for (int q = 0; q < E; q++) v[q] = s[padE<E>(j + q * T)];
+}
+
+#ifdef __CUDACC__
+// Whole FFT of length N = 2^log2N >= 2E for the T = N/E threads of one transform inside a CTA in which
+// EVERY thread calls this with the same N (barriers are CTA-wide).  v canonical in, canonical out.
+template <int DIR, int E>
+__device__ __forceinline__ void fft_blockE(cplx *v, cplx *s, int log2N, int j, const cplx *tw, int Nt) {
+    constexpr int LOG2E = (E == 16) ? 4 : 3;
+    const int T = 1 << (log2N - LOG2E);
+    int log2Ns = 0;
+    __syncthreads();
+    fft_passE<E, E, DIR, true>(v, s, j, T, 0, tw, Nt);
+    __syncthreads();
+    fft_load_canonicalE<E>(v, s, j, T);
+    log2Ns = LOG2E;
+#pragma unroll 1
+    while (log2Ns + LOG2E < log2N) {
+        __syncthreads();
+        fft_passE<E, E, DIR, true>(v, s, j, T, log2Ns, tw, Nt);
+        __syncthreads();
+        fft_load_canonicalE<E>(v, s, j, T);
+        log2Ns += LOG2E;
+    }
+    switch (log2N - log2Ns) {
+    case 4: if (E >= 16) fft_passE<E, (E >= 16 ? 16 : E), DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+    case 3: fft_passE<E, 8, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+    case 2: fft_passE<E, 4, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+    default: fft_passE<E, 2, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+    }
+}
+#endif
+
 // One Stockham pass of radix R on the canonical registers of thread j.
 //   N = FFT length, T = N/16, Ns = product of the radices of earlier passes (log2Ns given),
 //   tw[k] = exp(-2 pi i k / Nt) (Nt >= N, power of two).

@@ -20,7 +20,7 @@ __device__ __forceinline__ double ipow_small(double b, int e) {
 // ------------------------------------------------------------------ row pass
 // grid.x = ceil(ny / RPB); block = RPB * T threads, T = Hx/16.
 // dynamic smem: RPB * padded_len(Hx) cplx  +  RPB * 8 * 8 doubles (moment partials)
-__global__ void __launch_bounds__(256) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
+__global__ void __launch_bounds__(256, 2) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
                                                      cplx *__restrict__ inter, int NI, double *__restrict__ mu, int NMOM,
                                                      Geom g, const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -132,8 +132,8 @@ __global__ void __launch_bounds__(512) col_fwd_kernel(const cplx *__restrict__ i
 
 static int row_cfg(const Geom &g, int *threads, size_t *smem) {
     const int T = g.Hx >> 4;
-    int RPB = 256 / T; if (RPB < 1) RPB = 1;
-    *threads = RPB * T;
+    int RPB = 64 / T; if (RPB < 1) RPB = 1;   // one row per CTA once a row has >= 64 threads: several small CTAs per SM
+    *threads = RPB * T;                        // run in different phases (load / butterflies / store) and overlap
     *smem = (size_t)RPB * padded_len(g.Hx) * sizeof(cplx) + (size_t)RPB * 64 * sizeof(double);
     return RPB;
 }

@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(512) col_inv_kernel(const cplx *__restrict__ s
 }
 
 // grid.x = ceil(ny/RPB); block = RPB*T, T = Hx/16.  dynamic smem: RPB*padded_len(Hx) cplx
-__global__ void __launch_bounds__(256) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
+__global__ void __launch_bounds__(256, 2) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
                                                      const double *__restrict__ coef, double *__restrict__ D, Geom g,
                                                      const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -248,7 +248,7 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
     }
     { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw); }
     const int T = g.Hx >> 4;
-    int RPB = 256 / T; if (RPB < 1) RPB = 1;
+    int RPB = 64 / T; if (RPB < 1) RPB = 1;
     const size_t rsmem = (size_t)RPB * padded_len(g.Hx) * sizeof(cplx);
     { KLaunch kl(p, "row_inv"); row_inv_kernel<<<(g.ny + RPB - 1) / RPB, RPB * T, rsmem, st>>>(p->inter, S, coef, D, g, p->tw); }
     if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
