@@ -7,6 +7,7 @@
 // kx = 0..Hx, stored as Hx complex columns with column 0 = X[0] + i X[Hx] (both real).
 // The column pass transforms that packed column like any other (it is then the sum
 // F0 + i FH of two Hermitian column spectra; consumers untangle it, see sfft_assemble.cu).
+#include <cstdlib>
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -18,29 +19,30 @@ __device__ __forceinline__ double ipow_small(double b, int e) {
 }
 
 // ------------------------------------------------------------------ row pass
-// grid.x = ceil(ny / RPB); block = RPB * T threads, T = Hx/16.
-// dynamic smem: RPB * padded_len(Hx) cplx  +  RPB * 8 * 8 doubles (moment partials)
-__global__ void __launch_bounds__(256, 2) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
+// grid.x = ceil(ny / RPB); block = RPB * T threads, T = Hx/E (E values per thread).
+// dynamic smem: RPB * padded_lenE<E>(Hx) cplx  +  RPB * 8 * 8 doubles (moment partials)
+template <int E>
+__global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
                                                      cplx *__restrict__ inter, int NI, double *__restrict__ mu, int NMOM,
                                                      Geom g, const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Hx = g.Hx, T = Hx >> 4;
+    const int Hx = g.Hx, T = Hx / E;
     const int RPB = blockDim.x / T;
     const int rib = threadIdx.x / T, j = threadIdx.x - rib * T;
     const int row = blockIdx.x * RPB + rib;
     const bool live = row < g.ny;
-    cplx *s = reinterpret_cast<cplx *>(smem_raw) + (size_t)rib * padded_len(Hx);
-    double *wpart = reinterpret_cast<double *>(reinterpret_cast<cplx *>(smem_raw) + (size_t)RPB * padded_len(Hx));
+    cplx *s = reinterpret_cast<cplx *>(smem_raw) + (size_t)rib * padded_lenE<E>(Hx);
+    double *wpart = reinterpret_cast<double *>(reinterpret_cast<cplx *>(smem_raw) + (size_t)RPB * padded_lenE<E>(Hx));
     const double inv_nx = 1.0 / (double)g.nx;
     const size_t rowoff = (size_t)row * g.nx;
 
     for (int i = 0; i < NI; i++) {
-        cplx v[16];
+        cplx v[E];
         double mom[8];
 #pragma unroll
         for (int m = 0; m < 8; m++) mom[m] = 0.0;
 #pragma unroll
-        for (int q = 0; q < 16; q++) {
+        for (int q = 0; q < E; q++) {
             const int x0 = 2 * (j + q * T);
             double a = 0.0, b = 0.0;
             if (live) {
@@ -76,17 +78,17 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const double *__restric
                     mu[(size_t)m * g.ny + row] = acc;
                 }
         }
-        fft_block<-1>(v, s, g.log2Hx, j, tw, g.Nt);
+        fft_blockE<-1, E>(v, s, g.log2Hx, j, tw, g.Nt);
         __syncthreads();
 #pragma unroll
-        for (int q = 0; q < 16; q++) s[pad16(j + q * T)] = v[q];
+        for (int q = 0; q < E; q++) s[padE<E>(j + q * T)] = v[q];
         __syncthreads();
         // untangle: X[k] = E[k] + exp(-2 pi i k/Mx) O[k],  E = (Z[k] + conj Z[Hx-k])/2, O = (Z[k] - conj Z[Hx-k])/(2i)
         cplx *dst = inter + ((size_t)i * g.ny + row) * Hx;
 #pragma unroll
-        for (int q = 0; q < 16; q++) {
+        for (int q = 0; q < E; q++) {
             const int k = j + q * T;
-            const cplx A = s[pad16(k)], B = cconj(s[pad16((Hx - k) & (Hx - 1))]);
+            const cplx A = s[padE<E>(k)], B = cconj(s[padE<E>((Hx - k) & (Hx - 1))]);
             const cplx E = mk(0.5 * (A.x + B.x), 0.5 * (A.y + B.y));
             const cplx O = mk(0.5 * (A.y - B.y), -0.5 * (A.x - B.x));
             cplx X;
@@ -100,7 +102,6 @@ __global__ void __launch_bounds__(256, 2) row_fwd_kernel(const double *__restric
 // ------------------------------------------------------------------ column pass
 // block b -> (spectrum k = b % ns, column group b / ns); C columns per CTA, T = My/16 threads each,
 // thread tid -> (c = tid % C, j = tid / C).  dynamic smem: C * padded_len(My) cplx.
-struct ColJobs { int ns; int ii[MAX_NP]; int jj[MAX_NP]; };
 
 __global__ void __launch_bounds__(512) col_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJobs jobs,
                                                      int C, Geom g, const cplx *__restrict__ tw) {
@@ -130,11 +131,21 @@ __global__ void __launch_bounds__(512) col_fwd_kernel(const cplx *__restrict__ i
     for (int q = 0; q < 16; q++) dst[(size_t)(j + q * T) * Hx] = v[q];
 }
 
-static int row_cfg(const Geom &g, int *threads, size_t *smem) {
-    const int T = g.Hx >> 4;
+// values per thread of the row / column transforms: 8 keeps a thread under 64 registers (twice the
+// resident warps of 16) at the price of one more shared-memory exchange; SFFT_ROW_E / SFFT_COL_E override
+int fft_E(const char *env, int N, int dflt) {
+    int E = dflt;
+    if (const char *s = getenv(env)) E = atoi(s) == 8 ? 8 : 16;
+    if (N / 8 > 256 && E == 8) E = 16;   // a transform is at most 256 threads
+    if (N < 32) E = 8;
+    return E;
+}
+
+int row_cfg(const Geom &g, int E, int *threads, size_t *smem) {
+    const int T = g.Hx / E;
     int RPB = 64 / T; if (RPB < 1) RPB = 1;   // one row per CTA once a row has >= 64 threads: several small CTAs per SM
     *threads = RPB * T;                        // run in different phases (load / butterflies / store) and overlap
-    *smem = (size_t)RPB * padded_len(g.Hx) * sizeof(cplx) + (size_t)RPB * 64 * sizeof(double);
+    *smem = (size_t)RPB * (E == 8 ? padded_lenE<8>(g.Hx) : padded_lenE<16>(g.Hx)) * sizeof(cplx) + (size_t)RPB * 64 * sizeof(double);
     return RPB;
 }
 
@@ -149,19 +160,30 @@ int col_cfg(const Geom &g, int *threads, size_t *smem) {
 cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI, double *mu, int NMOM) {
     const Geom &g = p->g;
     int threads; size_t smem;
-    const int RPB = row_cfg(g, &threads, &smem);
+    const int E = fft_E("SFFT_ROW_E", g.Hx, 16);
+    const int RPB = row_cfg(g, E, &threads, &smem);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    { KLaunch kl(p, NI > 1 ? "row_fwd_R" : "row_fwd_S"); row_fwd_kernel<<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw); }
+    {
+        KLaunch kl(p, NI > 1 ? "row_fwd_R" : "row_fwd_S");
+        if (E == 8) row_fwd_kernel<8><<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+        else row_fwd_kernel<16><<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+    }
     return cudaGetLastError();
 }
 
 cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj) {
     const Geom &g = p->g;
+    if (colpipe_ok(g)) {
+        int nsrc = 0;
+        for (int k = 0; k < ns; k++) if (ii[k] + 1 > nsrc) nsrc = ii[k] + 1;
+        return launch_colpipe_fwd(p, inter, spec, ns, ii, jj, nsrc);
+    }
     int threads; size_t smem;
     const int C = col_cfg(g, &threads, &smem);
     static bool attr_set = false;

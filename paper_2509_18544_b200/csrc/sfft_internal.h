@@ -95,6 +95,11 @@ cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask,
 // columns: inter[ii[k]] * yt^jj[k] -> spec[k] (My x Hx), k = 0..ns-1
 cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj);
 
+struct ColJobs { int ns; int ii[MAX_NP]; int jj[MAX_NP]; };   // column-pass outputs: spec[k] = FFT_y(yt^jj[k] * inter[ii[k]])
+bool colpipe_ok(const Geom &g);
+cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj, int nsrc);
+cudaError_t launch_colpipe_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter);
+
 struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split; };
 void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c);
 int border_chunks();

@@ -108,40 +108,41 @@ __global__ void __launch_bounds__(512) col_inv_kernel(const cplx *__restrict__ s
     }
 }
 
-// grid.x = ceil(ny/RPB); block = RPB*T, T = Hx/16.  dynamic smem: RPB*padded_len(Hx) cplx
-__global__ void __launch_bounds__(256, 2) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
+// grid.x = ceil(ny/RPB); block = RPB*T, T = Hx/E.  dynamic smem: RPB*padded_lenE<E>(Hx) cplx
+template <int E>
+__global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
                                                      const double *__restrict__ coef, double *__restrict__ D, Geom g,
                                                      const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Hx = g.Hx, T = Hx >> 4;
+    const int Hx = g.Hx, T = Hx / E;
     const int RPB = blockDim.x / T;
     const int rib = threadIdx.x / T, j = threadIdx.x - rib * T;
     const int row = blockIdx.x * RPB + rib;
     const bool live = row < g.ny;
-    cplx *s = reinterpret_cast<cplx *>(smem_raw) + (size_t)rib * padded_len(Hx);
+    cplx *s = reinterpret_cast<cplx *>(smem_raw) + (size_t)rib * padded_lenE<E>(Hx);
     const cplx *src = inter + (size_t)row * Hx;
 #pragma unroll
-    for (int q = 0; q < 16; q++) {
+    for (int q = 0; q < E; q++) {
         const int k = j + q * T;
-        s[pad16(k)] = live ? src[k] : mk(0, 0);
+        s[padE<E>(k)] = live ? src[k] : mk(0, 0);
     }
     __syncthreads();
-    cplx v[16];
+    cplx v[E];
 #pragma unroll
-    for (int q = 0; q < 16; q++) {
+    for (int q = 0; q < E; q++) {
         const int k = j + q * T;
         if (k == 0) {
             const cplx X = s[0]; // (DC, Nyquist), both real
             v[q] = mk(0.5 * (X.x + X.y), 0.5 * (X.x - X.y));
         } else {
-            const cplx A = s[pad16(k)], B = cconj(s[pad16(Hx - k)]);
+            const cplx A = s[padE<E>(k)], B = cconj(s[padE<E>(Hx - k)]);
             const cplx Ev = mk(0.5 * (A.x + B.x), 0.5 * (A.y + B.y));
             cplx e = tw[(size_t)k * (g.Nt / g.Mx)]; e.y = -e.y; // exp(+2 pi i k/Mx)
             const cplx Od = cmul(mk(0.5 * (A.x - B.x), 0.5 * (A.y - B.y)), e);
             v[q] = mk(Ev.x - Od.y, Ev.y + Od.x); // E + i O
         }
     }
-    fft_block<1>(v, s, g.log2Hx, j, tw, g.Nt);
+    fft_blockE<1, E>(v, s, g.log2Hx, j, tw, g.Nt);
     if (!live) return;
     // background polynomial of this row: B(x) = sum_p cx[p] xt^p, cx[p] = sum_q b_(p,q) yt^q
     double cx[MAX_DEG + 1];
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(256, 2) row_inv_kernel(const cplx *__restrict_
     const size_t ro = (size_t)row * g.nx;
     const bool vec = ((g.nx & 1) == 0) && (((size_t)S | (size_t)D) & 15) == 0;
 #pragma unroll
-    for (int q = 0; q < 16; q++) {
+    for (int q = 0; q < E; q++) {
         const int x0 = 2 * (j + q * T);
         if (x0 >= g.nx) continue;
         const double xa = (2.0 * x0 + 1.0 - g.nx) * inx, xb = (2.0 * x0 + 3.0 - g.nx) * inx;
@@ -231,26 +232,35 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
 }
 
 int col_cfg(const Geom &g, int *threads, size_t *smem); // sfft_fwd.cu
+int row_cfg(const Geom &g, int E, int *threads, size_t *smem);
+int fft_E(const char *env, int N, int dflt);
 
 cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D) {
     const Geom &g = p->g;
     cudaStream_t st = p->stream;
-    { KLaunch kl(p, "ktab"); ktab_kernel<<<dim3((g.Hx + 1 + 127) / 128, g.w + 1, g.NK), 128, 0, st>>>(coef, p->E, g, p->tw); }
+    const bool pipe = colpipe_ok(g);
+    if (!pipe) { KLaunch kl(p, "ktab"); ktab_kernel<<<dim3((g.Hx + 1 + 127) / 128, g.w + 1, g.NK), 128, 0, st>>>(coef, p->E, g, p->tw); }
     int threads; size_t smem;
     const int C = col_cfg(g, &threads, &smem);
     smem += (size_t)g.NK * g.L * (C + 1) * sizeof(cplx);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(col_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw); }
-    const int T = g.Hx >> 4;
-    int RPB = 64 / T; if (RPB < 1) RPB = 1;
-    const size_t rsmem = (size_t)RPB * padded_len(g.Hx) * sizeof(cplx);
-    { KLaunch kl(p, "row_inv"); row_inv_kernel<<<(g.ny + RPB - 1) / RPB, RPB * T, rsmem, st>>>(p->inter, S, coef, D, g, p->tw); }
+    if (pipe) { cudaError_t e = launch_colpipe_inv(p, p->specTo, coef, p->inter); if (e != cudaSuccess) return e; }
+    else { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw); }
+    const int ER = fft_E("SFFT_ROW_E", g.Hx, 16);
+    int rthreads; size_t rsmem;
+    const int RPB = row_cfg(g, ER, &rthreads, &rsmem);
+    {
+        KLaunch kl(p, "row_inv");
+        if (ER == 8) row_inv_kernel<8><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
+        else row_inv_kernel<16><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
+    }
     if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
         const long long nb = 2LL * g.w * g.nx + 2LL * g.w * (g.ny - 2 * g.w);
         KLaunch kl(p, "wrapfix");
