@@ -80,22 +80,32 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
 #pragma unroll
     for (int d = 0; d < NACC; d++) acc[d] = mk(0.0, 0.0);
 
+    // division-free tile copy: a thread copies the same (spectrum, kx) column slots of every stage
+    // (row_elems <= 2 blockDim: np >= ns - 1), 16 rows each, plus one phase factor
+    const cplx *gsrc[2]; int soff[2];
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+        const int idx = threadIdx.x + u * blockDim.x;
+        gsrc[u] = nullptr; soff[u] = 0;
+        if (idx < row_elems) {
+            const int s = idx / KXC; int kx = kx0 + (idx - s * KXC); if (kx >= Hx) kx = Hx - 1;
+            gsrc[u] = ss.p[s] + kx; soff[u] = idx;
+        }
+    }
+    const size_t astride = (size_t)Tb * Hx;
     auto issue = [&](int it) {
         if (it < nIt) {
             cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
             const int b = b0 + it;
-            for (int e = threadIdx.x; e < stage_elems; e += blockDim.x) {
-                const cplx *src;
-                if (e < LC_NA * row_elems) {
-                    const int a = e / row_elems, o = e - a * row_elems;
-                    const int s = o / KXC; int kx = kx0 + (o - s * KXC); if (kx >= Hx) kx = Hx - 1;
-                    src = ss.p[s] + (size_t)(b + Tb * a) * Hx + kx;
-                } else {
-                    const int d = e - LC_NA * row_elems + 1;
-                    src = tw + (size_t)((b * d) & (My - 1)) * twsy;
+#pragma unroll
+            for (int u = 0; u < 2; u++)
+                if (gsrc[u]) {
+                    const cplx *src = gsrc[u] + (size_t)b * Hx;
+#pragma unroll
+                    for (int a = 0; a < LC_NA; a++) cp_async16(st + a * row_elems + soff[u], src + a * astride);
                 }
-                cp_async16(st + e, src);
-            }
+            for (int d = threadIdx.x; d < WB; d += blockDim.x)
+                cp_async16(st + LC_NA * row_elems + d, tw + (size_t)((b * (d + 1)) & (My - 1)) * twsy);
         }
         cp_async_commit();
     };
