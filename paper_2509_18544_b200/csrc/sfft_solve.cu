@@ -49,49 +49,67 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
         areg[q] = v;
         xr[q] = (have_rows && r0 + r < n && c < bs) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
     }
+    // Rolled over the 16 column groups (4 columns each) so the code stays small: the register window is
+    // shifted down by one group per iteration, areg[qq] holds columns 4 (j4 + qq) + cq.
+#pragma unroll 1
+    for (int j4 = 0; j4 < CB / 4; j4++) {
+        const int lim = ((r - cq) >> 2) - j4; // r >= cq is not guaranteed: arithmetic shift keeps lim < 0 then
 #pragma unroll
-    for (int j = 0; j < CB; j++) {
-        double *cj = col[j & 1];
-        if (cq == (j & 3) && r >= j) cj[r] = areg[j >> 2];
-        __syncthreads();
-        double piv = cj[j];
-        if (!(piv > PIVOT_MIN)) { if (tid == 0 && blockIdx.x == 0) *flag = 1; piv = 1.0; }
-        const double inv = rsqrt(piv);
-        const double lr = (r == j) ? piv * inv : cj[r] * inv;
-        if (tid == 0) rd[j] = inv;
-        if (cq == (j & 3) && r >= j) areg[j >> 2] = lr;
-        if (r > j) {
+        for (int jj = 0; jj < 4; jj++) {
+            const int j = 4 * j4 + jj;
+            double *cj = col[jj & 1];
+            if (cq == jj && r >= j) cj[r] = areg[0];
+            __syncthreads();
+            double piv = cj[j];
+            if (!(piv > PIVOT_MIN)) { if (tid == 0 && blockIdx.x == 0) *flag = 1; piv = 1.0; }
+            const double inv = rsqrt(piv);
+            const double lr = (r == j) ? piv * inv : cj[r] * inv;
+            if (tid == 0) rd[j] = inv;
+            if (cq == jj && r >= j) areg[0] = lr;
+            if (r > j) {
+                // c = 4 (j4 + qq) + cq in (j, r]:  qq <= lim  (and cq > jj for qq = 0)
+                const double lri = -lr * inv;
+                const double *cjc = cj + 4 * j4 + cq;
+                if (cq > jj && lim >= 0) areg[0] = fma(lri, cjc[0], areg[0]);
 #pragma unroll
-            for (int q = j >> 2; q < 16; q++) {
-                const int c = 4 * q + cq;
-                if (c > j && c <= r) areg[q] = fma(-lr, cj[c] * inv, areg[q]);
+                for (int qq = 1; qq < 16; qq++)
+                    if (qq <= lim) areg[qq] = fma(lri, cjc[4 * qq], areg[qq]);
             }
         }
-    }
+        {
+            const int c = 4 * j4 + cq;
+            l[r][c] = c <= r ? areg[0] : 0.0;
+            if (blockIdx.x == 0 && r < bs && c <= r) Lf[(size_t)(k0 + r) * n + k0 + c] = areg[0];
+        }
 #pragma unroll
-    for (int q = 0; q < 16; q++) {
-        const int c = 4 * q + cq;
-        l[r][c] = c <= r ? areg[q] : 0.0;
-        if (blockIdx.x == 0 && r < bs && c <= r) Lf[(size_t)(k0 + r) * n + k0 + c] = areg[q];
+        for (int qq = 0; qq < 15; qq++) areg[qq] = areg[qq + 1];
+        areg[15] = 0.0;
     }
     __syncthreads();
     if (!have_rows) return;
-    // x_j = x_j / l_jj, then x_c -= x_j l_cj for c > j; lanes 4g..4g+3 hold row r
+    // panel rows: x_j = x_j / l_jj, then x_c -= x_j l_cj for c > j; lanes 4g..4g+3 hold row r; same window shift
+#pragma unroll 1
+    for (int j4 = 0; j4 < CB / 4; j4++) {
 #pragma unroll
-    for (int j = 0; j < CB; j++) {
-        double xj = xr[j >> 2] * rd[j];
-        xj = __shfl_sync(0xffffffffu, xj, (lane & ~3) | (j & 3));
-        if (cq == (j & 3)) xr[j >> 2] = xj;
+        for (int jj = 0; jj < 4; jj++) {
+            const int j = 4 * j4 + jj;
+            double xj = xr[0] * rd[j];
+            xj = __shfl_sync(0xffffffffu, xj, (lane & ~3) | jj);
+            if (cq == jj) xr[0] = xj;
+            const double *lc = &l[4 * j4 + cq][j];
+            const double nxj = -xj;
+            if (cq > jj) xr[0] = fma(nxj, lc[0], xr[0]);
 #pragma unroll
-        for (int q = j >> 2; q < 16; q++) {
-            const int c = 4 * q + cq;
-            if (c > j) xr[q] = fma(-xj, l[c][j], xr[q]);
+            for (int qq = 1; qq < 16; qq++)
+                if (qq < CB / 4 - j4) xr[qq] = fma(nxj, lc[(size_t)4 * qq * (CB + 1)], xr[qq]);
         }
-    }
+        {
+            const int c = 4 * j4 + cq;
+            if (r0 + r < n && c < bs) Lf[(size_t)(r0 + r) * n + k0 + c] = xr[0];
+        }
 #pragma unroll
-    for (int q = 0; q < 16; q++) {
-        const int c = 4 * q + cq;
-        if (r0 + r < n && c < bs) Lf[(size_t)(r0 + r) * n + k0 + c] = xr[q];
+        for (int qq = 0; qq < 15; qq++) xr[qq] = xr[qq + 1];
+        xr[15] = 0.0;
     }
 }
 
