@@ -81,6 +81,9 @@ static void free_plan(sfft_plan *p) {
         if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
         if (p->ev1[s]) cudaEventDestroy(p->ev1[s]);
     }
+    if (p->side) cudaStreamDestroy(p->side);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     for (int k = 0; k < MAX_KREC; k++)
         if (p->krec[k].e0) { cudaEventDestroy(p->krec[k].e0); cudaEventDestroy(p->krec[k].e1); }
     delete p;
@@ -162,7 +165,10 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     }
     *p->flag_host = 0;
     for (int s = 0; s < SFFT_NUM_STAGES; s++) { cudaEventCreate(&p->ev0[s]); cudaEventCreate(&p->ev1[s]); }
-    p->stream = 0;
+    p->stream = 0; p->cur = 0;
+    cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
+    cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
     // Phi (pin P7): closed form, mask independent
     double phi[MAX_NP * MAX_NP];
@@ -181,7 +187,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
 
 sfft_status sfft_plan_set_stream(sfft_plan *p, void *cuda_stream) {
     if (!p) return SFFT_ERR_INVALID_ARG;
-    p->stream = (cudaStream_t)cuda_stream;
+    p->stream = (cudaStream_t)cuda_stream; p->cur = p->stream;
     return SFFT_OK;
 }
 
@@ -220,8 +226,10 @@ static sfft_status template_side(sfft_plan *p) {
     }
     {
         StageTimer tm(p, SFFT_STAGE_A2_OMEGA);
-        CK(launch_lags(p, p->plO, 2 * g.w, p->lagO, false), "lags(Omega)");
-        CK(launch_gamma(p), "gamma");
+        fork_side(p);
+        CK(launch_gamma(p), "gamma");           // on the side stream, beside the Omega column pass
+        back_to_main(p);
+        CK(launch_lags(p, p->plO, 2 * g.w, p->lagO, false), "lags(Omega)"); // joins the side stream
     }
     {
         StageTimer tm(p, SFFT_STAGE_A3_GATHER);
@@ -241,8 +249,10 @@ static sfft_status science_side(sfft_plan *p) {
     }
     {
         StageTimer tm(p, SFFT_STAGE_A2_THETA);
-        CK(launch_lags(p, p->plT, g.w, p->lagT, true), "lags(Theta)");
+        fork_side(p);
         CK(launch_delta(p), "delta");
+        back_to_main(p);
+        CK(launch_lags(p, p->plT, g.w, p->lagT, true), "lags(Theta)");
         CK(launch_gather_h(p), "gather h");
     }
     return SFFT_OK;
@@ -345,6 +355,7 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
 sfft_status sfft_sync_status(sfft_plan *p) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     CK(cudaStreamSynchronize(p->stream), "sync");
+    if (p->side) CK(cudaStreamSynchronize(p->side), "sync side");
     if (p->have_factor) {
         CK(cudaMemcpy(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost), "read flag");
         if (*p->flag_host) return fail(p, SFFT_ERR_NOT_SPD, "pivot <= 1e-12: matrix not positive definite");

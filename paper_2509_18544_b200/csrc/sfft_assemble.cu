@@ -129,24 +129,24 @@ __global__ void gather_h_kernel(const double *__restrict__ lagT, const double *_
 cudaError_t launch_gamma(sfft_plan *p) {
     const Geom &g = p->g;
     const long long total = (long long)(g.DK + 1) * (g.DB + 1) * g.L * g.ny;
-    { KLaunch kl(p, "gamma_rows"); gamma_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->stream>>>(p->muR, p->R, p->mask, p->gamA, g); }
-    { KLaunch kl(p, "gamma_cols"); gamma_cols_kernel<<<dim3(g.L * g.L, g.NB, g.NK), 128, 0, p->stream>>>(p->gamA, p->gam, g); }
+    { KLaunch kl(p, "gamma_rows"); gamma_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->muR, p->R, p->mask, p->gamA, g); }
+    { KLaunch kl(p, "gamma_cols"); gamma_cols_kernel<<<dim3(g.L * g.L, g.NB, g.NK), 128, 0, p->cur>>>(p->gamA, p->gam, g); }
     return cudaGetLastError();
 }
 
 cudaError_t launch_delta(sfft_plan *p) {
-    { KLaunch kl(p, "delta"); delta_kernel<<<p->g.NB, 128, 0, p->stream>>>(p->muS, p->delta, p->g); }
+    { KLaunch kl(p, "delta"); delta_kernel<<<p->g.NB, 128, 0, p->cur>>>(p->muS, p->delta, p->g); }
     return cudaGetLastError();
 }
 
 cudaError_t launch_gather_G(sfft_plan *p) {
     const long long total = (long long)p->g.n * p->g.n;
-    { KLaunch kl(p, "gather_G"); gather_G_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->stream>>>(p->lagO, p->gam, p->phi, p->G, p->g); }
+    { KLaunch kl(p, "gather_G"); gather_G_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->lagO, p->gam, p->phi, p->G, p->g); }
     return cudaGetLastError();
 }
 
 cudaError_t launch_gather_h(sfft_plan *p) {
-    { KLaunch kl(p, "gather_h"); gather_h_kernel<<<(p->g.n + 255) / 256, 256, 0, p->stream>>>(p->lagT, p->delta, p->h, p->g); }
+    { KLaunch kl(p, "gather_h"); gather_h_kernel<<<(p->g.n + 255) / 256, 256, 0, p->cur>>>(p->lagT, p->delta, p->h, p->g); }
     return cudaGetLastError();
 }
 

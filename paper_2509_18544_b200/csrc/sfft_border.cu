@@ -167,7 +167,7 @@ int border_linpair_chunks() { return 4; }
 template <int EA, int EB>
 static void run_linpair(sfft_plan *p, const double *SBa, const double *SBb, int W, int NL, int CH, int nchunk) {
     const size_t smem = (size_t)(2 * CH + 2 * W) * sizeof(double);
-    linpair_kernel<EA, EB><<<dim3(nchunk, W * W, 4), 256, smem, p->stream>>>(SBa, SBb, W, NL, CH, p->LP, p->g);
+    linpair_kernel<EA, EB><<<dim3(nchunk, W * W, 4), 256, smem, p->cur>>>(SBa, SBb, W, NL, CH, p->LP, p->g);
 }
 
 // bpart[pair][(2W+1)^2] <- X_N - X_M for the pair list (science: b = m.S, else b = the template images)
@@ -180,7 +180,7 @@ cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science,
     {
         KLaunch kl(p, science ? "strip_gather_S" : "strip_gather_R");
         // template strips are gathered with the template's W on the Omega call and again (narrower) on Theta calls
-        strip_gather_kernel<<<dim3((NL + 255) / 256, W, science ? 8 : 4), 256, 0, p->stream>>>(p->R, p->S, p->mask, SB, W, NL, 0, g);
+        strip_gather_kernel<<<dim3((NL + 255) / 256, W, science ? 8 : 4), 256, 0, p->cur>>>(p->R, p->S, p->mask, SB, W, NL, 0, g);
     }
     {
         KLaunch kl(p, science ? "linpair_theta" : "linpair_omega");
@@ -201,7 +201,7 @@ cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science,
     {
         KLaunch kl(p, science ? "border_combine_theta" : "border_combine_omega");
         const int total = pl.np * (2 * W + 1) * (2 * W + 1);
-        border_combine_kernel<<<(total + 127) / 128, 128, 0, p->stream>>>(p->LP, nchunk, W, g.DK + 1, science ? 1 : g.DK + 1, pl,
+        border_combine_kernel<<<(total + 127) / 128, 128, 0, p->cur>>>(p->LP, nchunk, W, g.DK + 1, science ? 1 : g.DK + 1, pl,
                                                                             science ? 1 : 0, p->R, p->S, p->mask, bpart, g);
     }
     return cudaGetLastError();

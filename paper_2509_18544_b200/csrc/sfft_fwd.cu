@@ -160,7 +160,7 @@ int col_cfg(const Geom &g, int *threads, size_t *smem) {
 cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI, double *mu, int NMOM) {
     const Geom &g = p->g;
     int threads; size_t smem;
-    const int E = fft_E("SFFT_ROW_E", g.Hx, 16);
+    const int E = fft_E("SFFT_ROW_E", g.Hx, 8);
     const int RPB = row_cfg(g, E, &threads, &smem);
     static bool attr_set = false;
     if (!attr_set) {

@@ -39,7 +39,10 @@ struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of
 
 struct sfft_plan {
     sfft::Geom g;
-    cudaStream_t stream;
+    cudaStream_t stream;     // the caller's stream: every call is ordered on it
+    cudaStream_t side;       // plan-owned: small independent kernels run beside the big ones (fork/join by events)
+    cudaStream_t cur;        // stream the launchers enqueue on right now (stream, or side inside a fork)
+    cudaEvent_t ev_fork, ev_join;
     // device workspaces
     sfft::cplx *tw;          // [Nt]
     sfft::cplx *inter;       // [(DK+1)][ny][Hx] row-transformed intermediates (a1) / a5 intermediate
@@ -134,11 +137,25 @@ struct KLaunch {
             r = &p->krec[p->nkrec];
             if (!r->e0) { cudaEventCreate(&r->e0); cudaEventCreate(&r->e1); }
             r->name = name; p->nkrec++;
-            cudaEventRecord(r->e0, p->stream);
+            cudaEventRecord(r->e0, p->cur);
         }
     }
-    ~KLaunch() { if (r) cudaEventRecord(r->e1, p->stream); }
+    ~KLaunch() { if (r) cudaEventRecord(r->e1, p->cur); }
 };
+
+// side stream: fork = side waits for everything enqueued on the main stream so far; join = main waits for side.
+// In per-launch timing mode everything stays on the main stream so that kernel times do not overlap.
+inline void fork_side(sfft_plan *p) {
+    if (p->ktiming || !p->side) return;
+    cudaEventRecord(p->ev_fork, p->stream); cudaStreamWaitEvent(p->side, p->ev_fork, 0);
+    p->cur = p->side;
+}
+inline void back_to_main(sfft_plan *p) { p->cur = p->stream; }
+inline void join_side(sfft_plan *p) {
+    p->cur = p->stream;
+    if (p->ktiming || !p->side) return;
+    cudaEventRecord(p->ev_join, p->side); cudaStreamWaitEvent(p->stream, p->ev_join, 0);
+}
 
 inline int ilog2(int v) { int l = 0; while ((1 << l) < v) l++; return l; }
 

@@ -129,7 +129,7 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
         __syncthreads();
     }
     const int kx = kx0 + lane;
-    if (active && kx < Hx) {
+    if (active && kx < Hx && kx > 0) { // kx = 0 is the packed column: lagedge_kernel owns Q[.][.][0]
         cplx *q = Q + ((size_t)(zsplit * pl.np + p) * (2 * W + 1)) * (Hx + 1) + kx;
 #pragma unroll
         for (int d = DLO; d <= DHI; d++)
@@ -276,7 +276,7 @@ static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const Pai
     cudaError_t e = cudaFuncSetAttribute(lagcol_kernel<WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) return e;
     dim3 grid(c.nkb, c.ngr, c.nsplit * c.halves);
-    { KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega"); lagcol_kernel<WB><<<grid, c.npg * c.KXC, smem, p->stream>>>(ss, ns, pl, c.npg, c.KXC, W, c.rows_per_split, p->Q, g, p->tw); }
+    { KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega"); lagcol_kernel<WB><<<grid, c.npg * c.KXC, smem, p->cur>>>(ss, ns, pl, c.npg, c.KXC, W, c.rows_per_split, p->Q, g, p->tw); }
     return cudaGetLastError();
 }
 
@@ -291,13 +291,9 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     LagCfg c; lagcol_config(g, pl.np, ns, W, &c);
     const int nsplit = c.nsplit;
     cudaError_t e;
-    if (c.WB == 3) e = run_lagcol<3>(p, ss, ns, pl, W, c, science);
-    else if (c.WB == 5) e = run_lagcol<5>(p, ss, ns, pl, W, c, science);
-    else if (c.WB == 6) e = run_lagcol<6>(p, ss, ns, pl, W, c, science);
-    else if (c.WB == 10) e = run_lagcol<10>(p, ss, ns, pl, W, c, science);
-    else e = run_lagcol<20>(p, ss, ns, pl, W, c, science);
-    if (e != cudaSuccess) return e;
-    { KLaunch kl(p, science ? "lagedge_theta" : "lagedge_omega"); lagedge_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(ss, pl, W, nsplit, p->Q, g, p->tw); }
+    // side stream: the packed column kx = 0 / Hx and the wrap corrections (independent of the column pass)
+    if (!p->ktiming && p->side) p->cur = p->side; // the caller forked already (template_side / science_side)
+    { KLaunch kl(p, science ? "lagedge_theta" : "lagedge_omega"); lagedge_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->cur>>>(ss, pl, W, nsplit, p->Q, g, p->tw); }
     int nchunk = 0;
     double *bpart = p->bpart;
     if (g.Mx != g.nx || g.My != g.ny) {
@@ -305,7 +301,15 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
         if (W > 0) { e = launch_border(p, pl, W, science, bpart); if (e != cudaSuccess) return e; }
         else nchunk = 0;
     }
-    { KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega"); lagrow_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->stream>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw); }
+    back_to_main(p);
+    if (c.WB == 3) e = run_lagcol<3>(p, ss, ns, pl, W, c, science);
+    else if (c.WB == 5) e = run_lagcol<5>(p, ss, ns, pl, W, c, science);
+    else if (c.WB == 6) e = run_lagcol<6>(p, ss, ns, pl, W, c, science);
+    else if (c.WB == 10) e = run_lagcol<10>(p, ss, ns, pl, W, c, science);
+    else e = run_lagcol<20>(p, ss, ns, pl, W, c, science);
+    if (e != cudaSuccess) return e;
+    join_side(p);
+    { KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega"); lagrow_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw); }
     return cudaGetLastError();
 }
 

@@ -253,7 +253,7 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
     }
     if (pipe) { cudaError_t e = launch_colpipe_inv(p, p->specTo, coef, p->inter); if (e != cudaSuccess) return e; }
     else { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw); }
-    const int ER = fft_E("SFFT_ROW_E", g.Hx, 16);
+    const int ER = fft_E("SFFT_ROW_E", g.Hx, 8);
     int rthreads; size_t rsmem;
     const int RPB = row_cfg(g, ER, &rthreads, &rsmem);
     {
