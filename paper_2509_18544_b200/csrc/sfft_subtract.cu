@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_inv_kernel(const cpl
 // the padding) where the method wants R((x-u) mod nx, (y-v) mod ny): subtract the difference.
 __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__ R, const double *__restrict__ coef,
                                                      double *__restrict__ D, Geom g) {
-    const int nx = g.nx, ny = g.ny, w = g.w, L = g.L;
+    const int nx = g.nx, ny = g.ny, w = g.w, L = g.L, LL = L * L;
     const long long nA = 2LL * w * nx, nB = 2LL * w * (ny - 2 * w);
     const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (id >= nA + nB) return;
@@ -192,40 +192,36 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
     if (id < nA) { const int r = (int)(id / nx); x = (int)(id - (long long)r * nx); y = r < w ? r : ny - 2 * w + r; }
     else { const long long k = id - nA; const int r = (int)(k / (2 * w)), cidx = (int)(k - (long long)r * 2 * w); y = w + r; x = cidx < w ? cidx : nx - 2 * w + cidx; }
     const double inx = 1.0 / nx, iny = 1.0 / ny;
+    // taps whose source column leaves the frame: u in (x, w] (left edge) or u in [-w, x - nx] (right edge)
+    const int ulo_in = max(-w, x - nx + 1), uhi_in = min(w, x); // u in [ulo_in, uhi_in] stays inside
     double corr = 0.0;
+    // K(u,v; x',y') R(x',y') at a wrapped source pixel
+    auto term = [&](int u, int v, int xs, int ys) {
+        const double xt = (2.0 * xs + 1.0 - nx) * inx, yt = (2.0 * ys + 1.0 - ny) * iny;
+        double xp[MAX_DEG + 1], yp[MAX_DEG + 1];
+        xp[0] = 1.0; yp[0] = 1.0;
+#pragma unroll
+        for (int k = 1; k <= MAX_DEG; k++) { xp[k] = xp[k - 1] * xt; yp[k] = yp[k - 1] * yt; }
+        const double *a = coef + (size_t)(v + w) * L + (u + w);
+        double k = 0.0;
+        int t = 0;
+#pragma unroll
+        for (int d = 0; d <= MAX_DEG; d++)
+#pragma unroll
+            for (int j = 0; j <= d; j++, t++)
+                if (d <= g.DK) k = fma(a[(size_t)t * LL], xp[d - j] * yp[j], k);
+        return k * R[(size_t)ys * nx + xs];
+    };
     for (int v = -w; v <= w; v++) {
         const int ys = y - v;
         const bool oy = ys < 0 || ys >= ny;
+        const int yN = ys < 0 ? ys + ny : (ys >= ny ? ys - ny : ys), yM = (ys + g.My) & (g.My - 1);
         for (int u = -w; u <= w; u++) {
+            if (!oy && u >= ulo_in && u <= uhi_in) { u = uhi_in; continue; } // skip the in-frame run
             const int xs = x - u;
-            const bool ox = xs < 0 || xs >= nx;
-            if (!ox && !oy) continue;
-            const int xN = xs < 0 ? xs + nx : (xs >= nx ? xs - nx : xs), yN = ys < 0 ? ys + ny : (ys >= ny ? ys - ny : ys);
-            const int xM = (xs + g.Mx) & (g.Mx - 1), yM = (ys + g.My) & (g.My - 1);
-            const double *a = coef + (size_t)(v + w) * L + (u + w);
-            // native-grid wrap: + value
-            {
-                const double xt = (2.0 * xN + 1.0 - nx) * inx, yt = (2.0 * yN + 1.0 - ny) * iny;
-                double k = 0.0;
-                for (int t = 0; t < g.NK; t++) {
-                    double wgt = 1.0;
-                    for (int e = 0; e < g.pi[t]; e++) wgt *= xt;
-                    for (int e = 0; e < g.pj[t]; e++) wgt *= yt;
-                    k = fma(a[(size_t)t * L * L], wgt, k);
-                }
-                corr = fma(k, R[(size_t)yN * nx + xN], corr);
-            }
-            if (xM < nx && yM < ny) { // padded-grid wrap landed on a real pixel: - value
-                const double xt = (2.0 * xM + 1.0 - nx) * inx, yt = (2.0 * yM + 1.0 - ny) * iny;
-                double k = 0.0;
-                for (int t = 0; t < g.NK; t++) {
-                    double wgt = 1.0;
-                    for (int e = 0; e < g.pi[t]; e++) wgt *= xt;
-                    for (int e = 0; e < g.pj[t]; e++) wgt *= yt;
-                    k = fma(a[(size_t)t * L * L], wgt, k);
-                }
-                corr = fma(-k, R[(size_t)yM * nx + xM], corr);
-            }
+            const int xN = xs < 0 ? xs + nx : (xs >= nx ? xs - nx : xs), xM = (xs + g.Mx) & (g.Mx - 1);
+            corr += term(u, v, xN, yN);                                  // native-grid wrap: + value
+            if (xM < nx && yM < ny) corr -= term(u, v, xM, yM);          // padded-grid wrap landed on a real pixel
         }
     }
     D[(size_t)y * nx + x] -= corr;
