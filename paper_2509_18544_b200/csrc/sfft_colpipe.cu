@@ -66,8 +66,11 @@ __device__ __forceinline__ void store_pair(cplx *tile_dst, const cplx (&v)[2][CP
 
 // One radix-R pass over both columns; twiddles shared.  X: single-column padded scratch.
 // STORE: exchange through X (column 0, then column 1); else results stay canonical in v.
-template <int R, int DIR, bool STORE>
-__device__ __forceinline__ void pass2(cplx (&v)[2][CP_E], cplx *X, int j, int T, int log2Ns, const cplx *tw, int Nt) {
+// wpre: for radix-8 passes (one butterfly per thread) the pass twiddle exp(-2 pi i k/(8 Ns)), k = j mod Ns, is the
+// same for every tile a thread transforms: it is loaded once per kernel and passed in (HAVEW).
+template <int R, int DIR, bool STORE, bool HAVEW = false>
+__device__ __forceinline__ void pass2(cplx (&v)[2][CP_E], cplx *X, int j, int T, int log2Ns, const cplx *tw, int Nt,
+                                      cplx wpre = cplx()) {
     constexpr int NBF = CP_E / R;
     constexpr int LOG2R = (R == 8) ? 3 : (R == 4) ? 2 : 1;
     const int Ns = 1 << log2Ns;
@@ -82,7 +85,7 @@ __device__ __forceinline__ void pass2(cplx (&v)[2][CP_E], cplx *X, int j, int T,
             const int jb = j + b * T;
             const int k = jb & (Ns - 1);
             if (log2Ns > 0) {
-                cplx w1 = tw[(size_t)k * (Nt >> (log2Ns + LOG2R))];
+                cplx w1 = HAVEW ? wpre : tw[(size_t)k * (Nt >> (log2Ns + LOG2R))];
                 if (DIR > 0) w1.y = -w1.y;
                 twiddle_powers<R>(x, w1);
             }
@@ -104,15 +107,28 @@ __device__ __forceinline__ void pass2(cplx (&v)[2][CP_E], cplx *X, int j, int T,
     }
 }
 
-template <int DIR>
-__device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N, int j, const cplx *tw, int Nt) {
+// twiddles of the radix-8 passes 2..4 of this thread (log2Ns = 3, 6, 9), loaded once per kernel
+struct PassTw { cplx w[3]; };
+__device__ __forceinline__ PassTw load_pass_tw(int log2N, int j, const cplx *tw, int Nt) {
+    PassTw p;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const int log2Ns = 3 * (k + 1);
+        p.w[k] = (log2Ns + 3 <= log2N) ? tw[(size_t)(j & ((1 << log2Ns) - 1)) * (Nt >> (log2Ns + 3))] : mk(1.0, 0.0);
+    }
+    return p;
+}
+
+template <int DIR, bool PW>
+__device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N, int j, const cplx *tw, int Nt, const PassTw &pw) {
     const int T = 1 << (log2N - 3);
     pass2<8, DIR, true>(v, X, j, T, 0, tw, Nt);
-    int log2Ns = 3;
-#pragma unroll 1
-    while (log2Ns + 3 < log2N) { pass2<8, DIR, true>(v, X, j, T, log2Ns, tw, Nt); log2Ns += 3; }
+    int log2Ns = 3, ip = 0;
+#pragma unroll
+    for (int it = 0; it < 2; it++)
+        if (log2Ns + 3 < log2N) { pass2<8, DIR, true, PW>(v, X, j, T, log2Ns, tw, Nt, pw.w[ip]); log2Ns += 3; ip++; }
     switch (log2N - log2Ns) {
-    case 3: pass2<8, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
+    case 3: pass2<8, DIR, false, PW>(v, X, j, T, log2Ns, tw, Nt, pw.w[ip]); break;
     case 2: pass2<4, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
     default: pass2<2, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
     }
@@ -132,6 +148,7 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
     const int nitems = my_tiles * nsrc;
     const size_t src_plane = (size_t)g.ny * Hx, plane = (size_t)My * Hx;
     const double inv_ny = 1.0 / (double)g.ny;
+    const PassTw pw = PassTw(); // the forward kernel is register-bound: it reloads the pass twiddles (L1 hits)
     auto issue_item = [&](int n) {
         if (n < nitems) {
             const int tile = blockIdx.x + (n / nsrc) * gridDim.x, i = n % nsrc;
@@ -159,7 +176,7 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
                 v[1][q] = cscale(e[1], wgt);
             }
             if (k == last) { __syncwarp(); issue_item(n + 1); } // both lanes of a pair have read: the slots are free
-            fft2col<-1>(v, X, g.log2My, j, tw, g.Nt);
+            fft2col<-1, false>(v, X, g.log2My, j, tw, g.Nt, pw);
             store_pair(spec + (size_t)k * plane + 2 * tile, v, Hx, My, j, T);
         }
     }
@@ -170,14 +187,15 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
 // K^ of one (t, column) at the 4 rows jrow + 2 q' T (q' < 4) of a thread (jrow = j + h T):
 //   K^[jrow + 2 q' T] = sum_v (E[v] e^{-2 pi i jrow v/My}) e^{-2 pi i q' v/4}  -- a 4-point DFT of the
 // L phase-shifted taps binned by v mod 4.  taps e[l * estride], l = v + w; phases from tw.
-__device__ __forceinline__ void khat4(cplx (&kh)[4], const cplx *e, int estride, int w, int jrow, int My, const cplx *tw,
-                                      int twsy) {
+// p1 = exp(-2 pi i jrow/My); the phase of tap v is p1^v, built by repeated multiplication (v <= 10).
+__device__ __forceinline__ void khat4(cplx (&kh)[4], const cplx *e, int estride, int w, cplx p1) {
     kh[0] = e[w * estride];
     kh[1] = mk(0.0, 0.0); kh[2] = mk(0.0, 0.0); kh[3] = mk(0.0, 0.0);
+    cplx p = mk(1.0, 0.0);
 #pragma unroll
     for (int v = 1; v <= (MAX_L - 1) / 2; v++) {
         if (v <= w) {
-            const cplx p = tw[(size_t)((jrow * v) & (My - 1)) * twsy];         // exp(-2 pi i jrow v/My)
+            p = cmul(p, p1);                                                   // exp(-2 pi i jrow v/My)
             const cplx a = cmul(e[(w + v) * estride], p), b = cmul(e[(w - v) * estride], cconj(p));
             kh[v & 3] = cadd(kh[v & 3], a);
             kh[(4 - (v & 3)) & 3] = cadd(kh[(4 - (v & 3)) & 3], b);
@@ -201,6 +219,8 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
     const int nchunks = my_tiles * NK * 2;
     const size_t plane = (size_t)My * Hx;
     const int twsy = g.Nt / My;
+    const PassTw pw = load_pass_tw(g.log2My, j, tw, g.Nt);
+    const cplx ph1[2] = {tw[(size_t)j * twsy], tw[(size_t)(j + T) * twsy]}; // exp(-2 pi i (j + h T)/My), h = 0, 1
     auto issue_chunk = [&](int s) { // chunk s = ((tile index * NK) + t) * 2 + h  ->  slot h
         if (s < nchunks) {
             const int tile = blockIdx.x + (s / (2 * NK)) * gridDim.x, t = (s >> 1) % NK, h = s & 1;
@@ -230,8 +250,8 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
             for (int h = 0; h < 2; h++) {
                 const int s = (it * NK + t) * 2 + h;
                 cplx k0[4], k1[4];
-                khat4(k0, et + (size_t)t * L * 3 + 0, 3, w, j + h * T, My, tw, twsy);
-                khat4(k1, et + (size_t)t * L * 3 + 1, 3, w, j + h * T, My, tw, twsy);
+                khat4(k0, et + (size_t)t * L * 3 + 0, 3, w, ph1[h]);
+                khat4(k1, et + (size_t)t * L * 3 + 1, 3, w, ph1[h]);
                 cpa_wait<1>();
                 __syncwarp();
                 const cplx *slot = ring + h * My;
@@ -247,7 +267,7 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
                 __syncwarp();
                 issue_chunk(s + 2);
                 if (tile == 0) {
-                    khat4(k0, et + (size_t)t * L * 3 + 2, 3, w, j + h * T, My, tw, twsy);
+                    khat4(k0, et + (size_t)t * L * 3 + 2, 3, w, ph1[h]);
                     const cplx *zc = spec + (size_t)t * plane;
 #pragma unroll
                     for (int qq = 0; qq < 4; qq++) {
@@ -259,7 +279,7 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
                 }
             }
         }
-        fft2col<1>(acc, X, g.log2My, j, tw, g.Nt);
+        fft2col<1, true>(acc, X, g.log2My, j, tw, g.Nt, pw);
         store_pair(inter + 2 * tile, acc, Hx, g.ny, j, T);
     }
     cpa_wait<0>();

@@ -112,9 +112,9 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
 
     for (int it = 0; it < LC_NST - 1; it++) issue(it);
     for (int it = 0; it < nIt; it++) {
-        issue(it + LC_NST - 1);
-        cp_async_wait<LC_NST - 1>();
-        __syncthreads();
+        cp_async_wait<LC_NST - 2>();   // this thread's copies of stage `it` have landed
+        __syncthreads();               // ... everyone's have, and everyone is done with stage it-1
+        issue(it + LC_NST - 1);        // refill the buffer of stage it-1: one barrier per step
         if (active) {
             const cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
             cplx x[LC_NA];
@@ -126,7 +126,6 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
             dft16<1>(x);
             lag_fold<DLO, DHI>(x, st + LC_NA * row_elems, acc);
         }
-        __syncthreads();
     }
     const int kx = kx0 + lane;
     if (active && kx < Hx && kx > 0) { // kx = 0 is the packed column: lagedge_kernel owns Q[.][.][0]
