@@ -65,9 +65,9 @@ template <typename T> static cudaError_t dalloc(sfft_plan *p, T **ptr, size_t co
 struct StageTimer {
     sfft_plan *p; int stage;
     StageTimer(sfft_plan *p_, int s) : p(p_), stage(s) {
-        if (p->timing) { cudaEventRecord(p->ev0[stage], p->stream); p->ev_used[stage] = true; }
+        if (p->timing) { cudaEventRecord(p->ev0[stage], p->cur); p->ev_used[stage] = true; }
     }
-    ~StageTimer() { if (p->timing) cudaEventRecord(p->ev1[stage], p->stream); }
+    ~StageTimer() { if (p->timing) cudaEventRecord(p->ev1[stage], p->cur); }
 };
 
 static void free_plan(sfft_plan *p) {
@@ -84,6 +84,9 @@ static void free_plan(sfft_plan *p) {
     if (p->side) cudaStreamDestroy(p->side);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
+    if (p->fstream) cudaStreamDestroy(p->fstream);
+    if (p->ev_ffork) cudaEventDestroy(p->ev_ffork);
+    if (p->ev_fjoin) cudaEventDestroy(p->ev_fjoin);
     for (int k = 0; k < MAX_KREC; k++)
         if (p->krec[k].e0) { cudaEventDestroy(p->krec[k].e0); cudaEventDestroy(p->krec[k].e1); }
     delete p;
@@ -169,6 +172,14 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
     cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+    {   // highest priority: the factorisation is a chain of small dependent launches; its CTAs should take
+        // the next free SM slots rather than queue behind the full-grid kernels of the science side
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        cudaStreamCreateWithPriority(&p->fstream, cudaStreamNonBlocking, hi);
+    }
+    cudaEventCreateWithFlags(&p->ev_ffork, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&p->ev_fjoin, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
     // Phi (pin P7): closed form, mask independent
     double phi[MAX_NP * MAX_NP];
@@ -193,6 +204,7 @@ sfft_status sfft_plan_set_stream(sfft_plan *p, void *cuda_stream) {
 
 sfft_status sfft_plan_destroy(sfft_plan *p) {
     if (!p) return SFFT_OK;
+    join_factor(p);
     cudaStreamSynchronize(p->stream);
     free_plan(p);
     return SFFT_OK;
@@ -263,10 +275,22 @@ extern "C" {
 sfft_status sfft_build_system(sfft_plan *p, const double *S, const double *R, const uint8_t *mask) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (!S || !R) return fail(p, SFFT_ERR_INVALID_ARG, "build_system: NULL image");
+    join_factor(p); // a factorisation still in flight reads G
     p->S = S; p->R = R; p->mask = mask;
     p->have_template = p->have_system = p->have_factor = p->have_solution = false;
     sfft_status st = template_side(p);
     if (st != SFFT_OK) return st;
+    if (!p->ktiming && p->fstream && !getenv("SFFT_NO_FACTOR_OVERLAP")) {
+        // G depends on the template only: factor it (a4) on its own stream while the science side (a1, Theta)
+        // runs on the caller's stream; sfft_solve joins.
+        fork_factor(p);
+        {
+            StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
+            CK(launch_factor(p), "factor");
+        }
+        back_to_main(p);
+        p->have_factor = true;
+    }
     st = science_side(p);
     if (st != SFFT_OK) return st;
     p->have_template = true; p->have_system = true;
@@ -276,6 +300,7 @@ sfft_status sfft_build_system(sfft_plan *p, const double *S, const double *R, co
 sfft_status sfft_solve(sfft_plan *p) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (!p->have_system) return fail(p, SFFT_ERR_STATE, "solve before build_system");
+    join_factor(p);
     if (!p->have_factor) {
         StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
         CK(launch_factor(p), "factor");
@@ -315,6 +340,7 @@ sfft_status sfft_subtract_with(sfft_plan *p, const double *S, const double *coef
 sfft_status sfft_set_template(sfft_plan *p, const double *R, const uint8_t *mask) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (!R) return fail(p, SFFT_ERR_INVALID_ARG, "set_template: NULL image");
+    join_factor(p);
     p->R = R; p->mask = mask; p->S = nullptr;
     p->have_template = p->have_system = p->have_factor = p->have_solution = false;
     sfft_status st = template_side(p);
@@ -354,6 +380,7 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
 
 sfft_status sfft_sync_status(sfft_plan *p) {
     if (!p) return SFFT_ERR_INVALID_ARG;
+    join_factor(p);
     CK(cudaStreamSynchronize(p->stream), "sync");
     if (p->side) CK(cudaStreamSynchronize(p->side), "sync side");
     if (p->have_factor) {

@@ -303,11 +303,16 @@ __global__ void __launch_bounds__(128) ktab_plain_kernel(const double *__restric
 
 bool colpipe_ok(const Geom &g) { return g.My >= 512 && g.My <= 4096 && g.Hx >= 2 && getenv("SFFT_NO_COLPIPE") == nullptr; }
 
-static int colpipe_grid(const Geom &g) {
+static int colpipe_reserve() { const char *e = getenv("SFFT_FACTOR_SMS"); return e ? atoi(e) : 12; }
+static int colpipe_grid(const Geom &g, int reserve) {
     static int sms = 0;
     if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
     const int ntiles = g.Hx / 2;
-    return ntiles < sms ? ntiles : sms;
+    int grid = ntiles < sms ? ntiles : sms;
+    // while a factorisation runs beside us, leave a few SMs to it: a persistent full-register CTA would
+    // otherwise block its chain of small launches for the whole kernel
+    if (reserve > 0 && grid > 4 * reserve) grid -= reserve;
+    return grid;
 }
 
 cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj, int nsrc) {
@@ -322,7 +327,7 @@ cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int 
     ColJobs jobs; jobs.ns = ns;
     for (int k = 0; k < ns; k++) { jobs.ii[k] = ii[k]; jobs.jj[k] = jj[k]; }
     KLaunch kl(p, ns > 1 ? "col_fwd_R" : "col_fwd_S");
-    colpipe_fwd_kernel<<<colpipe_grid(g), g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
+    colpipe_fwd_kernel<<<colpipe_grid(g, p->factor_pending ? colpipe_reserve() : 0), g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
     return cudaGetLastError();
 }
 
@@ -337,7 +342,7 @@ cudaError_t launch_colpipe_inv(sfft_plan *p, const cplx *spec, const double *coe
         attr_set = true;
     }
     KLaunch kl(p, "col_inv");
-    colpipe_inv_kernel<<<colpipe_grid(g), g.My / CP_E, smem, p->stream>>>(spec, p->E, inter, g, p->tw);
+    colpipe_inv_kernel<<<colpipe_grid(g, 0), g.My / CP_E, smem, p->stream>>>(spec, p->E, inter, g, p->tw);
     return cudaGetLastError();
 }
 

@@ -43,6 +43,9 @@ struct sfft_plan {
     cudaStream_t side;       // plan-owned: small independent kernels run beside the big ones (fork/join by events)
     cudaStream_t cur;        // stream the launchers enqueue on right now (stream, or side inside a fork)
     cudaEvent_t ev_fork, ev_join;
+    cudaStream_t fstream;    // plan-owned: the factorisation of a single pair runs here, beside the science-side a1/a2
+    cudaEvent_t ev_ffork, ev_fjoin;
+    bool factor_pending;     // factor kernels are enqueued on fstream and not yet joined into `stream`
     // device workspaces
     sfft::cplx *tw;          // [Nt]
     sfft::cplx *inter;       // [(DK+1)][ny][Hx] row-transformed intermediates (a1) / a5 intermediate
@@ -155,6 +158,18 @@ inline void join_side(sfft_plan *p) {
     p->cur = p->stream;
     if (p->ktiming || !p->side) return;
     cudaEventRecord(p->ev_join, p->side); cudaStreamWaitEvent(p->stream, p->ev_join, 0);
+}
+
+// the factorisation stream: same fork/join protocol as the side stream
+inline void fork_factor(sfft_plan *p) {
+    cudaEventRecord(p->ev_ffork, p->stream); cudaStreamWaitEvent(p->fstream, p->ev_ffork, 0);
+    p->cur = p->fstream; p->factor_pending = true;
+}
+inline void join_factor(sfft_plan *p) {
+    p->cur = p->stream;
+    if (!p->factor_pending) return;
+    cudaEventRecord(p->ev_fjoin, p->fstream); cudaStreamWaitEvent(p->stream, p->ev_fjoin, 0);
+    p->factor_pending = false;
 }
 
 inline int ilog2(int v) { int l = 0; while ((1 << l) < v) l++; return l; }

@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict_
 
 cudaError_t launch_factor(sfft_plan *p) {
     const int n = p->g.n;
-    cudaStream_t st = p->stream;
+    cudaStream_t st = p->cur;
     cudaMemsetAsync(p->flag, 0, sizeof(int), st);
     { KLaunch kl(p, "equil_diag"); equil_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(p->G, p->dscale, n, p->flag); }
     const long long total = (long long)n * n;
