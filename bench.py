@@ -207,6 +207,33 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------
+# multi-GPU host logic: replicas only -- no data-path collective
+# ------------------------------------------------------------------------------------------
+def max_over_ranks(values, device):
+    """Element-wise MAX over all ranks of a list of floats (device times); identity when not distributed."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def replica_throughput(world, ms_per_step):
+    """Whole-job images/s of `world` independent replicas that each finish one image per step."""
+    return world * 1e3 / ms_per_step
+
+
+def ncu_traffic(kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.json)."""
+    f = ROOT / "profiles" / "ncu_traffic.json"
+    try:
+        return json.loads(f.read_text())["kernels"][kernel]["dram_bytes_per_launch"]
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -279,13 +306,10 @@ def run_ours(args):
     ms_e2e = f0.elapsed_time(f1)
     clk = clocks.stop()
 
-    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], "cuda")
     ms_step = ms_total / args.steps
-    value = world * 1e3 / ms_step
-    e2e_value = world * 1e3 / (ms_e2e / args.steps)
+    value = replica_throughput(world, ms_step)
+    e2e_value = replica_throughput(world, ms_e2e / args.steps)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -350,7 +374,7 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
     per_launch_ms = kernels[dom] / kcnt[dom]
     ach = kbytes[dom] / (per_launch_ms * 1e-3) / 1e9
     out["roofline"] = {"kernel": dom, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
-                       "frac": round(ach / peak, 4), "traffic": None, "peak_source": peak_src,
+                       "frac": round(ach / peak, 4), "traffic": ncu_traffic(dom), "peak_source": peak_src,
                        "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": round(per_launch_ms, 4),
                        "share_of_step": round(kernels[dom] / sum(kernels.values()), 3)}
     t_path = sum(stages[k] for k in ("a1_template", "a1_science", "a2_omega", "a2_theta", "a3_gather", "a5_subtract"))
