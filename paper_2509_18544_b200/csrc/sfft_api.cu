@@ -169,6 +169,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     *p->flag_host = 0;
     for (int s = 0; s < SFFT_NUM_STAGES; s++) { cudaEventCreate(&p->ev0[s]); cudaEventCreate(&p->ev1[s]); }
     p->stream = 0; p->cur = 0;
+    p->no_side = getenv("SFFT_NO_SIDE") != nullptr;
     cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
     cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);

@@ -70,9 +70,10 @@ __global__ void __launch_bounds__(128) gamma_cols_kernel(const double *__restric
     const int i = g.pi[t], j = g.pj[t], pp = g.pi[s], qq = g.pj[s];
     const double *A = gamA + (((size_t)i * (g.DB + 1) + pp) * L + ui) * ny;
     double acc = 0.0;
+    const double inv_ny = 1.0 / (double)ny;
     for (int y = threadIdx.x; y < ny; y += blockDim.x) {
         int y2 = y + v; if (y2 >= ny) y2 -= ny; if (y2 < 0) y2 += ny;
-        const double yt = (2.0 * y + 1.0 - ny) / ny, yt2 = (2.0 * y2 + 1.0 - ny) / ny;
+        const double yt = (2.0 * y + 1.0 - ny) * inv_ny, yt2 = (2.0 * y2 + 1.0 - ny) * inv_ny;
         acc += ipw(yt, j) * ipw(yt2, qq) * A[y];
     }
     acc = block_sum2(acc, sh);
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(128) delta_kernel(const double *__restrict__ m
     const int s = blockIdx.x, pp = g.pi[s], qq = g.pj[s], ny = g.ny;
     double acc = 0.0;
     for (int y = threadIdx.x; y < ny; y += blockDim.x)
-        acc += ipw((2.0 * y + 1.0 - ny) / ny, qq) * muS[(size_t)pp * ny + y];
+        acc += ipw((2.0 * y + 1.0 - ny) * (1.0 / (double)ny), qq) * muS[(size_t)pp * ny + y];
     acc = block_sum2(acc, sh);
     if (threadIdx.x == 0) delta[s] = acc;
 }

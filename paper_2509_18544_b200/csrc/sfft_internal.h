@@ -45,6 +45,7 @@ struct sfft_plan {
     cudaEvent_t ev_fork, ev_join;
     cudaStream_t fstream;    // plan-owned: the factorisation of a single pair runs here, beside the science-side a1/a2
     cudaEvent_t ev_ffork, ev_fjoin;
+    bool no_side;            // SFFT_NO_SIDE: keep the small kernels on the caller's stream (experiments)
     bool factor_pending;     // factor kernels are enqueued on fstream and not yet joined into `stream`
     // device workspaces
     sfft::cplx *tw;          // [Nt]
@@ -149,14 +150,14 @@ struct KLaunch {
 // side stream: fork = side waits for everything enqueued on the main stream so far; join = main waits for side.
 // In per-launch timing mode everything stays on the main stream so that kernel times do not overlap.
 inline void fork_side(sfft_plan *p) {
-    if (p->ktiming || !p->side) return;
+    if (p->ktiming || !p->side || p->no_side) return;
     cudaEventRecord(p->ev_fork, p->stream); cudaStreamWaitEvent(p->side, p->ev_fork, 0);
     p->cur = p->side;
 }
 inline void back_to_main(sfft_plan *p) { p->cur = p->stream; }
 inline void join_side(sfft_plan *p) {
     p->cur = p->stream;
-    if (p->ktiming || !p->side) return;
+    if (p->ktiming || !p->side || p->no_side) return;
     cudaEventRecord(p->ev_join, p->side); cudaStreamWaitEvent(p->stream, p->ev_join, 0);
 }
 

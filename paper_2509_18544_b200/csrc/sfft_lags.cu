@@ -201,7 +201,6 @@ __global__ void __launch_bounds__(256) lagedge_kernel(SpecSet ss, PairList pl, i
 __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q, int np, int W, int nsplit,
                                                     const double *__restrict__ bpart, int nchunk,
                                                     double *__restrict__ lag, Geom g, const cplx *__restrict__ tw) {
-    __shared__ double sh[32];
     const int p = blockIdx.x, dvi = blockIdx.y, Hx = g.Hx, Mx = g.Mx;
     constexpr int WM = MAX_L - 1; // 20
     double sc[WM + 1], sn[WM + 1];
@@ -219,23 +218,32 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
                 sc[d] = fma(q.x, e.x, sc[d]); sn[d] = fma(q.y, -e.y, sn[d]);
             }
     }
+    // one reduction for all 2(W+1) sums: shuffles inside a warp, then one pass through shared memory
+    __shared__ double red[8][2 * (WM + 1)];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 0; d <= WM; d++)
+        if (d <= W) {
+            double c = sc[d], sv = sn[d];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) { c += __shfl_down_sync(0xffffffffu, c, off); sv += __shfl_down_sync(0xffffffffu, sv, off); }
+            if (lane == 0) { red[wid][2 * d] = c; red[wid][2 * d + 1] = sv; }
+        }
+    __syncthreads();
     const double scale = 1.0 / ((double)g.Mx * (double)g.My);
     const int nl = (2 * W + 1) * (2 * W + 1);
-    for (int d = 0; d <= W; d++) {
-        double c = 0.0, s = 0.0;
-#pragma unroll
-        for (int k = 0; k <= WM; k++) if (k == d) { c = sc[k]; s = sn[k]; }
-        c = block_sum(c, sh); s = block_sum(s, sh);
-        if (threadIdx.x == 0) {
-            double vp = (c - s) * scale, vm = (c + s) * scale; // Re(q e^{+i th}), Re(q e^{-i th})
-            const int ip = dvi * (2 * W + 1) + (W + d), im = dvi * (2 * W + 1) + (W - d);
-            for (int k = 0; k < nchunk; k++) {
-                vp += bpart[((size_t)k * np + p) * nl + ip];
-                if (d > 0) vm += bpart[((size_t)k * np + p) * nl + im];
-            }
-            lag[(size_t)p * nl + ip] = vp;
-            if (d > 0) lag[(size_t)p * nl + im] = vm;
+    if ((int)threadIdx.x <= W) {
+        const int d = threadIdx.x;
+        double c = 0.0, sv = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); k++) { c += red[k][2 * d]; sv += red[k][2 * d + 1]; }
+        double vp = (c - sv) * scale, vm = (c + sv) * scale; // Re(q e^{+i th}), Re(q e^{-i th})
+        const int ip = dvi * (2 * W + 1) + (W + d), im = dvi * (2 * W + 1) + (W - d);
+        for (int k = 0; k < nchunk; k++) {
+            vp += bpart[((size_t)k * np + p) * nl + ip];
+            if (d > 0) vm += bpart[((size_t)k * np + p) * nl + im];
         }
+        lag[(size_t)p * nl + ip] = vp;
+        if (d > 0) lag[(size_t)p * nl + im] = vm;
     }
 }
 
@@ -291,7 +299,7 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     const int nsplit = c.nsplit;
     cudaError_t e;
     // side stream: the packed column kx = 0 / Hx and the wrap corrections (independent of the column pass)
-    if (!p->ktiming && p->side) p->cur = p->side; // the caller forked already (template_side / science_side)
+    if (!p->ktiming && p->side && !p->no_side) p->cur = p->side; // the caller forked already (template_side / science_side)
     { KLaunch kl(p, science ? "lagedge_theta" : "lagedge_omega"); lagedge_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->cur>>>(ss, pl, W, nsplit, p->Q, g, p->tw); }
     int nchunk = 0;
     double *bpart = p->bpart;
