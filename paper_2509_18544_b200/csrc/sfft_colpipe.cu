@@ -119,10 +119,23 @@ __device__ __forceinline__ PassTw load_pass_tw(int log2N, int j, const cplx *tw,
     return p;
 }
 
-template <int DIR, bool PW>
-__device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N, int j, const cplx *tw, int Nt, const PassTw &pw) {
+// LOG2N_CT != 0: length fixed at compile time (My = 4096), all index arithmetic folds to constants.
+template <int DIR, bool PW, int LOG2N_CT>
+__device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N_rt, int j, const cplx *tw, int Nt, const PassTw &pw) {
+    const int log2N = LOG2N_CT ? LOG2N_CT : log2N_rt;
     const int T = 1 << (log2N - 3);
     pass2<8, DIR, true>(v, X, j, T, 0, tw, Nt);
+    if (LOG2N_CT) {
+        if (6 < log2N) pass2<8, DIR, true, PW>(v, X, j, T, 3, tw, Nt, pw.w[0]);
+        if (9 < log2N) pass2<8, DIR, true, PW>(v, X, j, T, 6, tw, Nt, pw.w[1]);
+        const int log2Ns = (9 < log2N) ? 9 : (6 < log2N) ? 6 : 3, ip = log2Ns / 3 - 1;
+        switch (log2N - log2Ns) {
+        case 3: pass2<8, DIR, false, PW>(v, X, j, T, log2Ns, tw, Nt, pw.w[ip]); break;
+        case 2: pass2<4, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
+        default: pass2<2, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
+        }
+        return;
+    }
     int log2Ns = 3, ip = 0;
 #pragma unroll
     for (int it = 0; it < 2; it++)
@@ -136,11 +149,12 @@ __device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N, 
 
 // ------------------------------------------------------------------------------------------ forward
 // grid = min(#SM, Hx/2) persistent CTAs; block = My/8; dynamic smem = (padded_lenE<8>(My) + 2 My) cplx.
+template <int LOG2N_CT>
 __global__ void __launch_bounds__(CP_MAXT, 1)
 colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJobs jobs, int nsrc, Geom g,
                    const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int My = g.My, Hx = g.Hx, T = My / CP_E, j = threadIdx.x;
+    const int My = LOG2N_CT ? (1 << LOG2N_CT) : g.My, Hx = g.Hx, T = My / CP_E, j = threadIdx.x;
     cplx *X = reinterpret_cast<cplx *>(smem_raw);
     cplx *ring = X + padded_lenE<CP_E>(My);
     const int ntiles = Hx / 2;
@@ -176,7 +190,7 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
                 v[1][q] = cscale(e[1], wgt);
             }
             if (k == last) { __syncwarp(); issue_item(n + 1); } // both lanes of a pair have read: the slots are free
-            fft2col<-1, false>(v, X, g.log2My, j, tw, g.Nt, pw);
+            fft2col<-1, false, LOG2N_CT>(v, X, g.log2My, j, tw, g.Nt, pw);
             store_pair(spec + (size_t)k * plane + 2 * tile, v, Hx, My, j, T);
         }
     }
@@ -206,11 +220,12 @@ __device__ __forceinline__ void khat4(cplx (&kh)[4], const cplx *e, int estride,
 
 // grid = min(#SM, Hx/2); block = My/8; dynamic smem = (padded_lenE<8>(My) + 2 My + 3 NK L) cplx.
 // Ep: plain taps [NK][L][Hx+1].
+template <int LOG2N_CT>
 __global__ void __launch_bounds__(CP_MAXT, 1)
 colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, cplx *__restrict__ inter, Geom g,
                    const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int My = g.My, Hx = g.Hx, T = My / CP_E, j = threadIdx.x, L = g.L, w = g.w, NK = g.NK;
+    const int My = LOG2N_CT ? (1 << LOG2N_CT) : g.My, Hx = g.Hx, T = My / CP_E, j = threadIdx.x, L = g.L, w = g.w, NK = g.NK;
     cplx *X = reinterpret_cast<cplx *>(smem_raw);
     cplx *ring = X + padded_lenE<CP_E>(My);
     cplx *et = ring + 2 * My; // [t*L + l][3]: columns 0, 1 of the tile; slot 2: second tap set of the packed column
@@ -279,7 +294,7 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
                 }
             }
         }
-        fft2col<1, true>(acc, X, g.log2My, j, tw, g.Nt, pw);
+        fft2col<1, true, LOG2N_CT>(acc, X, g.log2My, j, tw, g.Nt, pw);
         store_pair(inter + 2 * tile, acc, Hx, g.ny, j, T);
     }
     cpa_wait<0>();
@@ -320,14 +335,17 @@ cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int 
     const size_t smem = (size_t)(padded_lenE<CP_E>(g.My) + 2 * g.My) * sizeof(cplx);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(colpipe_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(colpipe_fwd_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(colpipe_fwd_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     ColJobs jobs; jobs.ns = ns;
     for (int k = 0; k < ns; k++) { jobs.ii[k] = ii[k]; jobs.jj[k] = jj[k]; }
     KLaunch kl(p, ns > 1 ? "col_fwd_R" : "col_fwd_S");
-    colpipe_fwd_kernel<<<colpipe_grid(g, p->factor_pending ? colpipe_reserve() : 0), g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
+    const int grid = colpipe_grid(g, p->factor_pending ? colpipe_reserve() : 0);
+    if (g.log2My == 12) colpipe_fwd_kernel<12><<<grid, g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
+    else colpipe_fwd_kernel<0><<<grid, g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
     return cudaGetLastError();
 }
 
@@ -337,12 +355,14 @@ cudaError_t launch_colpipe_inv(sfft_plan *p, const cplx *spec, const double *coe
     const size_t smem = (size_t)(padded_lenE<CP_E>(g.My) + 2 * g.My + 3 * g.NK * g.L) * sizeof(cplx);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(colpipe_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(colpipe_inv_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(colpipe_inv_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     KLaunch kl(p, "col_inv");
-    colpipe_inv_kernel<<<colpipe_grid(g, 0), g.My / CP_E, smem, p->stream>>>(spec, p->E, inter, g, p->tw);
+    if (g.log2My == 12) colpipe_inv_kernel<12><<<colpipe_grid(g, 0), g.My / CP_E, smem, p->stream>>>(spec, p->E, inter, g, p->tw);
+    else colpipe_inv_kernel<0><<<colpipe_grid(g, 0), g.My / CP_E, smem, p->stream>>>(spec, p->E, inter, g, p->tw);
     return cudaGetLastError();
 }
 

@@ -176,16 +176,42 @@ template <int E> SFFT_HD void fft_load_canonicalE(cplx *v, const cplx *s, int j,
 #ifdef __CUDACC__
 // Whole FFT of length N = 2^log2N >= 2E for the T = N/E threads of one transform inside a CTA in which
 // EVERY thread calls this with the same N (barriers are CTA-wide).  v canonical in, canonical out.
-template <int DIR, int E>
-__device__ __forceinline__ void fft_blockE(cplx *v, cplx *s, int log2N, int j, const cplx *tw, int Nt) {
+// LOG2N_CT != 0 fixes the length at compile time (the hot sizes): every shift, mask, padded index and
+// twiddle stride below then folds to a constant and the passes unroll, which removes most of the
+// integer instructions that otherwise outnumber the FP64 ones.
+template <int DIR, int E, int LOG2N_CT = 0>
+__device__ __forceinline__ void fft_blockE(cplx *v, cplx *s, int log2N_rt, int j, const cplx *tw, int Nt) {
     constexpr int LOG2E = (E == 16) ? 4 : 3;
+    const int log2N = LOG2N_CT ? LOG2N_CT : log2N_rt;
     const int T = 1 << (log2N - LOG2E);
-    int log2Ns = 0;
     __syncthreads();
     fft_passE<E, E, DIR, true>(v, s, j, T, 0, tw, Nt);
     __syncthreads();
     fft_load_canonicalE<E>(v, s, j, T);
-    log2Ns = LOG2E;
+    if (LOG2N_CT) {
+        // up to two more full-radix passes (N <= E^4), all bounds known
+        if (LOG2E + LOG2E < log2N) {
+            __syncthreads();
+            fft_passE<E, E, DIR, true>(v, s, j, T, LOG2E, tw, Nt);
+            __syncthreads();
+            fft_load_canonicalE<E>(v, s, j, T);
+        }
+        if (3 * LOG2E < log2N) {
+            __syncthreads();
+            fft_passE<E, E, DIR, true>(v, s, j, T, 2 * LOG2E, tw, Nt);
+            __syncthreads();
+            fft_load_canonicalE<E>(v, s, j, T);
+        }
+        const int log2Ns = (3 * LOG2E < log2N) ? 3 * LOG2E : (2 * LOG2E < log2N) ? 2 * LOG2E : LOG2E;
+        switch (log2N - log2Ns) {
+        case 4: if (E >= 16) fft_passE<E, (E >= 16 ? 16 : E), DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+        case 3: fft_passE<E, 8, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+        case 2: fft_passE<E, 4, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+        default: fft_passE<E, 2, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
+        }
+        return;
+    }
+    int log2Ns = LOG2E;
 #pragma unroll 1
     while (log2Ns + LOG2E < log2N) {
         __syncthreads();

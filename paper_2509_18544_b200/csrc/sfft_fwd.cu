@@ -21,14 +21,14 @@ __device__ __forceinline__ double ipow_small(double b, int e) {
 // ------------------------------------------------------------------ row pass
 // grid.x = ceil(ny / RPB); block = RPB * T threads, T = Hx/E (E values per thread).
 // dynamic smem: RPB * padded_lenE<E>(Hx) cplx  +  RPB * 8 * 8 doubles (moment partials)
-template <int E>
+template <int E, int LOG2N_CT = 0>
 __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
                                                      cplx *__restrict__ inter, int NI, double *__restrict__ mu, int NMOM,
                                                      Geom g, const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Hx = g.Hx, T = Hx / E;
-    const int RPB = blockDim.x / T;
-    const int rib = threadIdx.x / T, j = threadIdx.x - rib * T;
+    const int Hx = LOG2N_CT ? (1 << LOG2N_CT) : g.Hx, T = Hx / E;
+    const int RPB = LOG2N_CT ? 1 : blockDim.x / T; // the fixed-size instances run one row per CTA
+    const int rib = LOG2N_CT ? 0 : threadIdx.x / T, j = threadIdx.x - rib * T;
     const int row = blockIdx.x * RPB + rib;
     const bool live = row < g.ny;
     cplx *s = reinterpret_cast<cplx *>(smem_raw) + (size_t)rib * padded_lenE<E>(Hx);
@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_fwd_kernel(const dou
                     mu[(size_t)m * g.ny + row] = acc;
                 }
         }
-        fft_blockE<-1, E>(v, s, g.log2Hx, j, tw, g.Nt);
+        fft_blockE<-1, E, LOG2N_CT>(v, s, g.log2Hx, j, tw, g.Nt);
         __syncthreads();
 #pragma unroll
         for (int q = 0; q < E; q++) s[padE<E>(j + q * T)] = v[q];
@@ -166,12 +166,14 @@ cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask,
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<8, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     {
         KLaunch kl(p, NI > 1 ? "row_fwd_R" : "row_fwd_S");
-        if (E == 8) row_fwd_kernel<8><<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+        if (E == 8 && g.log2Hx == 11 && RPB == 1) row_fwd_kernel<8, 11><<<g.ny, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+        else if (E == 8) row_fwd_kernel<8><<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
         else row_fwd_kernel<16><<<(g.ny + RPB - 1) / RPB, threads, smem, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
     }
     return cudaGetLastError();

@@ -109,14 +109,14 @@ __global__ void __launch_bounds__(512) col_inv_kernel(const cplx *__restrict__ s
 }
 
 // grid.x = ceil(ny/RPB); block = RPB*T, T = Hx/E.  dynamic smem: RPB*padded_lenE<E>(Hx) cplx
-template <int E>
+template <int E, int LOG2N_CT = 0>
 __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
                                                      const double *__restrict__ coef, double *__restrict__ D, Geom g,
                                                      const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Hx = g.Hx, T = Hx / E;
-    const int RPB = blockDim.x / T;
-    const int rib = threadIdx.x / T, j = threadIdx.x - rib * T;
+    const int Hx = LOG2N_CT ? (1 << LOG2N_CT) : g.Hx, T = Hx / E;
+    const int RPB = LOG2N_CT ? 1 : blockDim.x / T;
+    const int rib = LOG2N_CT ? 0 : threadIdx.x / T, j = threadIdx.x - rib * T;
     const int row = blockIdx.x * RPB + rib;
     const bool live = row < g.ny;
     cplx *s = reinterpret_cast<cplx *>(smem_raw) + (size_t)rib * padded_lenE<E>(Hx);
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_inv_kernel(const cpl
             v[q] = mk(Ev.x - Od.y, Ev.y + Od.x); // E + i O
         }
     }
-    fft_blockE<1, E>(v, s, g.log2Hx, j, tw, g.Nt);
+    fft_blockE<1, E, LOG2N_CT>(v, s, g.log2Hx, j, tw, g.Nt);
     if (!live) return;
     // background polynomial of this row: B(x) = sum_p cx[p] xt^p, cx[p] = sum_q b_(p,q) yt^q
     double cx[MAX_DEG + 1];
@@ -244,6 +244,7 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
         cudaError_t e = cudaFuncSetAttribute(col_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<8, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -254,7 +255,8 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
     const int RPB = row_cfg(g, ER, &rthreads, &rsmem);
     {
         KLaunch kl(p, "row_inv");
-        if (ER == 8) row_inv_kernel<8><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
+        if (ER == 8 && g.log2Hx == 11 && RPB == 1) row_inv_kernel<8, 11><<<g.ny, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
+        else if (ER == 8) row_inv_kernel<8><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
         else row_inv_kernel<16><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
     }
     if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
