@@ -120,12 +120,26 @@ __device__ __forceinline__ PassTw load_pass_tw(int log2N, int j, const cplx *tw,
 }
 
 // LOG2N_CT != 0: length fixed at compile time (My = 4096), all index arithmetic folds to constants.
+// wsm (optional): the thread's pass twiddles parked in shared memory, wsm[pass * T + j] (the forward kernel has
+// no registers to spare and almost no L1 left beside its 200 KB of shared memory).
 template <int DIR, bool PW, int LOG2N_CT>
-__device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N_rt, int j, const cplx *tw, int Nt, const PassTw &pw) {
+__device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N_rt, int j, const cplx *tw, int Nt, const PassTw &pw,
+                                        const cplx *wsm = nullptr) {
     const int log2N = LOG2N_CT ? LOG2N_CT : log2N_rt;
     const int T = 1 << (log2N - 3);
     pass2<8, DIR, true>(v, X, j, T, 0, tw, Nt);
     if (LOG2N_CT) {
+        if (wsm) {
+            if (6 < log2N) pass2<8, DIR, true, true>(v, X, j, T, 3, tw, Nt, wsm[j]);
+            if (9 < log2N) pass2<8, DIR, true, true>(v, X, j, T, 6, tw, Nt, wsm[T + j]);
+            const int log2Ns = (9 < log2N) ? 9 : (6 < log2N) ? 6 : 3, ip = log2Ns / 3 - 1;
+            switch (log2N - log2Ns) {
+            case 3: pass2<8, DIR, false, true>(v, X, j, T, log2Ns, tw, Nt, wsm[ip * T + j]); break;
+            case 2: pass2<4, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
+            default: pass2<2, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
+            }
+            return;
+        }
         if (6 < log2N) pass2<8, DIR, true, PW>(v, X, j, T, 3, tw, Nt, pw.w[0]);
         if (9 < log2N) pass2<8, DIR, true, PW>(v, X, j, T, 6, tw, Nt, pw.w[1]);
         const int log2Ns = (9 < log2N) ? 9 : (6 < log2N) ? 6 : 3, ip = log2Ns / 3 - 1;
@@ -162,7 +176,14 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
     const int nitems = my_tiles * nsrc;
     const size_t src_plane = (size_t)g.ny * Hx, plane = (size_t)My * Hx;
     const double inv_ny = 1.0 / (double)g.ny;
-    const PassTw pw = PassTw(); // the forward kernel is register-bound: it reloads the pass twiddles (L1 hits)
+    const PassTw pw = PassTw();
+    const cplx *wsm = nullptr;
+    if (LOG2N_CT) { // park this thread's pass twiddles in shared memory (3 x T entries behind the ring)
+        cplx *wt = ring + 2 * My;
+        const PassTw ld = load_pass_tw(LOG2N_CT, j, tw, g.Nt);
+        wt[j] = ld.w[0]; wt[T + j] = ld.w[1]; wt[2 * T + j] = ld.w[2];
+        wsm = wt; // each thread reads back only its own entries: no barrier needed
+    }
     auto issue_item = [&](int n) {
         if (n < nitems) {
             const int tile = blockIdx.x + (n / nsrc) * gridDim.x, i = n % nsrc;
@@ -190,7 +211,7 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
                 v[1][q] = cscale(e[1], wgt);
             }
             if (k == last) { __syncwarp(); issue_item(n + 1); } // both lanes of a pair have read: the slots are free
-            fft2col<-1, false, LOG2N_CT>(v, X, g.log2My, j, tw, g.Nt, pw);
+            fft2col<-1, false, LOG2N_CT>(v, X, g.log2My, j, tw, g.Nt, pw, wsm);
             store_pair(spec + (size_t)k * plane + 2 * tile, v, Hx, My, j, T);
         }
     }
@@ -332,11 +353,11 @@ static int colpipe_grid(const Geom &g, int reserve) {
 
 cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj, int nsrc) {
     const Geom &g = p->g;
-    const size_t smem = (size_t)(padded_lenE<CP_E>(g.My) + 2 * g.My) * sizeof(cplx);
+    const size_t smem = (size_t)(padded_lenE<CP_E>(g.My) + 2 * g.My + (g.log2My == 12 ? 3 * g.My / CP_E : 0)) * sizeof(cplx);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(colpipe_fwd_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(colpipe_fwd_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(colpipe_fwd_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }

@@ -33,7 +33,8 @@ __global__ void equil_scale_kernel(const double *__restrict__ G, const double *_
 // X L_kk^T = A, by a register-resident right-looking substitution (4 lanes per row, shuffles only).
 // No FP64 division or sqrt on the dependent chain: inv = rsqrt(pivot), L_jj = pivot * inv.
 // grid = max(1, row tiles below); block 256; static smem.
-__global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ Lf, int n, int k0, int bs, int *flag) {
+__global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
+                                                         int bs, int *flag) {
     __shared__ double l[CB][CB + 1];
     __shared__ double col[2][CB];
     __shared__ double rd[CB];
@@ -79,7 +80,9 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
         {
             const int c = 4 * j4 + cq;
             l[r][c] = c <= r ? areg[0] : 0.0;
-            if (blockIdx.x == 0 && r < bs && c <= r) Lf[(size_t)(k0 + r) * n + k0 + c] = areg[0];
+            // the factored block goes to Ldiag, NOT back into Lf: the other CTAs of this launch read the
+            // unfactored block from Lf whenever they get scheduled
+            if (blockIdx.x == 0) Ldiag[r * CB + c] = c <= r ? areg[0] : 0.0;
         }
 #pragma unroll
         for (int qq = 0; qq < 15; qq++) areg[qq] = areg[qq + 1];
@@ -115,15 +118,14 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
 
 // Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves:
 // Linv[b][i][c], thread c solves column c of  L X = I  by forward substitution.  grid = nblk; block 64.
-__global__ void __launch_bounds__(CB) trinv_kernel(const double *__restrict__ Lf, double *__restrict__ Linv, int n) {
+__global__ void __launch_bounds__(CB) trinv_kernel(double *__restrict__ Linv, int n) {
     extern __shared__ __align__(16) double dsm[];
     double (*l)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm);
     double (*x)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm + CB * (CB + 1));
-    const int k0 = blockIdx.x * CB, bs = min(CB, n - k0), c = threadIdx.x;
-    for (int e = threadIdx.x; e < CB * CB; e += CB) {
-        const int r = e >> 6, cc = e & 63;
-        l[r][cc] = (r < bs && cc <= r) ? Lf[(size_t)(k0 + r) * n + k0 + cc] : (r == cc ? 1.0 : 0.0);
-    }
+    const int c = threadIdx.x;
+    // Linv[b] holds the factored diagonal block L_bb (identity-padded, written by potrf_panel_kernel): invert in place
+    const double *src = Linv + (size_t)blockIdx.x * CB * CB;
+    for (int e = threadIdx.x; e < CB * CB; e += CB) l[e >> 6][e & 63] = src[e];
     __syncthreads();
     for (int i = 0; i < CB; i++) {
         double s0 = (i == c) ? 1.0 : 0.0, s1 = 0.0;
@@ -307,10 +309,10 @@ cudaError_t launch_factor(sfft_plan *p) {
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
         const int rem = n - k0 - bs, nt = (rem + CB - 1) / CB;
-        { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, 0, st>>>(p->Lf, n, k0, bs, p->flag); }
+        { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, 0, st>>>(p->Lf, p->Linv + (size_t)kb * CB * CB, n, k0, bs, p->flag); }
         if (rem > 0) { KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs); }
     }
-    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, CB, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Lf, p->Linv, n); }
+    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, CB, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n); }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     return cudaGetLastError();
 }
