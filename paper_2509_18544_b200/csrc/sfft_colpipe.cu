@@ -177,13 +177,7 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
     const size_t src_plane = (size_t)g.ny * Hx, plane = (size_t)My * Hx;
     const double inv_ny = 1.0 / (double)g.ny;
     const PassTw pw = PassTw();
-    const cplx *wsm = nullptr;
-    if (LOG2N_CT) { // park this thread's pass twiddles in shared memory (3 x T entries behind the ring)
-        cplx *wt = ring + 2 * My;
-        const PassTw ld = load_pass_tw(LOG2N_CT, j, tw, g.Nt);
-        wt[j] = ld.w[0]; wt[T + j] = ld.w[1]; wt[2 * T + j] = ld.w[2];
-        wsm = wt; // each thread reads back only its own entries: no barrier needed
-    }
+    const cplx *wsm = nullptr; // (parking the pass twiddles in shared memory measured slower than the L1/L2 loads)
     auto issue_item = [&](int n) {
         if (n < nitems) {
             const int tile = blockIdx.x + (n / nsrc) * gridDim.x, i = n % nsrc;
@@ -353,7 +347,7 @@ static int colpipe_grid(const Geom &g, int reserve) {
 
 cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj, int nsrc) {
     const Geom &g = p->g;
-    const size_t smem = (size_t)(padded_lenE<CP_E>(g.My) + 2 * g.My + (g.log2My == 12 ? 3 * g.My / CP_E : 0)) * sizeof(cplx);
+    const size_t smem = (size_t)(padded_lenE<CP_E>(g.My) + 2 * g.My + 0) * sizeof(cplx);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(colpipe_fwd_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
