@@ -82,10 +82,16 @@ static void free_plan(sfft_plan *p) {
         if (p->ev1[s]) cudaEventDestroy(p->ev1[s]);
     }
     if (p->side) cudaStreamDestroy(p->side);
+    if (p->sideB) cudaStreamDestroy(p->sideB);
+    if (p->sideC) cudaStreamDestroy(p->sideC);
+    if (p->ev_joinB) cudaEventDestroy(p->ev_joinB);
+    if (p->ev_joinC) cudaEventDestroy(p->ev_joinC);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->fstream) cudaStreamDestroy(p->fstream);
     if (p->ev_ffork) cudaEventDestroy(p->ev_ffork);
+    if (p->cstream) cudaStreamDestroy(p->cstream);
+    if (p->ev_copy) cudaEventDestroy(p->ev_copy);
     if (p->ev_fjoin) cudaEventDestroy(p->ev_fjoin);
     for (int k = 0; k < MAX_KREC; k++)
         if (p->krec[k].e0) { cudaEventDestroy(p->krec[k].e0); cudaEventDestroy(p->krec[k].e1); }
@@ -171,6 +177,10 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     p->stream = 0; p->cur = 0;
     p->no_side = getenv("SFFT_NO_SIDE") != nullptr;
     cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
+    cudaStreamCreateWithFlags(&p->sideB, cudaStreamNonBlocking);
+    cudaStreamCreateWithFlags(&p->sideC, cudaStreamNonBlocking);
+    cudaEventCreateWithFlags(&p->ev_joinB, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&p->ev_joinC, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
     {   // highest priority: the factorisation is a chain of small dependent launches; its CTAs should take
@@ -180,6 +190,8 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
         cudaStreamCreateWithPriority(&p->fstream, cudaStreamNonBlocking, hi);
     }
     cudaEventCreateWithFlags(&p->ev_ffork, cudaEventDisableTiming);
+    cudaStreamCreateWithFlags(&p->cstream, cudaStreamNonBlocking);
+    cudaEventCreateWithFlags(&p->ev_copy, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_fjoin, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
     // Phi (pin P7): closed form, mask independent
@@ -240,7 +252,8 @@ static sfft_status template_side(sfft_plan *p) {
     {
         StageTimer tm(p, SFFT_STAGE_A2_OMEGA);
         fork_side(p);
-        CK(launch_gamma(p), "gamma");           // on the side stream, beside the Omega column pass
+        use_side(p, 2);
+        CK(launch_gamma(p), "gamma");           // on a side stream, beside the Omega column pass
         back_to_main(p);
         CK(launch_lags(p, p->plO, 2 * g.w, p->lagO, false), "lags(Omega)"); // joins the side stream
     }
@@ -263,6 +276,7 @@ static sfft_status science_side(sfft_plan *p) {
     {
         StageTimer tm(p, SFFT_STAGE_A2_THETA);
         fork_side(p);
+        use_side(p, 2);
         CK(launch_delta(p), "delta");
         back_to_main(p);
         CK(launch_lags(p, p->plT, g.w, p->lagT, true), "lags(Theta)");
@@ -291,6 +305,10 @@ sfft_status sfft_build_system(sfft_plan *p, const double *S, const double *R, co
         }
         back_to_main(p);
         p->have_factor = true;
+    }
+    if (p->science_waits_copy) { // sfft_difference_host: S is still on its way over PCIe (copy stream)
+        CK(cudaStreamWaitEvent(p->stream, p->ev_copy, 0), "wait for the S upload");
+        p->science_waits_copy = false;
     }
     st = science_side(p);
     if (st != SFFT_OK) return st;
@@ -383,7 +401,7 @@ sfft_status sfft_sync_status(sfft_plan *p) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     join_factor(p);
     CK(cudaStreamSynchronize(p->stream), "sync");
-    if (p->side) CK(cudaStreamSynchronize(p->side), "sync side");
+    if (p->side) { CK(cudaStreamSynchronize(p->side), "sync side"); CK(cudaStreamSynchronize(p->sideB), "sync side"); CK(cudaStreamSynchronize(p->sideC), "sync side"); }
     if (p->have_factor) {
         CK(cudaMemcpy(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost), "read flag");
         if (*p->flag_host) return fail(p, SFFT_ERR_NOT_SPD, "pivot <= 1e-12: matrix not positive definite");
@@ -401,9 +419,15 @@ sfft_status sfft_difference_host(sfft_plan *p, const double *S_host, const doubl
         CK(dalloc(p, &p->stD, npix), "alloc staging");
     }
     if (mask_host && !p->stM) CK(dalloc(p, &p->stM, npix), "alloc staging");
-    CK(cudaMemcpyAsync(p->stS, S_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->stream), "H2D S");
-    CK(cudaMemcpyAsync(p->stR, R_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->stream), "H2D R");
+    // R (and the mask) first on the caller's stream; S follows on the copy stream and overlaps the template-side
+    // a1/a2 (the previous call ended with a full synchronisation, so the staging buffers are free)
     if (mask_host) CK(cudaMemcpyAsync(p->stM, mask_host, npix, cudaMemcpyHostToDevice, p->stream), "H2D mask");
+    CK(cudaMemcpyAsync(p->stR, R_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->stream), "H2D R");
+    CK(cudaEventRecord(p->ev_copy, p->stream), "order the S upload after the R upload");
+    CK(cudaStreamWaitEvent(p->cstream, p->ev_copy, 0), "order the S upload");
+    CK(cudaMemcpyAsync(p->stS, S_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->cstream), "H2D S");
+    CK(cudaEventRecord(p->ev_copy, p->cstream), "H2D S done");
+    p->science_waits_copy = true;
     sfft_status st = sfft_build_system(p, p->stS, p->stR, mask_host ? p->stM : nullptr);
     if (st == SFFT_OK) st = sfft_solve(p);
     if (st == SFFT_OK) st = sfft_subtract(p, p->stD, nullptr);

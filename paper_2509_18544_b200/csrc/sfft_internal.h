@@ -41,10 +41,14 @@ struct sfft_plan {
     sfft::Geom g;
     cudaStream_t stream;     // the caller's stream: every call is ordered on it
     cudaStream_t side;       // plan-owned: small independent kernels run beside the big ones (fork/join by events)
+    cudaStream_t sideB, sideC; // two more, so that the independent small chains (packed column | wrap corrections |
+    cudaEvent_t ev_joinB, ev_joinC; // Gamma/Delta) also run beside EACH OTHER: each is latency-bound on a small grid
     cudaStream_t cur;        // stream the launchers enqueue on right now (stream, or side inside a fork)
     cudaEvent_t ev_fork, ev_join;
     cudaStream_t fstream;    // plan-owned: the factorisation of a single pair runs here, beside the science-side a1/a2
     cudaEvent_t ev_ffork, ev_fjoin;
+    cudaStream_t cstream;    // plan-owned copy stream: sfft_difference_host uploads S here while the template side computes
+    cudaEvent_t ev_copy; bool science_waits_copy;
     bool no_side;            // SFFT_NO_SIDE: keep the small kernels on the caller's stream (experiments)
     bool factor_pending;     // factor kernels are enqueued on fstream and not yet joined into `stream`
     // device workspaces
@@ -151,14 +155,21 @@ struct KLaunch {
 // In per-launch timing mode everything stays on the main stream so that kernel times do not overlap.
 inline void fork_side(sfft_plan *p) {
     if (p->ktiming || !p->side || p->no_side) return;
-    cudaEventRecord(p->ev_fork, p->stream); cudaStreamWaitEvent(p->side, p->ev_fork, 0);
+    cudaEventRecord(p->ev_fork, p->stream);
+    cudaStreamWaitEvent(p->side, p->ev_fork, 0); cudaStreamWaitEvent(p->sideB, p->ev_fork, 0); cudaStreamWaitEvent(p->sideC, p->ev_fork, 0);
     p->cur = p->side;
+}
+inline void use_side(sfft_plan *p, int k) { // after fork_side: enqueue on side stream k (0, 1, 2)
+    if (p->ktiming || !p->side || p->no_side) return;
+    p->cur = k == 0 ? p->side : k == 1 ? p->sideB : p->sideC;
 }
 inline void back_to_main(sfft_plan *p) { p->cur = p->stream; }
 inline void join_side(sfft_plan *p) {
     p->cur = p->stream;
     if (p->ktiming || !p->side || p->no_side) return;
     cudaEventRecord(p->ev_join, p->side); cudaStreamWaitEvent(p->stream, p->ev_join, 0);
+    cudaEventRecord(p->ev_joinB, p->sideB); cudaStreamWaitEvent(p->stream, p->ev_joinB, 0);
+    cudaEventRecord(p->ev_joinC, p->sideC); cudaStreamWaitEvent(p->stream, p->ev_joinC, 0);
 }
 
 // the factorisation stream: same fork/join protocol as the side stream

@@ -299,12 +299,13 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     const int nsplit = c.nsplit;
     cudaError_t e;
     // side stream: the packed column kx = 0 / Hx and the wrap corrections (independent of the column pass)
-    if (!p->ktiming && p->side && !p->no_side) p->cur = p->side; // the caller forked already (template_side / science_side)
+    use_side(p, 0); // the caller forked already (template_side / science_side)
     { KLaunch kl(p, science ? "lagedge_theta" : "lagedge_omega"); lagedge_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->cur>>>(ss, pl, W, nsplit, p->Q, g, p->tw); }
     int nchunk = 0;
     double *bpart = p->bpart;
     if (g.Mx != g.nx || g.My != g.ny) {
         nchunk = border_chunks();
+        use_side(p, 1);
         if (W > 0) { e = launch_border(p, pl, W, science, bpart); if (e != cudaSuccess) return e; }
         else nchunk = 0;
     }
