@@ -118,25 +118,29 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
 
 // Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves:
 // Linv[b][i][c], thread c solves column c of  L X = I  by forward substitution.  grid = nblk; block 64.
-__global__ void __launch_bounds__(CB) trinv_kernel(double *__restrict__ Linv, int n) {
+__global__ void __launch_bounds__(256) trinv_kernel(double *__restrict__ Linv, int n) {
     extern __shared__ __align__(16) double dsm[];
     double (*l)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm);
     double (*x)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm + CB * (CB + 1));
-    const int c = threadIdx.x;
+    __shared__ double rdg[CB];
     // Linv[b] holds the factored diagonal block L_bb (identity-padded, written by potrf_panel_kernel): invert in place
-    const double *src = Linv + (size_t)blockIdx.x * CB * CB;
-    for (int e = threadIdx.x; e < CB * CB; e += CB) l[e >> 6][e & 63] = src[e];
+    double *blk = Linv + (size_t)blockIdx.x * CB * CB;
+    for (int e = threadIdx.x; e < CB * CB; e += 256) l[e >> 6][e & 63] = blk[e];
     __syncthreads();
+    if (threadIdx.x < CB) rdg[threadIdx.x] = 1.0 / l[threadIdx.x][threadIdx.x];
+    __syncthreads();
+    // column c of X by forward substitution; its 4 lanes (adjacent, same warp) split every dot product
+    const int c = threadIdx.x >> 2, part = threadIdx.x & 3;
     for (int i = 0; i < CB; i++) {
-        double s0 = (i == c) ? 1.0 : 0.0, s1 = 0.0;
-        int m = c;
-        for (; m + 1 < i; m += 2) { s0 = fma(-l[i][m], x[m][c], s0); s1 = fma(-l[i][m + 1], x[m + 1][c], s1); }
-        if (m < i) s0 = fma(-l[i][m], x[m][c], s0);
-        x[i][c] = i >= c ? (s0 + s1) / l[i][i] : 0.0;
+        double s = 0.0;
+        for (int m = c + part; m < i; m += 4) s = fma(-l[i][m], x[m][c], s);
+        s += __shfl_xor_sync(0xffffffffu, s, 1);
+        s += __shfl_xor_sync(0xffffffffu, s, 2);
+        if (part == 0) x[i][c] = i >= c ? ((i == c ? 1.0 : 0.0) + s) * rdg[i] : 0.0;
+        __syncwarp();
     }
     __syncthreads();
-    double *dst = Linv + (size_t)blockIdx.x * CB * CB;
-    for (int e = threadIdx.x; e < CB * CB; e += CB) dst[e] = x[e >> 6][e & 63];
+    for (int e = threadIdx.x; e < CB * CB; e += 256) blk[e] = x[e >> 6][e & 63];
 }
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
@@ -312,7 +316,7 @@ cudaError_t launch_factor(sfft_plan *p) {
         { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, 0, st>>>(p->Lf, p->Linv + (size_t)kb * CB * CB, n, k0, bs, p->flag); }
         if (rem > 0) { KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs); }
     }
-    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, CB, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n); }
+    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, 256, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n); }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     return cudaGetLastError();
 }
