@@ -93,6 +93,9 @@ static void free_plan(sfft_plan *p) {
     if (p->cstream) cudaStreamDestroy(p->cstream);
     if (p->ev_copy) cudaEventDestroy(p->ev_copy);
     if (p->ev_fjoin) cudaEventDestroy(p->ev_fjoin);
+    if (p->fstream2) cudaStreamDestroy(p->fstream2);
+    if (p->ev_lookP) cudaEventDestroy(p->ev_lookP);
+    if (p->ev_lookB) cudaEventDestroy(p->ev_lookB);
     for (int k = 0; k < MAX_KREC; k++)
         if (p->krec[k].e0) { cudaEventDestroy(p->krec[k].e0); cudaEventDestroy(p->krec[k].e1); }
     delete p;
@@ -129,7 +132,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
 
     const size_t plane = (size_t)g.My * g.Hx;
     const int W2 = 4 * g.w + 1, n = g.n;
-    LagCfg cO, cT; lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.NK + 1, g.w, &cT);
+    LagCfg cO, cT; lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.NK + 1, g.w, &cT, 16);
     const size_t qO = (size_t)cO.nsplit * p->plO.np * W2 * (g.Hx + 1), qT = (size_t)cT.nsplit * p->plT.np * L * (g.Hx + 1);
     const size_t bO = (size_t)border_chunks() * p->plO.np * W2 * W2;
     cudaError_t e = cudaSuccess;
@@ -193,6 +196,13 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     cudaStreamCreateWithFlags(&p->cstream, cudaStreamNonBlocking);
     cudaEventCreateWithFlags(&p->ev_copy, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_fjoin, cudaEventDisableTiming);
+    {
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        cudaStreamCreateWithPriority(&p->fstream2, cudaStreamNonBlocking, hi);
+    }
+    cudaEventCreateWithFlags(&p->ev_lookP, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&p->ev_lookB, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
     // Phi (pin P7): closed form, mask independent
     double phi[MAX_NP * MAX_NP];

@@ -100,13 +100,14 @@ __global__ void __launch_bounds__(256) linpair_kernel(const double *__restrict__
     }
 }
 
-// One thread per (pair, du, dv): bpart[pair][dvIdx*(2W+1)+duIdx] = X_N - X_M (see the file header).
+// One WARP per (pair, du, dv): bpart[pair][dvIdx*(2W+1)+duIdx] = X_N - X_M (see the file header); the lanes
+// share the wrapped rows, the wrapped columns and the corner terms, then reduce by shuffles.
 __global__ void __launch_bounds__(128) border_combine_kernel(const double *__restrict__ LP, int nchunk, int W, int EA, int EB,
                                                             PairList pl, int sci, const double *__restrict__ R,
                                                             const double *__restrict__ S, const uint8_t *__restrict__ mask,
                                                             double *__restrict__ bpart, Geom g) {
     const int W2 = 2 * W + 1, nl = W2 * W2;
-    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    const int id = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (id >= pl.np * nl) return;
     const int p = id / nl, lag = id - p * nl;
     const int du = lag % W2 - W, dv = lag / W2 - W;
@@ -128,34 +129,35 @@ __global__ void __launch_bounds__(128) border_combine_kernel(const double *__res
         const double sign = pass == 0 ? 1.0 : -1.0;
         const int ddx = abs(du) - (pass == 0 ? 0 : g.Mx - nx), ddy = abs(dv) - (pass == 0 ? 0 : g.My - ny);
         // rows wrap in y, x linear
-        for (int k = 0; k < ddy; k++) {
+        for (int k = lane; k < ddy; k += 32) {
             int r, z, ya, yb, typ;
             if (dv > 0) { r = k + 1; z = ddy - r; ya = ny - r; yb = z; typ = 0; }
             else { z = k; r = ddy - z; ya = z; yb = ny - r; typ = 1; }
             corr += sign * bpw(cy(ya), ja) * bpw(cy(yb), jb) * lp(typ, r - 1, z, du + W, ia, sci ? 0 : ib);
         }
         // columns wrap in x, y linear
-        for (int k = 0; k < ddx; k++) {
+        for (int k = lane; k < ddx; k += 32) {
             int r, z, xa, xb, typ;
             if (du > 0) { r = k + 1; z = ddx - r; xa = nx - r; xb = z; typ = 0; }
             else { z = k; r = ddx - z; xa = z; xb = nx - r; typ = 1; }
             corr += sign * bpw(cx(xa), ia) * bpw(cx(xb), ib) * lp(2 + typ, r - 1, z, dv + W, ja, sci ? 0 : jb);
         }
         // corners: both wrap
-        for (int ky = 0; ky < ddy; ky++) {
-            int ya, yb;
+        const int ncorn = (ddx > 0 && ddy > 0) ? ddx * ddy : 0;
+        for (int e = lane; e < ncorn; e += 32) {
+            const int ky = e / ddx, kx = e - ky * ddx;
+            int ya, yb, xa, xb;
             if (dv > 0) { ya = ny - (ky + 1); yb = ddy - (ky + 1); } else { ya = ky; yb = ny - (ddy - ky); }
-            for (int kx = 0; kx < ddx; kx++) {
-                int xa, xb;
-                if (du > 0) { xa = nx - (kx + 1); xb = ddx - (kx + 1); } else { xa = kx; xb = nx - (ddx - kx); }
-                const size_t oa = (size_t)ya * nx + xa, ob = (size_t)yb * nx + xb;
-                double a = R[oa], b = sci ? S[ob] : R[ob];
-                if (mask) { if (!mask[oa]) a = 0.0; if (!mask[ob]) b = 0.0; }
-                corr += sign * (bpw(cx(xa), ia) * bpw(cy(ya), ja) * a) * (bpw(cx(xb), ib) * bpw(cy(yb), jb) * b);
-            }
+            if (du > 0) { xa = nx - (kx + 1); xb = ddx - (kx + 1); } else { xa = kx; xb = nx - (ddx - kx); }
+            const size_t oa = (size_t)ya * nx + xa, ob = (size_t)yb * nx + xb;
+            double a = R[oa], b = sci ? S[ob] : R[ob];
+            if (mask) { if (!mask[oa]) a = 0.0; if (!mask[ob]) b = 0.0; }
+            corr += sign * (bpw(cx(xa), ia) * bpw(cy(ya), ja) * a) * (bpw(cx(xb), ib) * bpw(cy(yb), jb) * b);
         }
     }
-    bpart[(size_t)p * nl + lag] = corr;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) corr += __shfl_down_sync(0xffffffffu, corr, off);
+    if (lane == 0) bpart[(size_t)p * nl + lag] = corr;
 }
 
 size_t border_lp_doubles(const Geom &g, int W, int EB) {
@@ -201,7 +203,7 @@ cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science,
     {
         KLaunch kl(p, science ? "border_combine_theta" : "border_combine_omega");
         const int total = pl.np * (2 * W + 1) * (2 * W + 1);
-        border_combine_kernel<<<(total + 127) / 128, 128, 0, p->cur>>>(p->LP, nchunk, W, g.DK + 1, science ? 1 : g.DK + 1, pl,
+        border_combine_kernel<<<(total + 3) / 4, 128, 0, p->cur>>>(p->LP, nchunk, W, g.DK + 1, science ? 1 : g.DK + 1, pl,
                                                                             science ? 1 : 0, p->R, p->S, p->mask, bpart, g);
     }
     return cudaGetLastError();

@@ -35,6 +35,7 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_fwd_kernel(const dou
     double *wpart = reinterpret_cast<double *>(reinterpret_cast<cplx *>(smem_raw) + (size_t)RPB * padded_lenE<E>(Hx));
     const double inv_nx = 1.0 / (double)g.nx;
     const size_t rowoff = (size_t)row * g.nx;
+    const bool vec = ((g.nx & 1) == 0) && (((size_t)img & 15) == 0);
 
     for (int i = 0; i < NI; i++) {
         cplx v[E];
@@ -46,8 +47,16 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_fwd_kernel(const dou
             const int x0 = 2 * (j + q * T);
             double a = 0.0, b = 0.0;
             if (live) {
-                if (x0 < g.nx) { a = img[rowoff + x0]; if (mask && !mask[rowoff + x0]) a = 0.0; }
-                if (x0 + 1 < g.nx) { b = img[rowoff + x0 + 1]; if (mask && !mask[rowoff + x0 + 1]) b = 0.0; }
+                if (vec) { // even nx, 16-byte aligned image: one 16-byte load per pixel pair
+                    if (x0 < g.nx) { const double2 ab = *reinterpret_cast<const double2 *>(img + rowoff + x0); a = ab.x; b = ab.y; }
+                } else {
+                    if (x0 < g.nx) a = img[rowoff + x0];
+                    if (x0 + 1 < g.nx) b = img[rowoff + x0 + 1];
+                }
+                if (mask) {
+                    if (x0 < g.nx && !mask[rowoff + x0]) a = 0.0;
+                    if (x0 + 1 < g.nx && !mask[rowoff + x0 + 1]) b = 0.0;
+                }
             }
             const double xa = (2.0 * x0 + 1.0 - g.nx) * inv_nx, xb = (2.0 * x0 + 3.0 - g.nx) * inv_nx;
             if (i == 0 && NMOM > 0) {

@@ -47,6 +47,8 @@ struct sfft_plan {
     cudaEvent_t ev_fork, ev_join;
     cudaStream_t fstream;    // plan-owned: the factorisation of a single pair runs here, beside the science-side a1/a2
     cudaEvent_t ev_ffork, ev_fjoin;
+    cudaStream_t fstream2;   // look-ahead of the blocked Cholesky: the rest of a trailing update runs here
+    cudaEvent_t ev_lookP, ev_lookB;
     cudaStream_t cstream;    // plan-owned copy stream: sfft_difference_host uploads S here while the template side computes
     cudaEvent_t ev_copy; bool science_waits_copy;
     bool no_side;            // SFFT_NO_SIDE: keep the small kernels on the caller's stream (experiments)
@@ -112,7 +114,8 @@ cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int 
 cudaError_t launch_colpipe_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter);
 
 struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split; };
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c);
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split = 1);
+int theta_min_split();
 int border_chunks();
 int border_linpair_chunks();
 size_t border_lp_doubles(const Geom &g, int W, int EB);

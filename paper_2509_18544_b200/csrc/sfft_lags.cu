@@ -18,6 +18,7 @@
 //   lagedge_kernel the packed column kx = 0 (DC + i Nyquist) untangled -> Q[.][.][0], Q[.][.][Hx]
 //   (sfft_border.cu) the wrap corrections X_N - X_M from border strips
 //   lagrow_kernel  stage 2: lag[p][dv][du] = 1/(Mx My) sum_kx g Re(Q e^{2 pi i kx du/Mx}) + border
+#include <cstdlib>
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -250,7 +251,9 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
 // ---------------------------------------------------------------- host side
 // Launch shape of stage 1 (also used by the plan to size Q): pick the kx chunk and the b split that
 // minimise  waves * (work per CTA)  on 148 SMs x CTAs per SM, preferring wide chunks and few splits.
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c) {
+// min_split > 1: cut the ky range into at least that many CTAs per kx chunk -- short-lived CTAs, so that the
+// kernels of a factorisation running beside this pass find free SM slots often (see sfft_build_system).
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split) {
     const int WB = W <= 3 ? 3 : W <= 5 ? 5 : W <= 6 ? 6 : W <= 10 ? 10 : 20;
     const int halves = WB > 10 ? 2 : 1, per_sm = WB > 10 ? 1 : 2, maxthreads = 192;
     const int Tb = g.My / LC_NA;
@@ -262,6 +265,7 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c) {
         const int ngr = (np + npg - 1) / npg, nkb = (g.Hx + KXC - 1) / KXC;
         for (int nsplit = 1; nsplit <= 16; nsplit *= 2) {
             if (Tb / nsplit < 4 && nsplit > 1) break;
+            if (nsplit < min_split && Tb / (2 * nsplit) >= 4 && nsplit < 16) continue;
             const long long ncta = (long long)nkb * ngr * nsplit * halves, slots = 148LL * per_sm;
             const long long waves = (ncta + slots - 1) / slots;
             // a CTA with few threads keeps the FP64 pipes idle: charge it as if it had at least 160
@@ -288,6 +292,7 @@ static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const Pai
 }
 
 int border_chunks() { return 1; }
+int theta_min_split() { static int v = -1; if (v < 0) { const char *e = getenv("SFFT_THETA_SPLIT"); v = e ? atoi(e) : 1; } return v; }
 
 cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bool science) {
     const Geom &g = p->g;
@@ -295,7 +300,7 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     for (int t = 0; t < g.NK; t++) ss.p[t] = p->specT + (size_t)t * g.My * g.Hx;
     ss.p[g.NK] = p->specS;
     const int ns = science ? g.NK + 1 : g.NK;
-    LagCfg c; lagcol_config(g, pl.np, ns, W, &c);
+    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, science && p->factor_pending ? theta_min_split() : 1);
     const int nsplit = c.nsplit;
     cudaError_t e;
     // side stream: the packed column kx = 0 / Hx and the wrap corrections (independent of the column pass)

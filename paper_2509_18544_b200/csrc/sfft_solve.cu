@@ -4,6 +4,7 @@
 // solve, trailing update C -= X X^T on the FP64 tensor pipe (mma.sync m8n8k4 f64 -- the one
 // dense contraction of the path).  A pivot L_kk^2 <= 1e-12 raises the device flag
 // (SFFT_ERR_NOT_SPD).  c = D^-1/2 L^-T L^-1 D^-1/2 h by two blocked triangular solves.
+#include <cstdlib>
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -150,14 +151,21 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
 
 // trailing update: for block rows bi >= bj > kb:  A[bi][bj] -= X_bi X_bj^T,  X = panel columns k0..k0+bs.
 // grid = ntile*(ntile+1)/2 lower-triangular tile pairs; block 256 = 8 warps, warp tile 16 x 32.
-__global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int n, int k0, int bs, int t0 /*first trailing row*/) {
+// mode 0: all tiles; 1: only the first block column (bj = 0; grid = ntile) -- all the next panel needs;
+// 2: the other block columns (bj >= 1; grid = (ntile-1) ntile/2), run beside the next panel (look-ahead).
+__global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int n, int k0, int bs, int t0 /*first trailing row*/,
+                                                  int mode) {
     extern __shared__ __align__(16) double dsm[];
     double (*As)[CLD] = reinterpret_cast<double (*)[CLD]>(dsm);
     double (*Bs)[CLD] = reinterpret_cast<double (*)[CLD]>(dsm + CB * CLD);
     // linear index -> (bi, bj), bj <= bi
-    int idx = blockIdx.x, bi = 0;
-    while (idx > bi) { idx -= bi + 1; bi++; }
-    const int bj = idx;
+    int idx = blockIdx.x, bi = 0, bj;
+    if (mode == 1) { bi = idx; bj = 0; }
+    else {
+        while (idx > bi) { idx -= bi + 1; bi++; }
+        bj = idx;
+        if (mode == 2) { bi++; bj++; }
+    }
     const int i0 = t0 + bi * CB, j0 = t0 + bj * CB;
     for (int e = threadIdx.x; e < CB * CB; e += blockDim.x) {
         const int r = e / CB, c = e % CB;
@@ -310,12 +318,31 @@ cudaError_t launch_factor(sfft_plan *p) {
     const size_t sm_syrk = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
     cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * CB * (CB + 1) * sizeof(double)));
+    // Look-ahead: panel k+1 needs only the first block column of panel k's trailing update.  That part runs on
+    // the factor's stream; the rest of the update runs on an auxiliary stream beside the next panel kernel
+    // (whose 64-step dependent chain leaves the machine almost empty).
+    cudaStream_t aux = (p->ktiming || !p->fstream2 || getenv("SFFT_NO_LOOKAHEAD")) ? nullptr : p->fstream2;
+    bool aux_busy = false;
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
         const int rem = n - k0 - bs, nt = (rem + CB - 1) / CB;
         { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, 0, st>>>(p->Lf, p->Linv + (size_t)kb * CB * CB, n, k0, bs, p->flag); }
-        if (rem > 0) { KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs); }
+        if (rem <= 0) continue;
+        if (!aux || nt < 2) {
+            if (aux_busy) { cudaStreamWaitEvent(st, p->ev_lookB, 0); aux_busy = false; }
+            KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs, 0);
+            continue;
+        }
+        cudaEventRecord(p->ev_lookP, st);                                   // panel k is in place
+        if (aux_busy) cudaStreamWaitEvent(st, p->ev_lookB, 0);              // the previous rest-update touched these tiles too
+        { KLaunch kl(p, "syrk"); syrk_kernel<<<nt, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs, 1); }
+        cudaStreamWaitEvent(aux, p->ev_lookP, 0);
+        syrk_kernel<<<(nt - 1) * nt / 2, 256, sm_syrk, aux>>>(p->Lf, n, k0, bs, k0 + bs, 2);
+        p->launches++;
+        cudaEventRecord(p->ev_lookB, aux);
+        aux_busy = true;
     }
+    if (aux_busy) cudaStreamWaitEvent(st, p->ev_lookB, 0);
     { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, 256, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n); }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     return cudaGetLastError();
