@@ -519,6 +519,17 @@ sfft_status sfft_debug_read(sfft_plan *p, int which, int idx, void *host_dst, si
     }
     if (nbytes != sz) return fail(p, SFFT_ERR_INVALID_ARG, "debug_read: size mismatch");
     CK(cudaStreamSynchronize(p->stream), "sync");
+    if (which <= 1) { // spectra are tile-major on the device (spec_idx): hand them out as [My][Hx]
+        cplx *tmp = (cplx *)malloc(sz);
+        if (!tmp) return fail(p, SFFT_ERR_ALLOC, "debug_read: host allocation failed");
+        cudaError_t e = cudaMemcpy(tmp, src, sz, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess)
+            for (int ky = 0; ky < g.My; ky++)
+                for (int kx = 0; kx < g.Hx; kx++) ((cplx *)host_dst)[(size_t)ky * g.Hx + kx] = tmp[spec_idx(ky, kx, g.My)];
+        free(tmp);
+        CK(e, "debug copy");
+        return SFFT_OK;
+    }
     CK(cudaMemcpy(host_dst, src, sz, cudaMemcpyDeviceToHost), "debug copy");
     return SFFT_OK;
 }

@@ -34,7 +34,8 @@ __device__ __forceinline__ double ipw3(double b, int e) { double r = 1.0; for (i
 // Lanes 2k, 2k+1 copy the two 16-byte halves of the SAME 32-byte row segment (first the even lane's
 // row, then the odd lane's), so a warp request covers whole sectors; the data of a thread is copied
 // by itself and its lane partner: cpa_wait + __syncwarp() make it visible, no CTA barrier.
-__device__ __forceinline__ void chunk_issue(cplx *slot, const cplx *tile_src, int h, int Hx, int nrows, int j, int T) {
+// rs = row stride of the source in complex elements (Hx for the row-major intermediates, 2 for tile-major spectra)
+__device__ __forceinline__ void chunk_issue(cplx *slot, const cplx *tile_src, int h, int rs, int nrows, int j, int T) {
     const int col = j & 1;
 #pragma unroll
     for (int qq = 0; qq < CP_E / 2; qq++) {
@@ -42,14 +43,14 @@ __device__ __forceinline__ void chunk_issue(cplx *slot, const cplx *tile_src, in
         for (int o = 0; o < 2; o++) {
             const int jo = (j & ~1) | o, row = jo + (2 * qq + h) * T;
             const bool ok = row < nrows;
-            cpa16(slot + (size_t)(qq * T + jo) * 2 + col, ok ? tile_src + (size_t)row * Hx + col : tile_src, ok);
+            cpa16(slot + (size_t)(qq * T + jo) * 2 + col, ok ? tile_src + (size_t)row * rs + col : tile_src, ok);
         }
     }
     cpa_commit();
 }
 
 // registers -> global, 32 contiguous bytes per lane pair and row (one shuffle per value)
-__device__ __forceinline__ void store_pair(cplx *tile_dst, const cplx (&v)[2][CP_E], int Hx, int nrows, int j, int T) {
+__device__ __forceinline__ void store_pair(cplx *tile_dst, const cplx (&v)[2][CP_E], int rs, int nrows, int j, int T) {
     const bool odd = j & 1;
 #pragma unroll
     for (int q = 0; q < CP_E; q++) {
@@ -59,8 +60,8 @@ __device__ __forceinline__ void store_pair(cplx *tile_dst, const cplx (&v)[2][CP
         recv.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
         const int rowA = (j & ~1) + q * T, rowB = rowA + 1;
         const cplx va = odd ? recv : v[0][q], vb = odd ? v[1][q] : recv;
-        if (rowA < nrows) tile_dst[(size_t)rowA * Hx + (odd ? 1 : 0)] = va;
-        if (rowB < nrows) tile_dst[(size_t)rowB * Hx + (odd ? 1 : 0)] = vb;
+        if (rowA < nrows) tile_dst[(size_t)rowA * rs + (odd ? 1 : 0)] = va;
+        if (rowB < nrows) tile_dst[(size_t)rowB * rs + (odd ? 1 : 0)] = vb;
     }
 }
 
@@ -206,7 +207,7 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
             }
             if (k == last) { __syncwarp(); issue_item(n + 1); } // both lanes of a pair have read: the slots are free
             fft2col<-1, false, LOG2N_CT>(v, X, g.log2My, j, tw, g.Nt, pw, wsm);
-            store_pair(spec + (size_t)k * plane + 2 * tile, v, Hx, My, j, T);
+            store_pair(spec + (size_t)k * plane + (size_t)tile * My * 2, v, 2, My, j, T);
         }
     }
     cpa_wait<0>();
@@ -254,7 +255,7 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
     auto issue_chunk = [&](int s) { // chunk s = ((tile index * NK) + t) * 2 + h  ->  slot h
         if (s < nchunks) {
             const int tile = blockIdx.x + (s / (2 * NK)) * gridDim.x, t = (s >> 1) % NK, h = s & 1;
-            chunk_issue(ring + h * My, spec + (size_t)t * plane + 2 * tile, h, Hx, My, j, T);
+            chunk_issue(ring + h * My, spec + (size_t)t * plane + (size_t)tile * My * 2, h, 2, My, j, T);
         } else cpa_commit();
     };
     issue_chunk(0); issue_chunk(1);
@@ -301,7 +302,7 @@ colpipe_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, c
                     const cplx *zc = spec + (size_t)t * plane;
 #pragma unroll
                     for (int qq = 0; qq < 4; qq++) {
-                        const cplx z = cconj(zc[(size_t)((My - (j + (2 * qq + h) * T)) & (My - 1)) * Hx]);
+                        const cplx z = cconj(zc[(size_t)((My - (j + (2 * qq + h) * T)) & (My - 1)) * 2]); // tile 0, column 0
                         cplx &a0 = acc[0][2 * qq + h];
                         a0.x = fma(z.x, k0[qq].x, fma(-z.y, k0[qq].y, a0.x));
                         a0.y = fma(z.x, k0[qq].y, fma(z.y, k0[qq].x, a0.y));

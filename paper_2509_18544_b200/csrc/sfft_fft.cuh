@@ -36,6 +36,13 @@ SFFT_HD cplx cscale(cplx a, double s) { return mk(a.x * s, a.y * s); }
 // multiply by DIR*i  (W4 = exp(DIR*2*pi*i/4))
 template <int DIR> SFFT_HD cplx mul_w4(cplx a) { return DIR > 0 ? mk(-a.y, a.x) : mk(a.y, -a.x); }
 
+// Spectra are stored TILE-MAJOR: column tiles of 2 adjacent kx, rows contiguous inside a tile,
+//   element (ky, kx) of a My x Hx spectrum  ->  ((kx >> 1) * My + ky) * 2 + (kx & 1).
+// The column pass then writes (and the subtraction reads) whole 128-byte lines -- scattered 32-byte
+// sector stores of the row-major layout ran at a quarter of the line-store rate -- and the lag pass
+// still finds the two columns of a tile in one 32-byte sector.
+SFFT_HD size_t spec_idx(int ky, int kx, int My) { return ((size_t)(kx >> 1) * My + ky) * 2 + (kx & 1); }
+
 SFFT_HD int pad16(int i) { return i + (i >> 4); }
 SFFT_HD int padded_len(int N) { return N + (N >> 4); }
 

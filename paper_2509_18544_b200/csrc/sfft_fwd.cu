@@ -135,9 +135,9 @@ __global__ void __launch_bounds__(512) col_fwd_kernel(const cplx *__restrict__ i
         v[q] = a;
     }
     fft_block<-1>(v, s, g.log2My, j, tw, g.Nt);
-    cplx *dst = spec + (size_t)k * My * Hx + col;
+    cplx *dst = spec + (size_t)k * My * Hx;
 #pragma unroll
-    for (int q = 0; q < 16; q++) dst[(size_t)(j + q * T) * Hx] = v[q];
+    for (int q = 0; q < 16; q++) dst[spec_idx(j + q * T, col, My)] = v[q];
 }
 
 // values per thread of the row / column transforms: 8 keeps a thread under 64 registers (twice the

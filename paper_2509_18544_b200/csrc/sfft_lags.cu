@@ -90,10 +90,10 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
         gsrc[u] = nullptr; soff[u] = 0;
         if (idx < row_elems) {
             const int s = idx / KXC; int kx = kx0 + (idx - s * KXC); if (kx >= Hx) kx = Hx - 1;
-            gsrc[u] = ss.p[s] + kx; soff[u] = idx;
+            gsrc[u] = ss.p[s] + spec_idx(0, kx, My); soff[u] = idx;
         }
     }
-    const size_t astride = (size_t)Tb * Hx;
+    const size_t astride = (size_t)Tb * 2; // tile-major spectra: consecutive ky of one column are 2 elements apart
     auto issue = [&](int it) {
         if (it < nIt) {
             cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
@@ -101,7 +101,7 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
 #pragma unroll
             for (int u = 0; u < 2; u++)
                 if (gsrc[u]) {
-                    const cplx *src = gsrc[u] + (size_t)b * Hx;
+                    const cplx *src = gsrc[u] + (size_t)b * 2;
 #pragma unroll
                     for (int a = 0; a < LC_NA; a++) cp_async16(st + a * row_elems + soff[u], src + a * astride);
                 }
@@ -179,8 +179,8 @@ __global__ void __launch_bounds__(256) lagedge_kernel(SpecSet ss, PairList pl, i
     double q0r = 0, q0i = 0, qhr = 0, qhi = 0;
     for (int ky = threadIdx.x; ky < My; ky += blockDim.x) {
         const int kn = (My - ky) & (My - 1);
-        const cplx a = FA[(size_t)ky * Hx], am = cconj(FA[(size_t)kn * Hx]);
-        const cplx b = FB[(size_t)ky * Hx], bm = cconj(FB[(size_t)kn * Hx]);
+        const cplx a = FA[(size_t)ky * 2], am = cconj(FA[(size_t)kn * 2]); // column 0 of tile 0
+        const cplx b = FB[(size_t)ky * 2], bm = cconj(FB[(size_t)kn * 2]);
         const cplx A0 = mk(0.5 * (a.x + am.x), 0.5 * (a.y + am.y)), AH = mk(0.5 * (a.y - am.y), -0.5 * (a.x - am.x));
         const cplx B0 = mk(0.5 * (b.x + bm.x), 0.5 * (b.y + bm.y)), BH = mk(0.5 * (b.y - bm.y), -0.5 * (b.x - bm.x));
         cplx e = tw[(size_t)((ky * (dv + My)) & (My - 1)) * (g.Nt / My)];

@@ -84,14 +84,14 @@ __global__ void __launch_bounds__(512) col_inv_kernel(const cplx *__restrict__ s
         if (col != 0) {
             for (int t = 0; t < NK; t++) {
                 const cplx k = khat(et + (size_t)t * L * es + c, es, w, cs, sn);
-                acc = cadd(acc, cmul(spec[(size_t)t * plane + (size_t)ky * Hx + col], k));
+                acc = cadd(acc, cmul(spec[(size_t)t * plane + spec_idx(ky, col, My)], k));
             }
         } else {
             // packed column: Z = F0 + i FH  ->  M0 = sum F0 K^(kx=0), MH = sum FH K^(kx=Hx), repacked M0 + i MH
             const int kn = (My - ky) & (My - 1);
             cplx a0 = mk(0, 0), aH = mk(0, 0);
             for (int t = 0; t < NK; t++) {
-                const cplx z = spec[(size_t)t * plane + (size_t)ky * Hx], zm = cconj(spec[(size_t)t * plane + (size_t)kn * Hx]);
+                const cplx z = spec[(size_t)t * plane + spec_idx(ky, 0, My)], zm = cconj(spec[(size_t)t * plane + spec_idx(kn, 0, My)]);
                 const cplx F0 = mk(0.5 * (z.x + zm.x), 0.5 * (z.y + zm.y)), FH = mk(0.5 * (z.y - zm.y), -0.5 * (z.x - zm.x));
                 a0 = cadd(a0, cmul(F0, khat(et + (size_t)t * L * es + 0, es, w, cs, sn)));
                 aH = cadd(aH, cmul(FH, khat(et + (size_t)t * L * es + C, es, w, cs, sn)));
