@@ -272,6 +272,8 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_spli
             const int thr = npg * KXC < 160 ? 160 : npg * KXC;
             double cost = (double)waves * thr * ((Tb + nsplit - 1) / nsplit + 6);
             cost *= 1.0 + 0.01 * nsplit + (KXC < 8 ? 0.03 * (8 - KXC) : 0.0);
+            if (KXC & 1) cost *= 1.2; // tile-major spectra: an odd chunk splits 32-byte sectors; and a grid that leaves a few
+                                      // CTA slots free lets the small side-stream kernels run beside this pass
             if (cost < best) { best = cost; bK = KXC; bS = nsplit; bG = npg; }
         }
     }
