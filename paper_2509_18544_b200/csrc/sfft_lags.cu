@@ -33,7 +33,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 constexpr int LC_NA = 16;  // decimation factor: ky = b + (My/16) a, a = 0..15
-constexpr int LC_NST = 4;  // cp.async stage buffers (two consumed, two in flight)
+constexpr int LC_NST = 3;  // cp.async pipeline stages
 
 // Stage 1, output-pruned inverse DFT along ky by decimation:
 //   Q[dv] = sum_ky P[ky] e^{2 pi i ky dv/My},  P = conj(A) B,  ky = b + Tb a  (Tb = My/16)
@@ -111,28 +111,21 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
         cp_async_commit();
     };
 
-    // 4 stage buffers, two b-steps per barrier: after the barrier everyone is done with the two stages of the
-    // previous iteration, which are refilled while the two current ones are consumed.
-    issue(0); issue(1);
-    for (int it = 0; it < nIt; it += 2) {
-        cp_async_wait<0>();            // this thread's copies of stages it, it+1 have landed
-        __syncthreads();               // ... everyone's have, and everyone is done with stages it-2, it-1
-        issue(it + 2); issue(it + 3);
+    for (int it = 0; it < LC_NST - 1; it++) issue(it);
+    for (int it = 0; it < nIt; it++) {
+        cp_async_wait<LC_NST - 2>();   // this thread's copies of stage `it` have landed
+        __syncthreads();               // ... everyone's have, and everyone is done with stage it-1
+        issue(it + LC_NST - 1);        // refill the buffer of stage it-1: one barrier per step
         if (active) {
+            const cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
+            cplx x[LC_NA];
 #pragma unroll
-            for (int sub = 0; sub < 2; sub++) {
-                if (it + sub < nIt) {
-                    const cplx *st = tile + (size_t)((it + sub) % LC_NST) * stage_elems;
-                    cplx x[LC_NA];
-#pragma unroll
-                    for (int a = 0; a < LC_NA; a++) {
-                        const cplx A = st[a * row_elems + sa * KXC + lane], B = st[a * row_elems + sb * KXC + lane];
-                        x[a] = cmulc(A, B);
-                    }
-                    dft16<1>(x);
-                    lag_fold<DLO, DHI>(x, st + LC_NA * row_elems, acc);
-                }
+            for (int a = 0; a < LC_NA; a++) {
+                const cplx A = st[a * row_elems + sa * KXC + lane], B = st[a * row_elems + sb * KXC + lane];
+                x[a] = cmulc(A, B);
             }
+            dft16<1>(x);
+            lag_fold<DLO, DHI>(x, st + LC_NA * row_elems, acc);
         }
     }
     const int kx = kx0 + lane;
