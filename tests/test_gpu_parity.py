@@ -86,6 +86,35 @@ def test_parity_small(nx, ny, L, DK, DB, masked):
     full_parity(S, R, mask, L, DK, DB, noise_rms=20.0)
 
 
+def test_masked_pair_on_the_pipelined_column_path():
+    """600 x 520 pads to 1024 x 1024: the persistent column kernels (My >= 512), tile-major spectra,
+    a mask (separate unmasked template spectra for the subtraction, reading C7) and wrap corrections."""
+    S, R = starfield.random_pair(600, 520, seed=41)
+    rng = np.random.default_rng(6)
+    mask = (rng.random((520, 600)) > 0.03).astype(np.uint8)
+    yy, xx = np.mgrid[:520, :600]
+    mask[(yy - 100) ** 2 + (xx - 450) ** 2 < 64] = 0
+    mask[:3, :40] = 0                                     # masked pixels on the frame border (wrap path)
+    full_parity(S, R, mask, 7, 2, 1, noise_rms=20.0)
+
+
+def test_debug_read_spectrum_layout():
+    """The test hook hands spectra out as [My][Hx] whatever the device layout is: compare the template
+    spectrum t = 0 (no weight) with numpy's rfft2 of the zero-padded frame."""
+    S, R = starfield.random_pair(96, 80, seed=5)
+    p = SfftPlan(96, 80, 3, 1, 0)
+    p.build_system(dev(S), dev(R))
+    Mx, My = p.debug_read(7)
+    spec = p.debug_read(0, 0)
+    pad = np.zeros((My, Mx)); pad[:80, :96] = R
+    ref = np.fft.rfft2(pad)
+    assert np.max(np.abs(spec[:, 1:] - ref[:, 1:Mx // 2])) <= 1e-9 * np.max(np.abs(ref))
+    # column 0 is packed: FFT_y(X[.,0] + i X[.,Hx]) (both real along x)
+    packed = np.fft.fft(np.fft.ifft(ref[:, 0]).real + 1j * np.fft.ifft(ref[:, Mx // 2]).real)
+    assert np.max(np.abs(spec[:, 0] - packed)) <= 1e-9 * np.max(np.abs(ref))
+    p.destroy()
+
+
 def test_minimum_frame_size():
     L = 5
     S, R = starfield.random_pair(2 * L - 1, 2 * L - 1, seed=3)
