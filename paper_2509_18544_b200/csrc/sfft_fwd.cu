@@ -22,7 +22,7 @@ __device__ __forceinline__ double ipow_small(double b, int e) {
 // grid.x = ceil(ny / RPB); block = RPB * T threads, T = Hx/E (E values per thread).
 // dynamic smem: RPB * padded_lenE<E>(Hx) cplx  +  RPB * 8 * 8 doubles (moment partials)
 template <int E, int LOG2N_CT = 0>
-__global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
+__global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
                                                      cplx *__restrict__ inter, int NI, double *__restrict__ mu, int NMOM,
                                                      Geom g, const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];

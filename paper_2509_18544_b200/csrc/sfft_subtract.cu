@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(512) col_inv_kernel(const cplx *__restrict__ s
 
 // grid.x = ceil(ny/RPB); block = RPB*T, T = Hx/E.  dynamic smem: RPB*padded_lenE<E>(Hx) cplx
 template <int E, int LOG2N_CT = 0>
-__global__ void __launch_bounds__(256, E == 16 ? 2 : 3) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
+__global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
                                                      const double *__restrict__ coef, double *__restrict__ D, Geom g,
                                                      const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
