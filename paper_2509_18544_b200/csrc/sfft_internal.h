@@ -114,7 +114,8 @@ cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int 
 cudaError_t launch_colpipe_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter);
 
 struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split; };
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split = 1);
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split = 1, int reserve = 0);
+int theta_reserve();
 int theta_min_split();
 int border_chunks();
 int border_linpair_chunks();

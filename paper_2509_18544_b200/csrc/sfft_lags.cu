@@ -18,6 +18,7 @@
 //   lagedge_kernel the packed column kx = 0 (DC + i Nyquist) untangled -> Q[.][.][0], Q[.][.][Hx]
 //   (sfft_border.cu) the wrap corrections X_N - X_M from border strips
 //   lagrow_kernel  stage 2: lag[p][dv][du] = 1/(Mx My) sum_kx g Re(Q e^{2 pi i kx du/Mx}) + border
+#include <cstdio>
 #include <cstdlib>
 #include "sfft_internal.h"
 
@@ -32,8 +33,24 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
+// mbarrier helpers (shared::cta): the lag pipeline synchronises per STAGE (copies landed / stage consumed)
+// instead of with CTA-wide barriers, so warps may run up to a stage apart
+__device__ __forceinline__ void mbar_init(unsigned long long *b, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *b) {
+    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_on_copies(unsigned long long *b) { // arrives when this thread's earlier cp.async land
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(b);
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(a), "r"(parity) : "memory");
+}
+
 constexpr int LC_NA = 16;  // decimation factor: ky = b + (My/16) a, a = 0..15
-constexpr int LC_NST = 3;  // cp.async pipeline stages
+constexpr int LC_NST = 4;  // cp.async pipeline stages (prefetch distance 2, refill of the stage consumed 2 steps ago)
 
 // Stage 1, output-pruned inverse DFT along ky by decimation:
 //   Q[dv] = sum_ky P[ky] e^{2 pi i ky dv/My},  P = conj(A) B,  ky = b + Tb a  (Tb = My/16)
@@ -111,13 +128,25 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
         cp_async_commit();
     };
 
-    for (int it = 0; it < LC_NST - 1; it++) issue(it);
+    // per-stage mbarriers: full[s] completes when every thread's copies of the stage have landed, done[s] when every
+    // thread has consumed it.  A stage is refilled two steps after its use, so both waits are normally already satisfied.
+    __shared__ unsigned long long full[LC_NST], done[LC_NST];
+    if (threadIdx.x == 0)
+        for (int k = 0; k < LC_NST; k++) { mbar_init(&full[k], blockDim.x); mbar_init(&done[k], blockDim.x); }
+    __syncthreads();
+    for (int it = 0; it < 2; it++)
+        if (it < nIt) { issue(it); mbar_arrive_on_copies(&full[it]); }
     for (int it = 0; it < nIt; it++) {
-        cp_async_wait<LC_NST - 2>();   // this thread's copies of stage `it` have landed
-        __syncthreads();               // ... everyone's have, and everyone is done with stage it-1
-        issue(it + LC_NST - 1);        // refill the buffer of stage it-1: one barrier per step
+        const int st_i = it % LC_NST;
+        mbar_wait(&full[st_i], (unsigned)(it / LC_NST) & 1u);
+        if (it + 2 < nIt) {
+            const int sr = (it + 2) % LC_NST;
+            if (it >= 2) mbar_wait(&done[sr], (unsigned)((it - 2) / LC_NST) & 1u);
+            issue(it + 2);
+            mbar_arrive_on_copies(&full[sr]);
+        }
         if (active) {
-            const cplx *st = tile + (size_t)(it % LC_NST) * stage_elems;
+            const cplx *st = tile + (size_t)st_i * stage_elems;
             cplx x[LC_NA];
 #pragma unroll
             for (int a = 0; a < LC_NA; a++) {
@@ -127,6 +156,7 @@ __device__ __forceinline__ void lagcol_body(const SpecSet &ss, int ns, const Pai
             dft16<1>(x);
             lag_fold<DLO, DHI>(x, st + LC_NA * row_elems, acc);
         }
+        mbar_arrive(&done[st_i]);
     }
     const int kx = kx0 + lane;
     if (active && kx < Hx && kx > 0) { // kx = 0 is the packed column: lagedge_kernel owns Q[.][.][0]
@@ -253,20 +283,23 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
 // minimise  waves * (work per CTA)  on 148 SMs x CTAs per SM, preferring wide chunks and few splits.
 // min_split > 1: cut the ky range into at least that many CTAs per kx chunk -- short-lived CTAs, so that the
 // kernels of a factorisation running beside this pass find free SM slots often (see sfft_build_system).
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split) {
+// reserve > 0: leave that many CTA slots free (a factorisation running beside this pass then finds room)
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split, int reserve) {
     const int WB = W <= 3 ? 3 : W <= 5 ? 5 : W <= 6 ? 6 : W <= 10 ? 10 : 20;
     const int halves = WB > 10 ? 2 : 1, per_sm = WB > 10 ? 1 : 2, maxthreads = 192;
     const int Tb = g.My / LC_NA;
     double best = 1e300; int bK = 4, bS = 1, bG = np;
     for (int KXC = 4; KXC <= 32; KXC++) {
         if (KXC > g.Hx) break;
-        if ((size_t)LC_NST * (LC_NA * ns * KXC + WB) * sizeof(cplx) > (size_t)(per_sm == 2 ? 100 : 200) * 1024) break;
+        if ((size_t)LC_NST * (LC_NA * ns * KXC + WB) * sizeof(cplx) > (size_t)(per_sm == 2 ? 113 : 200) * 1024) break;
         int npg = maxthreads / KXC; if (npg > np) npg = np; if (npg < 1) continue;
         const int ngr = (np + npg - 1) / npg, nkb = (g.Hx + KXC - 1) / KXC;
         for (int nsplit = 1; nsplit <= 16; nsplit *= 2) {
             if (Tb / nsplit < 4 && nsplit > 1) break;
             if (nsplit < min_split && Tb / (2 * nsplit) >= 4 && nsplit < 16) continue;
-            const long long ncta = (long long)nkb * ngr * nsplit * halves, slots = 148LL * per_sm;
+            const long long ncta = (long long)nkb * ngr * nsplit * halves;
+            long long slots = 148LL * per_sm;
+            if (reserve > 0 && slots > 4 * reserve) slots -= reserve;
             const long long waves = (ncta + slots - 1) / slots;
             // a CTA with few threads keeps the FP64 pipes idle: charge it as if it had at least 160
             const int thr = npg * KXC < 160 ? 160 : npg * KXC;
@@ -294,6 +327,7 @@ static cudaError_t run_lagcol(sfft_plan *p, const SpecSet &ss, int ns, const Pai
 }
 
 int border_chunks() { return 1; }
+int theta_reserve() { static int v = -1; if (v < 0) { const char *e = getenv("SFFT_THETA_RESERVE"); v = e ? atoi(e) : 40; } return v; }
 int theta_min_split() { static int v = -1; if (v < 0) { const char *e = getenv("SFFT_THETA_SPLIT"); v = e ? atoi(e) : 1; } return v; }
 
 cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bool science) {
@@ -302,8 +336,9 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     for (int t = 0; t < g.NK; t++) ss.p[t] = p->specT + (size_t)t * g.My * g.Hx;
     ss.p[g.NK] = p->specS;
     const int ns = science ? g.NK + 1 : g.NK;
-    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, science && p->factor_pending ? theta_min_split() : 1);
+    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, 1, science && p->factor_pending ? theta_reserve() : 0);
     const int nsplit = c.nsplit;
+    if (getenv("SFFT_VERBOSE")) fprintf(stderr, "lagcfg sci=%d np=%d WB=%d KXC=%d npg=%d nkb=%d ngr=%d nsplit=%d halves=%d threads=%d ctas=%d\n", (int)science, pl.np, c.WB, c.KXC, c.npg, c.nkb, c.ngr, c.nsplit, c.halves, c.npg * c.KXC, c.nkb * c.ngr * c.nsplit * c.halves);
     cudaError_t e;
     // side stream: the packed column kx = 0 / Hx and the wrap corrections (independent of the column pass)
     use_side(p, 0); // the caller forked already (template_side / science_side)
