@@ -128,6 +128,8 @@ __device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N_r
                                         const cplx *wsm = nullptr) {
     const int log2N = LOG2N_CT ? LOG2N_CT : log2N_rt;
     const int T = 1 << (log2N - 3);
+    cplx wa = cplx();
+    if (!PW && LOG2N_CT == 12 && !wsm) wa = tw[(size_t)(j & 7) * (Nt >> 6)];
     pass2<8, DIR, true>(v, X, j, T, 0, tw, Nt);
     if (LOG2N_CT) {
         if (wsm) {
@@ -139,6 +141,16 @@ __device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N_r
             case 2: pass2<4, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
             default: pass2<2, DIR, false>(v, X, j, T, log2Ns, tw, Nt); break;
             }
+            return;
+        }
+        if (!PW && LOG2N_CT == 12) {
+            // no registers for resident pass twiddles (forward kernel): fetch the twiddle of pass k+1 BEFORE the
+            // exchange of pass k, so that its L2 latency hides behind the barriers instead of stalling the butterflies
+            const cplx wb = tw[(size_t)(j & 63) * (Nt >> 9)];
+            pass2<8, DIR, true, true>(v, X, j, T, 3, tw, Nt, wa);
+            const cplx wc = tw[(size_t)(j & 511) * (Nt >> 12)];
+            pass2<8, DIR, true, true>(v, X, j, T, 6, tw, Nt, wb);
+            pass2<8, DIR, false, true>(v, X, j, T, 9, tw, Nt, wc);
             return;
         }
         if (6 < log2N) pass2<8, DIR, true, PW>(v, X, j, T, 3, tw, Nt, pw.w[0]);
@@ -166,7 +178,7 @@ __device__ __forceinline__ void fft2col(cplx (&v)[2][CP_E], cplx *X, int log2N_r
 // grid = min(#SM, Hx/2) persistent CTAs; block = My/8; dynamic smem = (padded_lenE<8>(My) + 2 My) cplx.
 template <int LOG2N_CT>
 __global__ void __launch_bounds__(CP_MAXT, 1)
-colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJobs jobs, int nsrc, Geom g,
+colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, unsigned long long jpack, int njobs, int nsrc, Geom g,
                    const cplx *__restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int My = LOG2N_CT ? (1 << LOG2N_CT) : g.My, Hx = g.Hx, T = My / CP_E, j = threadIdx.x;
@@ -190,13 +202,15 @@ colpipe_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, ColJ
     issue_item(0);
     for (int n = 0; n < nitems; n++) {
         const int tile = blockIdx.x + (n / nsrc) * gridDim.x, i = n % nsrc;
+        // jobs packed 4 bits each, (ii << 2) | jj, in a register: no table look-ups on the critical path
         int last = -1;
-        for (int k = 0; k < jobs.ns; k++) if (jobs.ii[k] == i) last = k;
+        for (int k = 0; k < njobs; k++) if ((int)((jpack >> (4 * k + 2)) & 3) == i) last = k;
         cpa_wait<0>();
         __syncwarp();
-        for (int k = 0; k < jobs.ns; k++) {
-            if (jobs.ii[k] != i) continue;
-            const int jp = jobs.jj[k];
+        for (int k = 0; k < njobs; k++) {
+            const int jb = (int)(jpack >> (4 * k)) & 15;
+            if ((jb >> 2) != i) continue;
+            const int jp = jb & 3;
             cplx v[2][CP_E];
 #pragma unroll
             for (int q = 0; q < CP_E; q++) {
@@ -356,12 +370,15 @@ cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int 
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    ColJobs jobs; jobs.ns = ns;
-    for (int k = 0; k < ns; k++) { jobs.ii[k] = ii[k]; jobs.jj[k] = jj[k]; }
+    unsigned long long jpack = 0; // job k: (ii << 2) | jj, both <= 3 (DK <= 3)
+    for (int k = 0; k < ns; k++) {
+        if (ii[k] < 0 || ii[k] > 3 || jj[k] < 0 || jj[k] > 3 || ns > 16) return cudaErrorInvalidValue;
+        jpack |= (unsigned long long)((ii[k] << 2) | jj[k]) << (4 * k);
+    }
     KLaunch kl(p, ns > 1 ? "col_fwd_R" : "col_fwd_S");
     const int grid = colpipe_grid(g, p->factor_pending ? colpipe_reserve() : 0);
-    if (g.log2My == 12) colpipe_fwd_kernel<12><<<grid, g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
-    else colpipe_fwd_kernel<0><<<grid, g.My / CP_E, smem, p->stream>>>(inter, spec, jobs, nsrc, g, p->tw);
+    if (g.log2My == 12) colpipe_fwd_kernel<12><<<grid, g.My / CP_E, smem, p->stream>>>(inter, spec, jpack, ns, nsrc, g, p->tw);
+    else colpipe_fwd_kernel<0><<<grid, g.My / CP_E, smem, p->stream>>>(inter, spec, jpack, ns, nsrc, g, p->tw);
     return cudaGetLastError();
 }
 

@@ -98,6 +98,18 @@ def test_masked_pair_on_the_pipelined_column_path():
     full_parity(S, R, mask, 7, 2, 1, noise_rms=20.0)
 
 
+def test_tall_frame_on_the_compile_time_4096_column_path():
+    """72 x 4000 pads to 128 x 4096: the My = 4096 instances of the pipelined column kernels (the ones the
+    4088 x 4088 bench runs) on a frame the oracle finishes in seconds: 96 zero rows, the packed column
+    kx = 0, a mask and wrap corrections."""
+    nx, ny = 72, 4000
+    S, R = starfield.random_pair(nx, ny, seed=77)
+    rng = np.random.default_rng(8)
+    mask = (rng.random((ny, nx)) > 0.04).astype(np.uint8)
+    mask[ny - 2:, :10] = 0
+    full_parity(S, R, mask, 5, 2, 1, noise_rms=20.0)
+
+
 def test_debug_read_spectrum_layout():
     """The test hook hands spectra out as [My][Hx] whatever the device layout is: compare the template
     spectrum t = 0 (no weight) with numpy's rfft2 of the zero-padded frame."""
