@@ -33,11 +33,93 @@ __global__ void equil_scale_kernel(const double *__restrict__ G, const double *_
 // shared), CTA 0 writes L_kk back, and CTA b then solves its own 64 rows below the block,
 // X L_kk^T = A, by a register-resident right-looking substitution (4 lanes per row, shuffles only).
 // No FP64 division or sqrt on the dependent chain: inv = rsqrt(pivot), L_jj = pivot * inv.
+// The chain is INSTRUCTION-bound (ncu: 40 % issue utilisation on the one busy SM, ~135 instructions per
+// column and thread), so the loops below are written for instruction count:
+//   * the 16 column groups run as 4 chunks of 4 with a compile-time register window WIN = 16, 12, 8, 4
+//     (rolled inside a chunk, the window shifts down one group per iteration);
+//   * the rank-1 updates are UNCONDITIONAL: entries right of the diagonal (c > r), rows already finished
+//     (r <= j) and window slots past the last column only ever receive values that are never read
+//     (every read of areg / xr is guarded by c <= r or c < bs), so no predicates are computed for them;
+//     shared arrays are padded so that those dead reads stay in bounds.
 // grid = max(1, row tiles below); block 256; static smem.
+constexpr int CPAD = CB + 16; // dead-slot reads reach index 63 + 4 * 3
+
+template <int WIN>
+__device__ __forceinline__ void potrf_chunk(double (&areg)[16], double (*col)[CPAD], double *rd, double (*l)[CB + 1],
+                                            double *__restrict__ Ldiag, int j4_0, int r, int cq, int tid, int *flag) {
+#pragma unroll 1
+    for (int j4 = j4_0; j4 < j4_0 + 4; j4++) {
+#pragma unroll
+        for (int jj = 0; jj < 4; jj++) {
+            const int j = 4 * j4 + jj;
+            double *cj = col[jj & 1];
+            if (cq == jj && r >= j) cj[r] = areg[0];
+            __syncthreads();
+            // all shared-memory reads of this step are issued before the rsqrt chain, so their latency hides behind it
+            const double *cjc = cj + 4 * j4 + cq;
+            double piv = cj[j];
+            const double cr = cj[r];
+            double cv[WIN];
+#pragma unroll
+            for (int qq = 0; qq < WIN; qq++) cv[qq] = cjc[4 * qq];
+            if (!(piv > PIVOT_MIN)) { if (tid == 0 && blockIdx.x == 0) *flag = 1; piv = 1.0; }
+            const double inv = rsqrt(piv);
+            const double lr = (r == j) ? piv * inv : cr * inv;
+            if (tid == 0) rd[j] = inv;
+            if (cq == jj && r >= j) areg[0] = lr;
+            const double lri = -lr * inv;
+            if (cq > jj) areg[0] = fma(lri, cv[0], areg[0]);
+#pragma unroll
+            for (int qq = 1; qq < WIN; qq++) areg[qq] = fma(lri, cv[qq], areg[qq]);
+        }
+        {
+            const int c = 4 * j4 + cq;
+            l[r][c] = c <= r ? areg[0] : 0.0;
+            // the factored block goes to Ldiag, NOT back into Lf: the other CTAs of this launch read the
+            // unfactored block from Lf whenever they get scheduled
+            if (blockIdx.x == 0) Ldiag[r * CB + c] = c <= r ? areg[0] : 0.0;
+        }
+#pragma unroll
+        for (int qq = 0; qq < WIN - 1; qq++) areg[qq] = areg[qq + 1];
+        areg[WIN - 1] = 0.0;
+    }
+}
+
+// panel rows: x_j = x_j / l_jj, then x_c -= x_j l_cj for c > j; lanes 4g..4g+3 hold row r; same window shift
+template <int WIN>
+__device__ __forceinline__ void panel_chunk(double (&xr)[16], const double *rd, double (*l)[CB + 1], double *__restrict__ Lf,
+                                            int j4_0, int r, int cq, int lane, int r0, int n, int k0, int bs) {
+#pragma unroll 1
+    for (int j4 = j4_0; j4 < j4_0 + 4; j4++) {
+#pragma unroll
+        for (int jj = 0; jj < 4; jj++) {
+            const int j = 4 * j4 + jj;
+            const double *lc = &l[4 * j4 + cq][j];
+            double lv[WIN];
+#pragma unroll
+            for (int qq = 0; qq < WIN; qq++) lv[qq] = lc[(size_t)4 * qq * (CB + 1)];
+            double xj = xr[0] * rd[j];
+            xj = __shfl_sync(0xffffffffu, xj, (lane & ~3) | jj);
+            if (cq == jj) xr[0] = xj;
+            const double nxj = -xj;
+            if (cq > jj) xr[0] = fma(nxj, lv[0], xr[0]);
+#pragma unroll
+            for (int qq = 1; qq < WIN; qq++) xr[qq] = fma(nxj, lv[qq], xr[qq]);
+        }
+        {
+            const int c = 4 * j4 + cq;
+            if (r0 + r < n && c < bs) Lf[(size_t)(r0 + r) * n + k0 + c] = xr[0];
+        }
+#pragma unroll
+        for (int qq = 0; qq < WIN - 1; qq++) xr[qq] = xr[qq + 1];
+        xr[WIN - 1] = 0.0;
+    }
+}
+
 __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
                                                          int bs, int *flag) {
-    __shared__ double l[CB][CB + 1];
-    __shared__ double col[2][CB];
+    __shared__ double l[CPAD][CB + 1];
+    __shared__ double col[2][CPAD];
     __shared__ double rd[CB];
     const int tid = threadIdx.x, r = tid >> 2, cq = tid & 3, lane = tid & 31;
     const int r0 = k0 + bs + blockIdx.x * CB;
@@ -51,70 +133,19 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
         areg[q] = v;
         xr[q] = (have_rows && r0 + r < n && c < bs) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
     }
-    // Rolled over the 16 column groups (4 columns each) so the code stays small: the register window is
-    // shifted down by one group per iteration, areg[qq] holds columns 4 (j4 + qq) + cq.
-#pragma unroll 1
-    for (int j4 = 0; j4 < CB / 4; j4++) {
-        const int lim = ((r - cq) >> 2) - j4; // r >= cq is not guaranteed: arithmetic shift keeps lim < 0 then
-#pragma unroll
-        for (int jj = 0; jj < 4; jj++) {
-            const int j = 4 * j4 + jj;
-            double *cj = col[jj & 1];
-            if (cq == jj && r >= j) cj[r] = areg[0];
-            __syncthreads();
-            double piv = cj[j];
-            if (!(piv > PIVOT_MIN)) { if (tid == 0 && blockIdx.x == 0) *flag = 1; piv = 1.0; }
-            const double inv = rsqrt(piv);
-            const double lr = (r == j) ? piv * inv : cj[r] * inv;
-            if (tid == 0) rd[j] = inv;
-            if (cq == jj && r >= j) areg[0] = lr;
-            if (r > j) {
-                // c = 4 (j4 + qq) + cq in (j, r]:  qq <= lim  (and cq > jj for qq = 0)
-                const double lri = -lr * inv;
-                const double *cjc = cj + 4 * j4 + cq;
-                if (cq > jj && lim >= 0) areg[0] = fma(lri, cjc[0], areg[0]);
-#pragma unroll
-                for (int qq = 1; qq < 16; qq++)
-                    if (qq <= lim) areg[qq] = fma(lri, cjc[4 * qq], areg[qq]);
-            }
-        }
-        {
-            const int c = 4 * j4 + cq;
-            l[r][c] = c <= r ? areg[0] : 0.0;
-            // the factored block goes to Ldiag, NOT back into Lf: the other CTAs of this launch read the
-            // unfactored block from Lf whenever they get scheduled
-            if (blockIdx.x == 0) Ldiag[r * CB + c] = c <= r ? areg[0] : 0.0;
-        }
-#pragma unroll
-        for (int qq = 0; qq < 15; qq++) areg[qq] = areg[qq + 1];
-        areg[15] = 0.0;
-    }
+    if (tid < 2 * CPAD) col[tid / CPAD][tid % CPAD] = 0.0;       // dead-slot reads must see numbers (0 * NaN would not matter, but keep it clean)
+    for (int e = tid; e < (CPAD - CB) * (CB + 1); e += 256) l[CB + e / (CB + 1)][e % (CB + 1)] = 0.0;
+    __syncthreads();
+    potrf_chunk<16>(areg, col, rd, l, Ldiag, 0, r, cq, tid, flag);
+    potrf_chunk<12>(areg, col, rd, l, Ldiag, 4, r, cq, tid, flag);
+    potrf_chunk<8>(areg, col, rd, l, Ldiag, 8, r, cq, tid, flag);
+    potrf_chunk<4>(areg, col, rd, l, Ldiag, 12, r, cq, tid, flag);
     __syncthreads();
     if (!have_rows) return;
-    // panel rows: x_j = x_j / l_jj, then x_c -= x_j l_cj for c > j; lanes 4g..4g+3 hold row r; same window shift
-#pragma unroll 1
-    for (int j4 = 0; j4 < CB / 4; j4++) {
-#pragma unroll
-        for (int jj = 0; jj < 4; jj++) {
-            const int j = 4 * j4 + jj;
-            double xj = xr[0] * rd[j];
-            xj = __shfl_sync(0xffffffffu, xj, (lane & ~3) | jj);
-            if (cq == jj) xr[0] = xj;
-            const double *lc = &l[4 * j4 + cq][j];
-            const double nxj = -xj;
-            if (cq > jj) xr[0] = fma(nxj, lc[0], xr[0]);
-#pragma unroll
-            for (int qq = 1; qq < 16; qq++)
-                if (qq < CB / 4 - j4) xr[qq] = fma(nxj, lc[(size_t)4 * qq * (CB + 1)], xr[qq]);
-        }
-        {
-            const int c = 4 * j4 + cq;
-            if (r0 + r < n && c < bs) Lf[(size_t)(r0 + r) * n + k0 + c] = xr[0];
-        }
-#pragma unroll
-        for (int qq = 0; qq < 15; qq++) xr[qq] = xr[qq + 1];
-        xr[15] = 0.0;
-    }
+    panel_chunk<16>(xr, rd, l, Lf, 0, r, cq, lane, r0, n, k0, bs);
+    panel_chunk<12>(xr, rd, l, Lf, 4, r, cq, lane, r0, n, k0, bs);
+    panel_chunk<8>(xr, rd, l, Lf, 8, r, cq, lane, r0, n, k0, bs);
+    panel_chunk<4>(xr, rd, l, Lf, 12, r, cq, lane, r0, n, k0, bs);
 }
 
 // Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves:
