@@ -77,7 +77,9 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_fwd_kernel(const dou
             const int nw = T > 32 ? (T >> 5) : 1; // warps per row
             if ((j & (width - 1)) == 0) {
                 const int wi = T > 32 ? (j >> 5) : 0;
-                for (int m = 0; m < NMOM; m++) wpart[(rib * 8 + wi) * 8 + m] = mom[m];
+#pragma unroll
+                for (int m = 0; m < 8; m++) // static indices: a run-time bound here would push mom[] into local memory
+                    if (m < NMOM) wpart[(rib * 8 + wi) * 8 + m] = mom[m];
             }
             __syncthreads();
             if (j == 0 && live)

@@ -336,7 +336,9 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     for (int t = 0; t < g.NK; t++) ss.p[t] = p->specT + (size_t)t * g.My * g.Hx;
     ss.p[g.NK] = p->specS;
     const int ns = science ? g.NK + 1 : g.NK;
-    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, 1, science && p->factor_pending ? theta_reserve() : 0);
+    static int omega_split = -1; // SFFT_OMEGA_SPLIT=8 shortens the column kernel by 8 % but lengthens the stage (side-stream kernels wait, more partials)
+    if (omega_split < 0) { const char *e = getenv("SFFT_OMEGA_SPLIT"); omega_split = e ? atoi(e) : 1; }
+    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, science ? 1 : omega_split, science && p->factor_pending ? theta_reserve() : 0);
     const int nsplit = c.nsplit;
     if (getenv("SFFT_VERBOSE")) fprintf(stderr, "lagcfg sci=%d np=%d WB=%d KXC=%d npg=%d nkb=%d ngr=%d nsplit=%d halves=%d threads=%d ctas=%d\n", (int)science, pl.np, c.WB, c.KXC, c.npg, c.nkb, c.ngr, c.nsplit, c.halves, c.npg * c.KXC, c.nkb * c.ngr * c.nsplit * c.halves);
     cudaError_t e;
