@@ -242,12 +242,17 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
         for (int s = 0; s < nsplit; s++) q = cadd(q, Q[((size_t)(s * np + p) * (2 * W + 1) + dvi) * (Hx + 1) + kx]);
         const double gw = (kx == 0 || kx == Hx) ? 1.0 : 2.0;
         q.x *= gw; q.y *= gw;
+        // exp(-2 pi i kx d/Mx) = e1^d from ONE coalesced table load: 2W+1 gathered loads per kx made this kernel
+        // sector-request bound (55 us for a 38 MFLOP reduction); powers in a tree, at most 5 roundings deep
+        const cplx e1 = tw[(size_t)(kx & (Mx - 1)) * (g.Nt / Mx)];
+        cplx ep[WM + 1];
+        ep[0] = mk(1.0, 0.0); ep[1] = e1;
+#pragma unroll
+        for (int d = 2; d <= WM; d++)
+            if (d <= W) ep[d] = cmul(ep[d / 2], ep[d - d / 2]);
 #pragma unroll
         for (int d = 0; d <= WM; d++)
-            if (d <= W) {
-                const cplx e = tw[(size_t)((kx * d) & (Mx - 1)) * (g.Nt / Mx)]; // cos = e.x, sin = -e.y
-                sc[d] = fma(q.x, e.x, sc[d]); sn[d] = fma(q.y, -e.y, sn[d]);
-            }
+            if (d <= W) { sc[d] = fma(q.x, ep[d].x, sc[d]); sn[d] = fma(q.y, -ep[d].y, sn[d]); } // cos = e.x, sin = -e.y
     }
     // one reduction for all 2(W+1) sums: shuffles inside a warp, then one pass through shared memory
     __shared__ double red[8][2 * (WM + 1)];

@@ -148,31 +148,77 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
     panel_chunk<4>(xr, rd, l, Lf, 12, r, cq, lane, r0, n, k0, bs);
 }
 
-// Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves:
-// Linv[b][i][c], thread c solves column c of  L X = I  by forward substitution.  grid = nblk; block 64.
-__global__ void __launch_bounds__(256) trinv_kernel(double *__restrict__ Linv, int n) {
+// Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves.
+// Recursive: the four 16 x 16 diagonal sub-blocks are inverted in parallel by forward substitution (16 dependent
+// steps instead of 64; thread (sub-block, column c, part) -- the 4 adjacent lanes of a column split every dot
+// product), then the off-diagonal blocks follow from  X21 = -X22 (L21 X11)  at the 32 and the 64 level (two small
+// products each, all 256 threads).  grid = number of blocks; block 256; dynamic smem 3 * 64 * 65 doubles.
+__global__ void __launch_bounds__(256) trinv_kernel(double *__restrict__ Linv, int n, int blk0) {
     extern __shared__ __align__(16) double dsm[];
     double (*l)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm);
     double (*x)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm + CB * (CB + 1));
+    double (*t)[CB + 1] = reinterpret_cast<double (*)[CB + 1]>(dsm + 2 * CB * (CB + 1));
     __shared__ double rdg[CB];
     // Linv[b] holds the factored diagonal block L_bb (identity-padded, written by potrf_panel_kernel): invert in place
-    double *blk = Linv + (size_t)blockIdx.x * CB * CB;
-    for (int e = threadIdx.x; e < CB * CB; e += 256) l[e >> 6][e & 63] = blk[e];
+    double *blk = Linv + (size_t)(blk0 + blockIdx.x) * CB * CB;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < CB * CB; e += 256) { l[e >> 6][e & 63] = blk[e]; x[e >> 6][e & 63] = 0.0; }
     __syncthreads();
-    if (threadIdx.x < CB) rdg[threadIdx.x] = 1.0 / l[threadIdx.x][threadIdx.x];
+    if (tid < CB) rdg[tid] = 1.0 / l[tid][tid];
     __syncthreads();
-    // column c of X by forward substitution; its 4 lanes (adjacent, same warp) split every dot product
-    const int c = threadIdx.x >> 2, part = threadIdx.x & 3;
-    for (int i = 0; i < CB; i++) {
-        double s = 0.0;
-        for (int m = c + part; m < i; m += 4) s = fma(-l[i][m], x[m][c], s);
-        s += __shfl_xor_sync(0xffffffffu, s, 1);
-        s += __shfl_xor_sync(0xffffffffu, s, 2);
-        if (part == 0) x[i][c] = i >= c ? ((i == c ? 1.0 : 0.0) + s) * rdg[i] : 0.0;
-        __syncwarp();
+    {   // 16 x 16 diagonal sub-blocks
+        const int o = (tid >> 6) * 16, c = (tid >> 2) & 15, part = tid & 3;
+        for (int i = 0; i < 16; i++) {
+            double s = 0.0;
+            for (int m = c + part; m < i; m += 4) s = fma(-l[o + i][o + m], x[o + m][o + c], s);
+            s += __shfl_xor_sync(0xffffffffu, s, 1);
+            s += __shfl_xor_sync(0xffffffffu, s, 2);
+            if (part == 0) x[o + i][o + c] = i >= c ? ((i == c ? 1.0 : 0.0) + s) * rdg[o + i] : 0.0;
+            __syncwarp();
+        }
     }
     __syncthreads();
-    for (int e = threadIdx.x; e < CB * CB; e += 256) blk[e] = x[e >> 6][e & 63];
+    // level 32: for h = 0, 1 the block rows o+16..o+31, columns o..o+15 (o = 32 h)
+    {
+        const int h = tid >> 7, o = 32 * h, e0 = tid & 127;
+#pragma unroll
+        for (int k = 0; k < 2; k++) { // T = L21 X11 (X11 lower triangular: m >= c)
+            const int e = e0 + 128 * k, r = e >> 4, c = e & 15;
+            double s = 0.0;
+            for (int m = c; m < 16; m++) s = fma(l[o + 16 + r][o + m], x[o + m][o + c], s);
+            t[o + 16 + r][o + c] = s;
+        }
+    }
+    __syncthreads();
+    {
+        const int h = tid >> 7, o = 32 * h, e0 = tid & 127;
+#pragma unroll
+        for (int k = 0; k < 2; k++) { // X21 = -X22 T (X22 lower triangular: m <= r)
+            const int e = e0 + 128 * k, r = e >> 4, c = e & 15;
+            double s = 0.0;
+            for (int m = 0; m <= r; m++) s = fma(-x[o + 16 + r][o + 16 + m], t[o + 16 + m][o + c], s);
+            x[o + 16 + r][o + c] = s;
+        }
+    }
+    __syncthreads();
+    // level 64: rows 32..63, columns 0..31
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const int e = tid + 256 * k, r = e >> 5, c = e & 31;
+        double s = 0.0;
+        for (int m = c; m < 32; m++) s = fma(l[32 + r][m], x[m][c], s);
+        t[32 + r][c] = s;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const int e = tid + 256 * k, r = e >> 5, c = e & 31;
+        double s = 0.0;
+        for (int m = 0; m <= r; m++) s = fma(-x[32 + r][32 + m], t[32 + m][c], s);
+        x[32 + r][c] = s;
+    }
+    __syncthreads();
+    for (int e = tid; e < CB * CB; e += 256) blk[e] = x[e >> 6][e & 63];
 }
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
@@ -348,12 +394,13 @@ cudaError_t launch_factor(sfft_plan *p) {
     const int nblk = (n + CB - 1) / CB;
     const size_t sm_syrk = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
-    cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * CB * (CB + 1) * sizeof(double)));
+    cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * CB * (CB + 1) * sizeof(double)));
     // Look-ahead: panel k+1 needs only the first block column of panel k's trailing update.  That part runs on
     // the factor's stream; the rest of the update runs on an auxiliary stream beside the next panel kernel
     // (whose 64-step dependent chain leaves the machine almost empty).
     cudaStream_t aux = (p->ktiming || !p->fstream2 || getenv("SFFT_NO_LOOKAHEAD")) ? nullptr : p->fstream2;
     bool aux_busy = false;
+    const int inv_done = 0; // (inverting block kb on the auxiliary stream right after its panel delayed the look-ahead updates queued behind it)
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
         const int rem = n - k0 - bs, nt = (rem + CB - 1) / CB;
@@ -374,7 +421,7 @@ cudaError_t launch_factor(sfft_plan *p) {
         aux_busy = true;
     }
     if (aux_busy) cudaStreamWaitEvent(st, p->ev_lookB, 0);
-    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, 256, 2 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n); }
+    if (inv_done < nblk) { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk - inv_done, 256, 3 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n, inv_done); }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     return cudaGetLastError();
 }

@@ -186,8 +186,11 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
                                                      double *__restrict__ D, Geom g) {
     const int nx = g.nx, ny = g.ny, w = g.w, L = g.L, LL = L * L;
     const long long nA = 2LL * w * nx, nB = 2LL * w * (ny - 2 * w);
-    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= nA + nB) return;
+    // 4 adjacent lanes share a pixel (tap rows v = -w + part, step 4): the per-thread chain of dependent R loads is 4x shorter
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int part = (int)(gid & 3);
+    const bool live = (gid >> 2) < nA + nB;
+    const long long id = live ? (gid >> 2) : 0;
     int x, y;
     if (id < nA) { const int r = (int)(id / nx); x = (int)(id - (long long)r * nx); y = r < w ? r : ny - 2 * w + r; }
     else { const long long k = id - nA; const int r = (int)(k / (2 * w)), cidx = (int)(k - (long long)r * 2 * w); y = w + r; x = cidx < w ? cidx : nx - 2 * w + cidx; }
@@ -212,7 +215,7 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
                 if (d <= g.DK) k = fma(a[(size_t)t * LL], xp[d - j] * yp[j], k);
         return k * R[(size_t)ys * nx + xs];
     };
-    for (int v = -w; v <= w; v++) {
+    for (int v = -w + part; v <= w; v += 4) {
         const int ys = y - v;
         const bool oy = ys < 0 || ys >= ny;
         const int yN = ys < 0 ? ys + ny : (ys >= ny ? ys - ny : ys), yM = (ys + g.My) & (g.My - 1);
@@ -224,7 +227,9 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
             if (xM < nx && yM < ny) corr -= term(u, v, xM, yM);          // padded-grid wrap landed on a real pixel
         }
     }
-    D[(size_t)y * nx + x] -= corr;
+    corr += __shfl_xor_sync(0xffffffffu, corr, 1);
+    corr += __shfl_xor_sync(0xffffffffu, corr, 2);
+    if (live && part == 0) D[(size_t)y * nx + x] -= corr;
 }
 
 int col_cfg(const Geom &g, int *threads, size_t *smem); // sfft_fwd.cu
@@ -262,7 +267,7 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
     if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
         const long long nb = 2LL * g.w * g.nx + 2LL * g.w * (g.ny - 2 * g.w);
         KLaunch kl(p, "wrapfix");
-        wrapfix_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(R, coef, D, g);
+        wrapfix_kernel<<<(unsigned)((4 * nb + 127) / 128), 128, 0, st>>>(R, coef, D, g);
     }
     return cudaGetLastError();
 }
