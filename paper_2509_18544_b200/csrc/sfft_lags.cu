@@ -229,11 +229,12 @@ __global__ void __launch_bounds__(256) lagedge_kernel(SpecSet ss, PairList pl, i
 
 // ---------------------------------------------------------------- stage 2
 // grid = (np, 2W+1 [dv]); block 256.
+// WM: compile-time bound on W (5, 10, 20) -- sized for MAX_L the accumulators took 228 registers (one CTA per SM, three waves)
+template <int WM>
 __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q, int np, int W, int nsplit,
                                                     const double *__restrict__ bpart, int nchunk,
                                                     double *__restrict__ lag, Geom g, const cplx *__restrict__ tw) {
     const int p = blockIdx.x, dvi = blockIdx.y, Hx = g.Hx, Mx = g.Mx;
-    constexpr int WM = MAX_L - 1; // 20
     double sc[WM + 1], sn[WM + 1];
 #pragma unroll
     for (int d = 0; d <= WM; d++) { sc[d] = 0.0; sn[d] = 0.0; }
@@ -366,7 +367,13 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     else e = run_lagcol<20>(p, ss, ns, pl, W, c, science);
     if (e != cudaSuccess) return e;
     join_side(p);
-    { KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega"); lagrow_kernel<<<dim3(pl.np, 2 * W + 1), 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw); }
+    {
+        KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega");
+        const dim3 gr(pl.np, 2 * W + 1);
+        if (W <= 5) lagrow_kernel<5><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
+        else if (W <= 10) lagrow_kernel<10><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
+        else lagrow_kernel<MAX_L - 1><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
+    }
     return cudaGetLastError();
 }
 
