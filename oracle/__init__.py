@@ -10,6 +10,8 @@ from .sfft_oracle import (  # noqa: F401
     build,
     build_system,
     build_system_dense,
+    convolve_stamp,
+    convolve_stamp_at,
     coord,
     design_matrix,
     lag_sum,

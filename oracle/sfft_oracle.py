@@ -235,3 +235,43 @@ def system_entry(S, R, mask, L, DK, DB, row, col, work=None):
     if rc:
         raise OracleError(rc, "system_entry")
     return out.value
+
+
+# ---------------------------------------------------------------------------------------------------
+# f2 -- cross-convolution with a PSF stamp (pipeline step 5: "Cross-convolve the template
+# PSF with the science image, and the science PSF with the template").
+# The paper gives no formula; the operation is the textbook discrete convolution
+#     out(x, y) = sum_{u,v} stamp(u, v) * img((x - u) mod nx, (y - v) mod ny),   |u|, |v| <= w = (P-1)/2,
+# with the same boundary as the subtraction (reading C6: circular at the native nx x ny) and the same
+# tap layout as the kernel coefficients: stamp[(v + w) * P + (u + w)].  Plain numpy, FP64: one shifted
+# copy of the image per tap, summed in the order (v, u) ascending -- no FFT, no blocking.
+# ---------------------------------------------------------------------------------------------------
+def convolve_stamp(img, stamp):
+    img = np.ascontiguousarray(img, dtype=np.float64)
+    stamp = np.ascontiguousarray(stamp, dtype=np.float64)
+    P = stamp.shape[0]
+    if stamp.ndim != 2 or stamp.shape[1] != P or P % 2 != 1:
+        raise ValueError("stamp must be P x P with P odd")
+    w = (P - 1) // 2
+    out = np.zeros_like(img)
+    for v in range(-w, w + 1):
+        for u in range(-w, w + 1):
+            # np.roll(img, (v, u))[y, x] = img[(y - v) mod ny, (x - u) mod nx]
+            out += stamp[v + w, u + w] * np.roll(img, (v, u), axis=(0, 1))
+    return out
+
+
+def convolve_stamp_at(img, stamp, xs, ys):
+    """The same sum at sampled output pixels (for full-size frames), one pixel at a time."""
+    img = np.ascontiguousarray(img, dtype=np.float64)
+    stamp = np.ascontiguousarray(stamp, dtype=np.float64)
+    ny, nx = img.shape
+    P = stamp.shape[0]
+    w = (P - 1) // 2
+    offs = np.arange(-w, w + 1)
+    out = np.empty(len(xs))
+    for k, (x, y) in enumerate(zip(xs, ys)):
+        rows = (int(y) - offs) % ny          # v ascending
+        cols = (int(x) - offs) % nx          # u ascending
+        out[k] = float(np.sum(stamp * img[np.ix_(rows, cols)]))
+    return out

@@ -360,3 +360,65 @@ def test_config0_conditioning_and_fit_quality():
     # residual RMS ~ sqrt(sigma_S^2 + |K|^2 sigma_R^2), well below the star signal
     assert 4.0 < D.std() < 12.0
     assert abs(c[: 49].sum() - 1.0) < 0.1  # flux scaling of the constant kernel term ~ 1
+
+
+# ---------------------------------------------------------------- f2: cross-convolution with a PSF stamp
+def _stamp(P, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((P, P))            # deliberately asymmetric: a flipped or transposed tap layout fails
+
+
+def test_convolve_stamp_delta_and_shift():
+    """A unit tap at offset (u0, v0) moves the image by (+u0, +v0) with wrap-around (reading C6)."""
+    rng = np.random.default_rng(3)
+    img = rng.standard_normal((23, 31))
+    P, w = 7, 3
+    yy, xx = np.mgrid[:23, :31]
+    for u0, v0 in [(0, 0), (2, -3), (-1, 1), (3, 3)]:
+        st = np.zeros((P, P)); st[v0 + w, u0 + w] = 1.0
+        out = oracle.convolve_stamp(img, st)
+        assert np.array_equal(out, img[(yy - v0) % 23, (xx - u0) % 31])
+
+
+def test_convolve_stamp_against_scipy_and_fft():
+    """Two independent routes: scipy.ndimage.convolve(mode='wrap') and the convolution theorem with numpy FFTs."""
+    from scipy import ndimage
+    rng = np.random.default_rng(4)
+    ny, nx, P = 40, 52, 9
+    w = (P - 1) // 2
+    img = rng.standard_normal((ny, nx)) * 50 + 100
+    st = _stamp(P, 5)
+    out = oracle.convolve_stamp(img, st)
+    ref = ndimage.convolve(img, st, mode="wrap")
+    assert np.max(np.abs(out - ref)) <= 1e-11 * np.max(np.abs(ref))
+    emb = np.zeros((ny, nx))
+    for v in range(-w, w + 1):
+        for u in range(-w, w + 1):
+            emb[v % ny, u % nx] = st[v + w, u + w]
+    ref2 = np.fft.ifft2(np.fft.fft2(img) * np.fft.fft2(emb)).real
+    assert np.max(np.abs(out - ref2)) <= 1e-11 * np.max(np.abs(ref2))
+    # flux: sum(out) = sum(img) * sum(stamp)
+    assert abs(out.sum() - img.sum() * st.sum()) <= 1e-9 * abs(img).sum() * abs(st).sum()
+
+
+def test_convolve_stamp_is_the_model_term_of_the_subtraction_oracle():
+    """D = S - R (*) K - B of the C oracle with DK = DB = 0, S = 0, b = 0 gives -(R (*) K): the two oracles
+    (numpy shifts here, C loops there) must agree on the tap layout and the boundary."""
+    rng = np.random.default_rng(6)
+    ny, nx, P = 33, 29, 5
+    R = rng.standard_normal((ny, nx)) * 10 + 30
+    st = _stamp(P, 7)
+    c = np.concatenate([st.ravel(), [0.0]])
+    D = oracle.subtract(np.zeros((ny, nx)), R, P, 0, 0, c)
+    out = oracle.convolve_stamp(R, st)
+    assert np.max(np.abs(out + D)) <= 1e-12 * np.max(np.abs(out))
+
+
+def test_convolve_stamp_at_matches_full():
+    rng = np.random.default_rng(8)
+    img = rng.standard_normal((37, 41))
+    st = _stamp(7, 9)
+    full = oracle.convolve_stamp(img, st)
+    xs = np.array([0, 1, 40, 20, 3, 39]); ys = np.array([0, 36, 2, 18, 35, 36])
+    got = oracle.convolve_stamp_at(img, st, xs, ys)
+    assert np.max(np.abs(got - full[ys, xs])) <= 1e-12 * np.max(np.abs(full))
