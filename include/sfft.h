@@ -131,6 +131,20 @@ sfft_status sfft_set_template(sfft_plan *plan, const double *R, const uint8_t *m
 sfft_status sfft_subtract_batch(sfft_plan *plan, const double *const *S, int B,
                                 double *const *D, double *coeffs);
 
+/* ---- f2: cross-convolution with a PSF stamp (pipeline step 5: "Cross-convolve the
+ * template PSF with the science image, and the science PSF with the template") ---------- */
+
+/* out(x, y) = sum_{|u|,|v| <= w} stamp[(v + w) * L + (u + w)] * img((x - u) mod nx, (y - v) mod ny):
+ * the discrete convolution of img (device, ny*nx doubles, row-major) with an L x L stamp (device, L*L
+ * doubles, same tap layout as the kernel coefficients; L, w = (L-1)/2 are the plan's), circular at the
+ * native nx x ny like the subtraction (reading C6).  out: device, ny*nx doubles, must not alias img.
+ * Runs the a1 transforms of img, the a5 K^ synthesis / inverse transforms and the border wrap
+ * correction; uses the plan's science-spectrum and intermediate buffers as scratch: call it BEFORE
+ * sfft_build_system / sfft_set_template or after sfft_subtract, not between them (no state check is
+ * made).  The plan's DK, DB are irrelevant.  Asynchronous on the plan's stream.
+ * Errors: INVALID_ARG (NULL or aliased pointers), CUDA. */
+sfft_status sfft_convolve_stamp(sfft_plan *plan, const double *img, const double *stamp, double *out);
+
 /* ---- host-buffer convenience (the end-to-end call bench.py times as `e2e`) ---------- */
 
 /* Whole single-pair path from HOST buffers: copies S, R (and mask, may be NULL) to plan-owned

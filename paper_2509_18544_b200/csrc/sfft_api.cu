@@ -366,6 +366,26 @@ sfft_status sfft_subtract_with(sfft_plan *p, const double *S, const double *coef
     return SFFT_OK;
 }
 
+// f2: out = img (*) stamp, circular at the native grid, through the a1/a5 kernels:
+// row + column transform of the unweighted image into the science-spectrum buffer, K^ synthesised from the L x L
+// taps, inverse transforms, wrap correction of the border pixels.  Geom is passed to kernels by value, so one
+// spectrum / no background is a temporary NK = 1, NB = 0, DK = 0 view of the plan's geometry.
+sfft_status sfft_convolve_stamp(sfft_plan *p, const double *img, const double *stamp, double *out) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!img || !stamp || !out) return fail(p, SFFT_ERR_INVALID_ARG, "convolve_stamp: NULL pointer");
+    if (img == out) return fail(p, SFFT_ERR_INVALID_ARG, "convolve_stamp: in-place operation is not supported");
+    back_to_main(p);
+    const Geom saved = p->g;
+    p->g.NK = 1; p->g.NB = 0; p->g.DK = 0; p->g.DB = 0;
+    const int i0 = 0, j0 = 0;
+    cudaError_t e = launch_row_fwd(p, img, nullptr, p->inter, 1, nullptr, 0);
+    if (e == cudaSuccess) e = launch_col_fwd(p, p->inter, p->specS, 1, &i0, &j0);
+    if (e == cudaSuccess) e = launch_subtract(p, nullptr, img, stamp, out, p->specS, 1);
+    p->g = saved;
+    CK(e, "convolve_stamp");
+    return SFFT_OK;
+}
+
 sfft_status sfft_set_template(sfft_plan *p, const double *R, const uint8_t *mask) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (!R) return fail(p, SFFT_ERR_INVALID_ARG, "set_template: NULL image");

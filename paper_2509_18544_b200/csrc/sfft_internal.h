@@ -135,7 +135,10 @@ cudaError_t launch_factor(sfft_plan *p);                      // G -> dscale, Lf
 cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c); // c = D (L^-T (L^-1 (D h)))
 
 // ---- a5 (sfft_subtract.cu) ---------------------------------------------------------------
-cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D);
+// spec: the NK spectra to convolve (default: the plan's unmasked template spectra); mode 0: D = S - M - B,
+// mode 1 (f2, sfft_convolve_stamp): D = +M, S unused
+cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D,
+                            const cplx *spec = nullptr, int mode = 0);
 
 // ---- probes (sfft_probe.cu) -------------------------------------------------------------------
 cudaError_t run_probe_fp64(int kind, int iters, double *tflops);

@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(512) col_inv_kernel(const cplx *__restrict__ s
 template <int E, int LOG2N_CT = 0>
 __global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S,
                                                      const double *__restrict__ coef, double *__restrict__ D, Geom g,
-                                                     const cplx *__restrict__ tw) {
+                                                     const cplx *__restrict__ tw, int mode) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int Hx = LOG2N_CT ? (1 << LOG2N_CT) : g.Hx, T = Hx / E;
     const int RPB = LOG2N_CT ? 1 : blockDim.x / T;
@@ -158,7 +158,8 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_inv_kernel(const cpl
             for (int p = 0; p <= MAX_DEG; p++) if (g.pi[sI] == p) cx[p] = fma(b[sI], yp, cx[p]);
         }
     }
-    const double scale = 1.0 / ((double)Hx * (double)g.My), inx = 1.0 / (double)g.nx;
+    // mode 1 (plain convolution, f2): D = +M; the science image is not read and there is no background (NB = 0)
+    const double scale = (mode ? -1.0 : 1.0) / ((double)Hx * (double)g.My), inx = 1.0 / (double)g.nx;
     const size_t ro = (size_t)row * g.nx;
     const bool vec = ((g.nx & 1) == 0) && (((size_t)S | (size_t)D) & 15) == 0;
 #pragma unroll
@@ -169,12 +170,12 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_inv_kernel(const cpl
         const double ba = fma(fma(fma(cx[3], xa, cx[2]), xa, cx[1]), xa, cx[0]);
         const double bb = fma(fma(fma(cx[3], xb, cx[2]), xb, cx[1]), xb, cx[0]);
         if (vec) {
-            const double2 sv = *reinterpret_cast<const double2 *>(S + ro + x0);
+            const double2 sv = mode ? make_double2(0.0, 0.0) : *reinterpret_cast<const double2 *>(S + ro + x0);
             double2 o; o.x = sv.x - scale * v[q].x - ba; o.y = sv.y - scale * v[q].y - bb;
             *reinterpret_cast<double2 *>(D + ro + x0) = o;
         } else {
-            D[ro + x0] = S[ro + x0] - scale * v[q].x - ba;
-            if (x0 + 1 < g.nx) D[ro + x0 + 1] = S[ro + x0 + 1] - scale * v[q].y - bb;
+            D[ro + x0] = (mode ? 0.0 : S[ro + x0]) - scale * v[q].x - ba;
+            if (x0 + 1 < g.nx) D[ro + x0 + 1] = (mode ? 0.0 : S[ro + x0 + 1]) - scale * v[q].y - bb;
         }
     }
 }
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(256, E == 16 ? 2 : 4) row_inv_kernel(const cpl
 // (x-u, y-v) leaves the frame, the padded-grid FFT used Rpad((x-u) mod Mx, (y-v) mod My) (zero in
 // the padding) where the method wants R((x-u) mod nx, (y-v) mod ny): subtract the difference.
 __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__ R, const double *__restrict__ coef,
-                                                     double *__restrict__ D, Geom g) {
+                                                     double *__restrict__ D, Geom g, int mode) {
     const int nx = g.nx, ny = g.ny, w = g.w, L = g.L, LL = L * L;
     const long long nA = 2LL * w * nx, nB = 2LL * w * (ny - 2 * w);
     // 4 adjacent lanes share a pixel (tap rows v = -w + part, step 4): the per-thread chain of dependent R loads is 4x shorter
@@ -229,15 +230,17 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
     }
     corr += __shfl_xor_sync(0xffffffffu, corr, 1);
     corr += __shfl_xor_sync(0xffffffffu, corr, 2);
-    if (live && part == 0) D[(size_t)y * nx + x] -= corr;
+    if (live && part == 0) D[(size_t)y * nx + x] -= mode ? -corr : corr;
 }
 
 int col_cfg(const Geom &g, int *threads, size_t *smem); // sfft_fwd.cu
 int row_cfg(const Geom &g, int E, int *threads, size_t *smem);
 int fft_E(const char *env, int N, int dflt);
 
-cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D) {
+cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D,
+                            const cplx *spec, int mode) {
     const Geom &g = p->g;
+    if (!spec) spec = p->specTo;
     cudaStream_t st = p->stream;
     const bool pipe = colpipe_ok(g);
     if (!pipe) { KLaunch kl(p, "ktab"); ktab_kernel<<<dim3((g.Hx + 1 + 127) / 128, g.w + 1, g.NK), 128, 0, st>>>(coef, p->E, g, p->tw); }
@@ -253,21 +256,21 @@ cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, cons
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    if (pipe) { cudaError_t e = launch_colpipe_inv(p, p->specTo, coef, p->inter); if (e != cudaSuccess) return e; }
-    else { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(p->specTo, p->E, p->inter, C, g, p->tw); }
+    if (pipe) { cudaError_t e = launch_colpipe_inv(p, spec, coef, p->inter); if (e != cudaSuccess) return e; }
+    else { KLaunch kl(p, "col_inv"); col_inv_kernel<<<g.Hx / C, threads, smem, st>>>(spec, p->E, p->inter, C, g, p->tw); }
     const int ER = fft_E("SFFT_ROW_E", g.Hx, 8);
     int rthreads; size_t rsmem;
     const int RPB = row_cfg(g, ER, &rthreads, &rsmem);
     {
         KLaunch kl(p, "row_inv");
-        if (ER == 8 && g.log2Hx == 11 && RPB == 1) row_inv_kernel<8, 11><<<g.ny, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
-        else if (ER == 8) row_inv_kernel<8><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
-        else row_inv_kernel<16><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw);
+        if (ER == 8 && g.log2Hx == 11 && RPB == 1) row_inv_kernel<8, 11><<<g.ny, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw, mode);
+        else if (ER == 8) row_inv_kernel<8><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw, mode);
+        else row_inv_kernel<16><<<(g.ny + RPB - 1) / RPB, rthreads, rsmem, st>>>(p->inter, S, coef, D, g, p->tw, mode);
     }
     if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
         const long long nb = 2LL * g.w * g.nx + 2LL * g.w * (g.ny - 2 * g.w);
         KLaunch kl(p, "wrapfix");
-        wrapfix_kernel<<<(unsigned)((4 * nb + 127) / 128), 128, 0, st>>>(R, coef, D, g);
+        wrapfix_kernel<<<(unsigned)((4 * nb + 127) / 128), 128, 0, st>>>(R, coef, D, g, mode);
     }
     return cudaGetLastError();
 }

@@ -23,7 +23,7 @@ _STATUS = {0: "OK", -1: "INVALID_ARG", -2: "ALLOC", -3: "CUDA", -4: "STATE", -5:
 SYMBOLS = (
     "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
     "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_with",
-    "sfft_set_template", "sfft_subtract_batch", "sfft_difference_host", "sfft_sync_status",
+    "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_difference_host", "sfft_sync_status",
     "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
     "sfft_kernel_timing_get", "sfft_launch_count",
     "sfft_last_error", "sfft_version", "sfft_debug_read", "sfft_probe_fp64",
@@ -59,6 +59,7 @@ def load_library():
     lib.sfft_solve.argtypes = [vp]
     lib.sfft_subtract.argtypes = [vp, dp, dp]
     lib.sfft_subtract_with.argtypes = [vp, dp, dp, dp]
+    lib.sfft_convolve_stamp.argtypes = [vp, dp, dp, dp]
     lib.sfft_set_template.argtypes = [vp, dp, dp]
     lib.sfft_subtract_batch.argtypes = [vp, ctypes.POINTER(vp), ci, ctypes.POINTER(vp), dp]
     lib.sfft_difference_host.argtypes = [vp, dp, dp, dp, dp, dp]
@@ -181,6 +182,20 @@ class SfftPlan:
         self._ck(self._lib.sfft_subtract_with(self._h, sp, _dev_f64(coeffs_in, (self.n,), "coeffs_in"),
                                               _dev_f64(D, self.shape, "D")), "sfft_subtract_with")
         return D
+
+    # -- f2: cross-convolution with a PSF stamp --------------------------------
+    def convolve_stamp(self, img, stamp, out=None):
+        """out = img (*) stamp (L x L taps, circular at the native grid); see sfft_convolve_stamp in include/sfft.h."""
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        self._ck(self._lib.sfft_convolve_stamp(self._h, _dev_f64(img, self.shape, "img"),
+                                               _dev_f64(stamp, (self.L, self.L), "stamp"),
+                                               _dev_f64(out, self.shape, "out")), "sfft_convolve_stamp")
+        return out
+
+    def cross_convolve(self, S, R, psf_S, psf_R):
+        """Pipeline step 5: (S (*) psf_R, R (*) psf_S)."""
+        return self.convolve_stamp(S, psf_R), self.convolve_stamp(R, psf_S)
 
     # -- batched --------------------------------------------------------------------------
     def set_template(self, R, mask=None):

@@ -120,3 +120,27 @@ def test_config4_large_kernel():
     sampled_D_check(S, R, L, DK, DB, c, D, rng, cfg["noise_rms"], nsamp=300)
     assert normal_equation_residual(S, R, L, DK, DB, D) <= 1e-12
     p.destroy()
+
+
+def test_cross_convolution_at_4088_sampled():
+    """f2 at the full Roman frame in the configuration bench.py times: S (*) psf_R and R (*) psf_S
+    with 11 x 11 stamps, compared on sampled pixels (border, corners and interior) the oracle computes one by one,
+    plus the flux invariant sum(out) = sum(img) sum(stamp) over the whole frame."""
+    from test_gpu_parity import TOL_CONV, _psf_stamp
+    cfg = starfield.make_pair(2)
+    S, R = cfg["S"], cfg["R"]
+    ny, nx = S.shape
+    P, w = 11, 5
+    psfS, psfR = _psf_stamp(P, 21, 1.0), _psf_stamp(P, 22, 0.85)
+    p = SfftPlan(nx, ny, P, 2, 2)
+    Sc, Rc = p.cross_convolve(dev(S), dev(R), dev(psfS), dev(psfR))
+    Sc, Rc = Sc.cpu().numpy(), Rc.cpu().numpy()
+    rng = np.random.default_rng(17)
+    xs = rng.integers(0, nx, 600); ys = rng.integers(0, ny, 600)
+    xs[:8] = [0, nx - 1, 0, nx - 1, w - 1, nx - w, nx // 2, 3]
+    ys[:8] = [0, 0, ny - 1, ny - 1, ny // 2, 5, ny - 1, w]
+    for img, st, out in ((S, psfR, Sc), (R, psfS, Rc)):
+        ref = oracle.convolve_stamp_at(img, st, xs, ys)
+        assert np.max(np.abs(out[ys, xs] - ref)) <= TOL_CONV * np.max(np.abs(img)) * np.abs(st).sum()
+        assert abs(out.sum() - img.sum() * st.sum()) <= 1e-10 * np.abs(img).sum() * np.abs(st).sum()
+    p.destroy()

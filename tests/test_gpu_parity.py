@@ -229,3 +229,73 @@ def test_difference_host_matches_device_path():
     p, G, h, cd, D = run_gpu(c["S"], c["R"], None, c["L"], c["DK"], c["DB"])
     Dh, ch = p.difference_host(torch.from_numpy(c["S"]).pin_memory(), torch.from_numpy(c["R"]).pin_memory())
     assert np.array_equal(Dh.numpy(), D) and np.array_equal(ch.numpy(), cd)
+
+
+# ---------------------------------------------------------------- f2: cross-convolution with a PSF stamp
+# Bar: |out_gpu - out_oracle| <= 1e-11 * max|img| * sum|stamp| everywhere.  The FFT route's rounding error is
+# ~ log2(Mx My) * 2^-53 * max|img| * sum|stamp| ~ 3e-15 of that product, so the bar has three
+# orders of margin and still catches a wrong tap, a flipped stamp or a missed border correction (errors ~ 1e-2).
+TOL_CONV = 1e-11
+
+
+def _psf_stamp(P, seed, sigma=1.3):
+    """A normalised, deliberately off-centre and asymmetric PSF-like stamp."""
+    rng = np.random.default_rng(seed)
+    w = (P - 1) // 2
+    yy, xx = np.mgrid[-w:w + 1, -w:w + 1]
+    st = np.exp(-0.5 * (((xx - 0.3) / sigma) ** 2 + ((yy + 0.2) / (1.4 * sigma)) ** 2)) + 0.01 * rng.random((P, P))
+    return st / st.sum()
+
+
+@pytest.mark.parametrize("nx,ny,P,DK,DB", [
+    (128, 64, 5, 0, 0),      # powers of two: no padding, no border correction
+    (100, 72, 7, 2, 1),      # zero padding + native-grid wrap correction; a plan whose DK, DB are not 0
+    (61, 67, 3, 1, 0),       # odd sizes
+    (90, 130, 1, 0, 0),      # a single tap
+    (600, 520, 11, 0, 0),    # the pipelined column kernels (My = 1024)
+    (72, 4000, 5, 0, 0),     # the My = 4096 instances
+])
+def test_convolve_stamp_parity(nx, ny, P, DK, DB):
+    S, R = starfield.random_pair(nx, ny, seed=nx + 3 * ny)
+    st = _psf_stamp(P, seed=P) if P > 1 else np.array([[0.7]])
+    p = SfftPlan(nx, ny, P, DK, DB)
+    out = p.convolve_stamp(dev(R), dev(st)).cpu().numpy()
+    ref = oracle.convolve_stamp(R, st)
+    assert np.max(np.abs(out - ref)) <= TOL_CONV * np.max(np.abs(R)) * np.abs(st).sum()
+    p.destroy()
+
+
+def test_cross_convolve_then_subtract_on_one_plan():
+    """Pipeline order: cross-convolve both images, then run the SFFT subtraction on the
+    cross-convolved pair with the SAME plan: the convolution must not disturb the plan's state."""
+    nx, ny, L = 100, 72, 5
+    S, R = starfield.random_pair(nx, ny, seed=11)
+    psfS, psfR = _psf_stamp(L, 1, 1.1), _psf_stamp(L, 2, 0.9)
+    p = SfftPlan(nx, ny, L, 1, 1)
+    Sc, Rc = p.cross_convolve(dev(S), dev(R), dev(psfS), dev(psfR))
+    Sc0, Rc0 = oracle.convolve_stamp(S, psfR), oracle.convolve_stamp(R, psfS)
+    assert np.max(np.abs(Sc.cpu().numpy() - Sc0)) <= TOL_CONV * np.max(np.abs(S)) * np.abs(psfR).sum()
+    assert np.max(np.abs(Rc.cpu().numpy() - Rc0)) <= TOL_CONV * np.max(np.abs(R)) * np.abs(psfS).sum()
+    p.build_system(Sc, Rc)
+    G, h = p.get_system()
+    p.solve()
+    D, c = p.subtract()
+    p.sync_status()
+    G0, h0 = oracle.build_system(Sc0, Rc0, None, L, 1, 1)
+    assert_system(G.cpu().numpy(), h.cpu().numpy(), G0, h0, Sc0)
+    c0 = oracle.solve(G0, h0)
+    assert_coeffs(c.cpu().numpy(), c0, L * L * 3)
+    D0 = oracle.subtract(Sc0, Rc0, L, 1, 1, c0)
+    assert np.max(np.abs(D.cpu().numpy() - D0)) <= TOL_D * 20.0
+    p.destroy()
+
+
+def test_convolve_stamp_argument_errors():
+    p = SfftPlan(64, 64, 3, 0, 0)
+    img = torch.zeros((64, 64), dtype=torch.float64, device="cuda")
+    st = torch.zeros((3, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(SfftError):
+        p.convolve_stamp(img, st, out=img)          # aliased
+    with pytest.raises(ValueError):
+        p.convolve_stamp(img, torch.zeros((5, 5), dtype=torch.float64, device="cuda"))
+    p.destroy()
