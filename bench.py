@@ -14,7 +14,8 @@ independent problem on its own GPU, no data-path collective; value = N / max-ove
 Extra objects on the JSON line: `roofline` (dominant kernel, timed live with CUDA events through
 the library's per-launch timers on the plan's stream), `path_roofline` (the metric's "% of HBM
 roofline": 34 r of algorithmic bytes over the a1+a2+a3+a5 time), `stages_ms`, `kernels_ms`,
-`batched` (configs[3]: template-side work once, per-science-image throughput), `cpu_baseline`
+`batched` (configs[3]: template-side work once, per-science-image throughput), `cross_convolve`
+(f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `cpu_baseline`
 (the oracle on this box's host cores, bounded sample), `clocks`.
 
 --impl reference times the CPU oracle (oracle/, as it stands) on the same config and metric.
@@ -388,6 +389,48 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
         out["fp64_probe_tflops"] = {"dfma": round(sfft.probe_fp64(0), 2), "dmma_m8n8k4": round(sfft.probe_fp64(1), 2)}
     except Exception as e:  # pragma: no cover
         out["fp64_probe_tflops"] = {"error": str(e)}
+
+    # f2: cross-convolution S (*) psf_R, R (*) psf_S with L x L stamps on the same plan.
+    # Algorithmic bytes per convolution: image 1 r + row intermediate 1 r written and read + spectrum 1 r written and
+    # read + inverse intermediate 1 r written and read + output 1 r = 8 r.  The oracle is timed on a bounded crop.
+    try:
+        import oracle
+        import time as _time
+        L = cfg["L"]
+        w = (L - 1) // 2
+        yy, xx = np.mgrid[-w:w + 1, -w:w + 1]
+        psfs = []
+        for sg in (1.0, 0.85):
+            st = np.exp(-0.5 * (xx * xx + yy * yy) / (sg * sg)); psfs.append(st / st.sum())
+        dpS, dpR = (torch.from_numpy(a).cuda() for a in psfs)
+        oS, oR = torch.empty_like(dS), torch.empty_like(dR)
+        stream = torch.cuda.current_stream()
+        for _ in range(3):
+            plan.convolve_stamp(dS, dpR, oS); plan.convolve_stamp(dR, dpS, oR)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            plan.convolve_stamp(dS, dpR, oS); plan.convolve_stamp(dR, dpS, oR)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / K
+        crop = 1022 if ny >= 1022 and nx >= 1022 else min(nx, ny)
+        t0 = _time.perf_counter()
+        ref = oracle.convolve_stamp(pair["S"][:crop, :crop], psfs[1])
+        t_cpu = _time.perf_counter() - t0
+        got = oS[:crop - w, :crop - w].cpu().numpy()[w:, w:]          # interior of the crop: same taps on both sides
+        err = float(np.max(np.abs(got - ref[w:crop - w, w:crop - w])))
+        r = nx * ny * 8.0
+        out["cross_convolve"] = {"workload": f"S (*) psf_R and R (*) psf_S, {L} x {L} stamps, {nx} x {ny} (PAPER.md:86)",
+                                 "ms": round(ms, 4), "pairs_per_s": round(1e3 / ms, 1),
+                                 "algorithmic_bytes": 16 * r, "achieved_gbs": round(16 * r / ms / 1e6, 1),
+                                 "frac_of_measured_hbm": round(16 * r / ms / 1e6 / peak, 4),
+                                 "oracle_check_max_abs_err": err,
+                                 "cpu_oracle": {"seconds_sample": round(t_cpu, 3), "sample": f"one convolution of the top-left {crop} x {crop} crop",
+                                                "pairs_per_s_full_frame_est": round(1.0 / (2 * t_cpu * (nx * ny) / (crop * crop)), 4)}}
+    except Exception as ex:  # pragma: no cover
+        out["cross_convolve"] = {"error": str(ex)}
 
     # batched variant (BASELINE.json configs[3]): template once, B science images
     B = args.batch
