@@ -15,7 +15,8 @@ Extra objects on the JSON line: `roofline` (dominant kernel, timed live with CUD
 the library's per-launch timers on the plan's stream), `path_roofline` (the metric's "% of HBM
 roofline": 34 r of algorithmic bytes over the a1+a2+a3+a5 time), `stages_ms`, `kernels_ms`,
 `batched` (configs[3]: template-side work once, per-science-image throughput), `cross_convolve`
-(f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `cpu_baseline`
+(f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `stamp_mode`
+(f4: the path on a 1000 x 1000 cut-out), `cpu_baseline`
 (the oracle on this box's host cores, bounded sample), `clocks`.
 
 --impl reference times the CPU oracle (oracle/, as it stands) on the same config and metric.
@@ -431,6 +432,36 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
                                                 "pairs_per_s_full_frame_est": round(1.0 / (2 * t_cpu * (nx * ny) / (crop * crop)), 4)}}
     except Exception as ex:  # pragma: no cover
         out["cross_convolve"] = {"error": str(ex)}
+
+    # f4: "decrease the processed stamp size ... down to a minimum size of 1000 x 1000 px": the same path
+    # on a contiguous 1000 x 1000 cut-out of the pair (a second, small plan; same L, DK, DB).
+    try:
+        from paper_2509_18544_b200 import SfftPlan as _Plan
+        sn = 1000
+        y0, x0 = (ny - sn) // 2, (nx - sn) // 2
+        cS, cR = dS[y0:y0 + sn, x0:x0 + sn].contiguous(), dR[y0:y0 + sn, x0:x0 + sn].contiguous()
+        sp = _Plan(sn, sn, cfg["L"], cfg["DK"], cfg["DB"])
+        cD = torch.empty_like(cS); cc = torch.empty(sp.n, dtype=torch.float64, device="cuda")
+        def sstep():
+            sp.build_system(cS, cR); sp.solve(); sp.subtract(cD, cc)
+        for _ in range(3):
+            sstep()
+        sp.sync_status()
+        stream = torch.cuda.current_stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            sstep()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        sp.sync_status()
+        sms = e0.elapsed_time(e1) / K
+        out["stamp_mode"] = {"workload": f"{sn} x {sn} cut-out of the same pair, L={cfg['L']}, DK={cfg['DK']}, DB={cfg['DB']} (PAPER.md:105)",
+                             "ms_per_step": round(sms, 4), "stamps_per_s": round(1e3 / sms, 1),
+                             "workspace_gb": round(sp.workspace_bytes / 1e9, 3)}
+        sp.destroy()
+    except Exception as ex:  # pragma: no cover
+        out["stamp_mode"] = {"error": str(ex)}
 
     # batched variant (BASELINE.json configs[3]): template once, B science images
     B = args.batch

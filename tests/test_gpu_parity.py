@@ -299,3 +299,10 @@ def test_convolve_stamp_argument_errors():
     with pytest.raises(ValueError):
         p.convolve_stamp(img, torch.zeros((5, 5), dtype=torch.float64, device="cuda"))
     p.destroy()
+
+
+def test_stamp_mode_1000_cutout():
+    """f4: the path on a 1000 x 1000 stamp ("minimum size of 1000 x 1000 px") with the configs[2]
+    recipe, L = 11, DK = 2, DB = 2: 1000 pads to 1024 (wrap corrections on), n = 732, full element-wise parity."""
+    c = starfield.make_pair(2, nx=1000, ny=1000, n_stars=3600)
+    full_parity(c["S"], c["R"], None, 11, 2, 2, c["noise_rms"])
