@@ -116,8 +116,49 @@ __device__ __forceinline__ void panel_chunk(double (&xr)[16], const double *rd, 
     }
 }
 
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b);
+
+// U = A B^T for two 64 x 64 shared-memory tiles (leading dimension CLD) on the FP64 tensor pipe, written to
+// out[r][c]; 8 warps, warp tile 16 x 32 (the same fragment layout as syrk_kernel).
+__device__ __forceinline__ void tile_abt(const double (*As)[CLD], const double (*Bs)[CLD], double (*out)[CB + 1], int tid) {
+    const int warp = tid >> 5, lane = tid & 31;
+    const int rw = (warp >> 1) * 16, cw = (warp & 1) * 32;
+    const int fr = lane >> 2, fk = lane & 3;
+    double acc[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int b = 0; b < 4; b++) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
+#pragma unroll 4
+    for (int kk = 0; kk < CB; kk += 4) {
+        double af[2], bf[4];
+#pragma unroll
+        for (int a = 0; a < 2; a++) af[a] = As[rw + 8 * a + fr][kk + fk];
+#pragma unroll
+        for (int b = 0; b < 4; b++) bf[b] = Bs[cw + 8 * b + fr][kk + fk];
+#pragma unroll
+        for (int a = 0; a < 2; a++)
+#pragma unroll
+            for (int b = 0; b < 4; b++) dmma884(acc[a][b][0], acc[a][b][1], af[a], bf[b]);
+    }
+#pragma unroll
+    for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int b = 0; b < 4; b++) {
+            out[rw + 8 * a + fr][cw + 8 * b + 2 * fk] = acc[a][b][0];
+            out[rw + 8 * a + fr][cw + 8 * b + 2 * fk + 1] = acc[a][b][1];
+        }
+}
+
+// FUSED look-ahead (k0 > 0): the update of block column k0 by the previous panel (columns k0-64..k0-1) is applied here,
+// in registers, instead of by a separate trailing-update launch on the critical path: every CTA forms
+// U_dd = X_d X_d^T (X_d: the previous panel's rows of this diagonal block) and U_bd = X_b X_d^T for its own rows
+// with DMMA and subtracts them from the tiles it has just loaded.  The trailing-update kernel then only covers
+// block columns >= k0 + 64 and runs beside this kernel (launch_factor).
+// dynamic smem: 2 * 64 * CLD doubles (X_b, X_d).
 __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
                                                          int bs, int *flag) {
+    extern __shared__ __align__(16) double psm[];
     __shared__ double l[CPAD][CB + 1];
     __shared__ double col[2][CPAD];
     __shared__ double rd[CB];
@@ -132,6 +173,42 @@ __global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ L
         if (r < bs && c < bs) v = (c <= r) ? Lf[(size_t)(k0 + r) * n + k0 + c] : 0.0;
         areg[q] = v;
         xr[q] = (have_rows && r0 + r < n && c < bs) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
+    }
+    if (k0 > 0) {
+        double (*Xb)[CLD] = reinterpret_cast<double (*)[CLD]>(psm);
+        double (*Xd)[CLD] = reinterpret_cast<double (*)[CLD]>(psm + CB * CLD);
+        const int kp = k0 - CB; // the previous panel is always a full block
+        double td[16], tb[16]; // all 32 loads in flight before the first store (one global round trip, not sixteen)
+#pragma unroll
+        for (int i = 0; i < 16; i++) {
+            const int e = tid + 256 * i, rr = e >> 6, cc = e & 63;
+            td[i] = (k0 + rr < n) ? Lf[(size_t)(k0 + rr) * n + kp + cc] : 0.0;
+            tb[i] = (have_rows && r0 + rr < n) ? Lf[(size_t)(r0 + rr) * n + kp + cc] : 0.0;
+        }
+#pragma unroll
+        for (int i = 0; i < 16; i++) {
+            const int e = tid + 256 * i, rr = e >> 6, cc = e & 63;
+            Xd[rr][cc] = td[i]; Xb[rr][cc] = tb[i];
+        }
+        __syncthreads();
+        tile_abt(Xd, Xd, l, tid);
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; q++) {
+            const int c = 4 * q + cq;
+            if (r < bs && c < bs && c <= r) areg[q] -= l[r][c];
+        }
+        __syncthreads();
+        if (have_rows) {
+            tile_abt(Xb, Xd, l, tid);
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < 16; q++) {
+                const int c = 4 * q + cq;
+                if (r0 + r < n && c < bs) xr[q] -= l[r][c];
+            }
+        }
+        __syncthreads();
     }
     if (tid < 2 * CPAD) col[tid / CPAD][tid % CPAD] = 0.0;       // dead-slot reads must see numbers (0 * NaN would not matter, but keep it clean)
     for (int e = tid; e < (CPAD - CB) * (CB + 1); e += 256) l[CB + e / (CB + 1)][e % (CB + 1)] = 0.0;
@@ -395,25 +472,29 @@ cudaError_t launch_factor(sfft_plan *p) {
     const size_t sm_syrk = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
     cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * CB * (CB + 1) * sizeof(double)));
-    // Look-ahead: panel k+1 needs only the first block column of panel k's trailing update.  That part runs on
-    // the factor's stream; the rest of the update runs on an auxiliary stream beside the next panel kernel
-    // (whose 64-step dependent chain leaves the machine almost empty).
+    // Look-ahead: panel k+1 needs only the first block column of panel k's trailing update.  That part is fused into
+    // the panel kernel of k+1; the rest of the update runs on an auxiliary stream beside it.
     cudaStream_t aux = (p->ktiming || !p->fstream2 || getenv("SFFT_NO_LOOKAHEAD")) ? nullptr : p->fstream2;
     bool aux_busy = false;
     const int inv_done = 0; // (inverting block kb on the auxiliary stream right after its panel delayed the look-ahead updates queued behind it)
+    const size_t sm_panel = 2 * CB * CLD * sizeof(double);
+    cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_panel);
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
         const int rem = n - k0 - bs, nt = (rem + CB - 1) / CB;
-        { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, 0, st>>>(p->Lf, p->Linv + (size_t)kb * CB * CB, n, k0, bs, p->flag); }
+        // panel kb, with the update of its block column by panel kb-1 fused in (potrf_panel_kernel).  It reads tiles the
+        // rest-update of panel kb-2 (auxiliary stream) also wrote: the wait for that update was enqueued in iteration kb-1.
+        { KLaunch kl(p, "potrf_panel"); potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, sm_panel, st>>>(p->Lf, p->Linv + (size_t)kb * CB * CB, n, k0, bs, p->flag); }
         if (rem <= 0) continue;
-        if (!aux || nt < 2) {
-            if (aux_busy) { cudaStreamWaitEvent(st, p->ev_lookB, 0); aux_busy = false; }
-            KLaunch kl(p, "syrk"); syrk_kernel<<<nt * (nt + 1) / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs, 0);
+        if (aux_busy) cudaStreamWaitEvent(st, p->ev_lookB, 0);              // panel kb+1 needs the rest-update of panel kb-1
+        if (nt < 2) continue;                   // a single block column left: its update is the next panel's fused prologue
+        // rest of the trailing update (block columns >= kb+2): beside the next panel kernel, whose 64-step dependent
+        // chain leaves the machine almost empty
+        if (!aux) {
+            KLaunch kl(p, "syrk"); syrk_kernel<<<(nt - 1) * nt / 2, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs, 2);
             continue;
         }
-        cudaEventRecord(p->ev_lookP, st);                                   // panel k is in place
-        if (aux_busy) cudaStreamWaitEvent(st, p->ev_lookB, 0);              // the previous rest-update touched these tiles too
-        { KLaunch kl(p, "syrk"); syrk_kernel<<<nt, 256, sm_syrk, st>>>(p->Lf, n, k0, bs, k0 + bs, 1); }
+        cudaEventRecord(p->ev_lookP, st);                                   // panel kb is in place
         cudaStreamWaitEvent(aux, p->ev_lookP, 0);
         syrk_kernel<<<(nt - 1) * nt / 2, 256, sm_syrk, aux>>>(p->Lf, n, k0, bs, k0 + bs, 2);
         p->launches++;
