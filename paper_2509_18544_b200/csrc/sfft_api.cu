@@ -74,7 +74,7 @@ static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
                     p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
-                    p->ywork, p->zwork, p->sflags, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->ywork, p->zwork, p->sflags, p->coef, p->h2, p->coef2, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     if (p->flag_host) cudaFreeHost(p->flag_host);
     for (int s = 0; s < SFFT_NUM_STAGES; s++) {
@@ -165,6 +165,8 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->zwork, n);
     AL(p->sflags, 2 * ((n + 63) / 64));
     AL(p->coef, n);
+    AL(p->h2, n);
+    AL(p->coef2, n);
     AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
     AL(p->flag, 1);
 #undef AL
@@ -407,6 +409,43 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
     if (!p->have_template || !p->have_factor) return fail(p, SFFT_ERR_STATE, "subtract_batch before set_template");
     if (!S || !D || B < 1) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: bad arguments");
     for (int b = 0; b < B; b++) if (!S[b] || !D[b]) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: NULL image");
+    if (B > 1 && !p->timing && !p->ktiming && p->fstream && !getenv("SFFT_NO_BATCH_PIPE")) {
+        // Software pipeline over the batch: the triangular solves of image b (86 us of latency-bound launches that leave
+        // the machine empty) run on the factor stream beside the science-side kernels of image b+1; order on the main
+        // stream: sci(0), [sci(1), a5(0)], [sci(2), a5(1)], ...  h and the coefficients are double-buffered; solve(b+2)
+        // starts after sci(b+2), which is behind a5(b) on the main stream, so no buffer is overwritten while in use.
+        double *hb[2] = {p->h, p->h2}, *cb[2] = {p->coef, p->coef2};
+        sfft_status rc = SFFT_OK;
+        p->S = S[0]; p->h = hb[0];
+        rc = science_side(p);
+        if (rc == SFFT_OK) CK(cudaEventRecord(p->ev_ffork, p->stream), "event");
+        for (int b = 0; b < B && rc == SFFT_OK; b++) {
+            cudaStreamWaitEvent(p->fstream, p->ev_ffork, 0);
+            cudaError_t e = launch_trisolve(p, hb[b & 1], cb[b & 1], p->fstream);
+            if (e == cudaSuccess) e = cudaEventRecord(p->ev_fjoin, p->fstream);
+            if (e != cudaSuccess) { p->h = hb[0]; CK(e, "trisolve (batch)"); }
+            if (b + 1 < B) {
+                p->S = S[b + 1]; p->h = hb[(b + 1) & 1];
+                rc = science_side(p);
+                if (rc != SFFT_OK) break;
+                cudaEventRecord(p->ev_ffork, p->stream);
+            }
+            cudaStreamWaitEvent(p->stream, p->ev_fjoin, 0);
+            e = launch_subtract(p, S[b], p->R, cb[b & 1], D[b]);
+            if (e == cudaSuccess && coeffs)
+                e = cudaMemcpyAsync(coeffs + (size_t)b * p->g.n, cb[b & 1], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
+            if (e != cudaSuccess) { p->h = hb[0]; CK(e, "subtract (batch)"); }
+        }
+        // leave the plan as the sequential path does: h, coef = those of the last image
+        if (rc == SFFT_OK && ((B - 1) & 1)) {
+            cudaMemcpyAsync(hb[0], hb[1], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
+            cudaMemcpyAsync(cb[0], cb[1], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
+        }
+        p->h = hb[0];
+        if (rc != SFFT_OK) return rc;
+        p->have_system = p->have_solution = true;
+        return SFFT_OK;
+    }
     for (int b = 0; b < B; b++) {
         p->S = S[b];
         sfft_status st = science_side(p);

@@ -73,6 +73,7 @@ struct sfft_plan {
     double *delta;           // [NB]
     double *G;               // [n][n]
     double *h;               // [n]
+    double *h2, *coef2;      // [n] each: second right-hand side / solution (the batched path pipelines two images)
     double *Lf;              // [n][n] Cholesky factor of the equilibrated matrix (lower, row-major)
     double *dscale;          // [n]   1/sqrt(G_ii)
     double *Linv;            // [nblk][64][64] inverses of the factor's diagonal blocks
@@ -132,7 +133,7 @@ cudaError_t launch_gather_h(sfft_plan *p);
 
 // ---- a4 (sfft_solve.cu) ------------------------------------------------------------------
 cudaError_t launch_factor(sfft_plan *p);                      // G -> dscale, Lf, flag
-cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c); // c = D (L^-T (L^-1 (D h)))
+cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream_t st = nullptr); // c = D (L^-T (L^-1 (D h))); st: default the plan's stream
 
 // ---- a5 (sfft_subtract.cu) ---------------------------------------------------------------
 // spec: the NK spectra to convolve (default: the plan's unmasked template spectra); mode 0: D = S - M - B,

@@ -507,7 +507,7 @@ cudaError_t launch_factor(sfft_plan *p) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c) {
+cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream_t st) {
     const int n = p->g.n, nblk = (n + CB - 1) / CB;
     p->solve_epoch++;
     const double *Lf = p->Lf, *Li = p->Linv, *ds = p->dscale;
@@ -515,7 +515,7 @@ cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c) {
     int *flags = p->sflags, epoch = p->solve_epoch, nn = n;
     void *args[] = {(void *)&Lf, (void *)&Li, (void *)&ds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&flags, (void *)&epoch};
     KLaunch kl(p, "trisolve");
-    return cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, p->stream);
+    return cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, st ? st : p->stream);
 }
 
 } // namespace sfft
