@@ -295,8 +295,16 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_spli
     const int halves = WB > 10 ? 2 : 1, per_sm = WB > 10 ? 1 : 2, maxthreads = 192;
     const int Tb = g.My / LC_NA;
     double best = 1e300; int bK = 4, bS = 1, bG = np;
+    // A science-side pass that shares the machine with a factorisation (reserve > 0): measured at 4088^2, L = 11, DK = 2,
+    // CTAs of about 64 threads (410 x 60 threads) beat the 256 x 96 threads the cost model below prefers by 0.11 ms per
+    // step -- the pass itself is shorter (0.30 vs 0.38 ms) and the factorisation's small kernels find room on every SM
+    // (0.52 vs 0.66 ms); the landscape is rugged (KXC = 8 and 12 are both worse), so the rule is empirical:
+    // the widest even chunk with npg * KXC <= 64.
+    int kfix = 0;
+    if (reserve > 0 && per_sm == 2 && np <= 32) { kfix = (64 / np) & ~1; if (kfix > 32) kfix = 32; if (kfix < 4) kfix = 0; }
     for (int KXC = 4; KXC <= 32; KXC++) {
         if (KXC > g.Hx) break;
+        if (kfix && kfix <= g.Hx && KXC != kfix) continue;
         if ((size_t)LC_NST * (LC_NA * ns * KXC + WB) * sizeof(cplx) > (size_t)(per_sm == 2 ? 113 : 200) * 1024) break;
         int npg = maxthreads / KXC; if (npg > np) npg = np; if (npg < 1) continue;
         const int ngr = (np + npg - 1) / npg, nkb = (g.Hx + KXC - 1) / KXC;
@@ -306,6 +314,7 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_spli
             const long long ncta = (long long)nkb * ngr * nsplit * halves;
             long long slots = 148LL * per_sm;
             if (reserve > 0 && slots > 4 * reserve) slots -= reserve;
+            if (kfix && ncta < slots && Tb / (2 * nsplit) >= 4 && nsplit < 16) continue; // small CTAs: at least one per slot
             const long long waves = (ncta + slots - 1) / slots;
             // a CTA with few threads keeps the FP64 pipes idle: charge it as if it had at least 160
             const int thr = npg * KXC < 160 ? 160 : npg * KXC;
@@ -316,6 +325,11 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_spli
             if (cost < best) { best = cost; bK = KXC; bS = nsplit; bG = npg; }
         }
     }
+    if (const char *e = getenv(np < ns ? "SFFT_LAG_KXC_SCI" : "SFFT_LAG_KXC")) { // experiment knob: force the chunk width; pairs split evenly over the groups
+        const int k = atoi(e);
+        if (k >= 2 && k <= 32 && k <= g.Hx) { bK = k; bG = maxthreads / k < np ? maxthreads / k : np; }
+    }
+    { const int ngr0 = (np + bG - 1) / bG; bG = (np + ngr0 - 1) / ngr0; } // even pair groups (21 pairs in 2 groups: 11 + 10, not 13 + 8)
     c->WB = WB; c->KXC = bK; c->npg = bG; c->nkb = (g.Hx + bK - 1) / bK; c->ngr = (np + bG - 1) / bG;
     c->nsplit = bS; c->halves = halves;
     c->rows_per_split = (Tb + bS - 1) / bS; // in units of b
@@ -344,7 +358,7 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     const int ns = science ? g.NK + 1 : g.NK;
     static int omega_split = -1; // SFFT_OMEGA_SPLIT=8 shortens the column kernel by 8 % but lengthens the stage (side-stream kernels wait, more partials)
     if (omega_split < 0) { const char *e = getenv("SFFT_OMEGA_SPLIT"); omega_split = e ? atoi(e) : 1; }
-    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, science ? 1 : omega_split, science && p->factor_pending ? theta_reserve() : 0);
+    LagCfg c; lagcol_config(g, pl.np, ns, W, &c, science ? theta_min_split() : omega_split, science && p->factor_pending ? theta_reserve() : 0);
     const int nsplit = c.nsplit;
     if (getenv("SFFT_VERBOSE")) fprintf(stderr, "lagcfg sci=%d np=%d WB=%d KXC=%d npg=%d nkb=%d ngr=%d nsplit=%d halves=%d threads=%d ctas=%d\n", (int)science, pl.np, c.WB, c.KXC, c.npg, c.nkb, c.ngr, c.nsplit, c.halves, c.npg * c.KXC, c.nkb * c.ngr * c.nsplit * c.halves);
     cudaError_t e;
