@@ -325,6 +325,14 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_spli
             if (cost < best) { best = cost; bK = KXC; bS = nsplit; bG = npg; }
         }
     }
+    // Template pass with all pairs in ONE group and fewer CTAs than slots (21 pairs, L = 11: 256 CTAs x 168 threads on 296
+    // slots -- 40 SMs get one CTA, the others two): the next narrower even chunk in two ky-splits deals out evenly
+    // (684 CTAs x 126 threads, 4-5 per SM).  Measured: 0.420 -> 0.392 ms for the column kernel, 0.495 -> 0.458 ms for the
+    // stage; 342 x 126 (no split) 0.457 ms, 1024 x 84 (KXC 4) 0.43 ms, 512 x 168 0.418 ms.  Only this shape is evidenced.
+    if (np >= ns && np >= 16 && per_sm == 2 && bS == 1 && bG == np && bK >= 8 && !(bK & 1) && min_split <= 1 &&
+        (long long)((g.Hx + bK - 1) / bK) < 148LL * per_sm && Tb >= 16) {
+        bK -= 2; bS = 2;
+    }
     if (const char *e = getenv(np < ns ? "SFFT_LAG_KXC_SCI" : "SFFT_LAG_KXC")) { // experiment knob: force the chunk width; pairs split evenly over the groups
         const int k = atoi(e);
         if (k >= 2 && k <= 32 && k <= g.Hx) { bK = k; bG = maxthreads / k < np ? maxthreads / k : np; }
