@@ -135,8 +135,8 @@ cudaError_t launch_gamma(sfft_plan *p) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_delta(sfft_plan *p) {
-    { KLaunch kl(p, "delta"); delta_kernel<<<p->g.NB, 128, 0, p->cur>>>(p->muS, p->delta, p->g); }
+cudaError_t launch_delta(sfft_plan *p, const double *muS, double *delta) {
+    { KLaunch kl(p, "delta"); delta_kernel<<<p->g.NB, 128, 0, p->cur>>>(muS ? muS : p->muS, delta ? delta : p->delta, p->g); }
     return cudaGetLastError();
 }
 
@@ -146,8 +146,8 @@ cudaError_t launch_gather_G(sfft_plan *p) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_gather_h(sfft_plan *p) {
-    { KLaunch kl(p, "gather_h"); gather_h_kernel<<<(p->g.n + 255) / 256, 256, 0, p->cur>>>(p->lagT, p->delta, p->h, p->g); }
+cudaError_t launch_gather_h(sfft_plan *p, const double *lagT, const double *delta, double *h) {
+    { KLaunch kl(p, "gather_h"); gather_h_kernel<<<(p->g.n + 255) / 256, 256, 0, p->cur>>>(lagT ? lagT : p->lagT, delta ? delta : p->delta, h ? h : p->h, p->g); }
     return cudaGetLastError();
 }
 

@@ -24,7 +24,7 @@
 
 namespace sfft {
 
-struct SpecSet { const cplx *p[MAX_NP + 1]; };
+struct SpecSet { const cplx *p[MAX_NP + 2]; };
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
     unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -358,12 +358,13 @@ int border_chunks() { return 1; }
 int theta_reserve() { static int v = -1; if (v < 0) { const char *e = getenv("SFFT_THETA_RESERVE"); v = e ? atoi(e) : 40; } return v; }
 int theta_min_split() { static int v = -1; if (v < 0) { const char *e = getenv("SFFT_THETA_SPLIT"); v = e ? atoi(e) : 1; } return v; }
 
-cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bool science) {
+cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bool science, int nsci) {
     const Geom &g = p->g;
     SpecSet ss;
     for (int t = 0; t < g.NK; t++) ss.p[t] = p->specT + (size_t)t * g.My * g.Hx;
     ss.p[g.NK] = p->specS;
-    const int ns = science ? g.NK + 1 : g.NK;
+    ss.p[g.NK + 1] = nsci > 1 ? p->specS2 : p->specS;
+    const int ns = science ? g.NK + nsci : g.NK;
     static int omega_split = -1; // SFFT_OMEGA_SPLIT=8 shortens the column kernel by 8 % but lengthens the stage (side-stream kernels wait, more partials)
     if (omega_split < 0) { const char *e = getenv("SFFT_OMEGA_SPLIT"); omega_split = e ? atoi(e) : 1; }
     LagCfg c; lagcol_config(g, pl.np, ns, W, &c, science ? theta_min_split() : omega_split, science && p->factor_pending && pl.np >= 6 ? theta_reserve() : 0); // DK <= 1: the factor is short, the plain config is 4 % faster
@@ -378,7 +379,16 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     if (g.Mx != g.nx || g.My != g.ny) {
         nchunk = border_chunks();
         use_side(p, 1);
-        if (W > 0) { e = launch_border(p, pl, W, science, bpart); if (e != cudaSuccess) return e; }
+        if (W > 0 && science && nsci > 1) {
+            // two science images: the wrap corrections image by image (their strips come from p->S), pairs of image 2 behind
+            // those of image 1 in bpart (border_chunks() == 1)
+            const int nl = (2 * W + 1) * (2 * W + 1);
+            e = launch_border(p, p->plT, W, true, bpart); if (e != cudaSuccess) return e;
+            const double *keep = p->S; p->S = p->S2;
+            e = launch_border(p, p->plT, W, true, bpart + (size_t)g.NK * nl);
+            p->S = keep;
+            if (e != cudaSuccess) return e;
+        } else if (W > 0) { e = launch_border(p, pl, W, science, bpart); if (e != cudaSuccess) return e; }
         else nchunk = 0;
     }
     back_to_main(p);

@@ -306,3 +306,27 @@ def test_stamp_mode_1000_cutout():
     recipe, L = 11, DK = 2, DB = 2: 1000 pads to 1024 (wrap corrections on), n = 732, full element-wise parity."""
     c = starfield.make_pair(2, nx=1000, ny=1000, n_stars=3600)
     full_parity(c["S"], c["R"], None, 11, 2, 2, c["noise_rms"])
+
+
+@pytest.mark.parametrize("B", [2, 4, 5])
+def test_batched_pairs_of_images_masked(B):
+    """The batched path takes the science images two at a time through one Theta pass (2 NK pairs over NK + 2 spectra)
+    and pipelines the pairs; even and odd batch sizes, a mask and a zero-padded frame, every image against the
+    single-pair path (same arithmetic per (pair, kx), so the bar is rounding level: 1e-12 relative on the
+    coefficients, 1e-9 of the noise RMS on D)."""
+    nx, ny, L, DK, DB = 100, 72, 5, 2, 1
+    _, R = starfield.random_pair(nx, ny, seed=100)
+    Ss = [starfield.random_pair(nx, ny, seed=101 + b)[0] for b in range(B)]
+    rng = np.random.default_rng(9)
+    mask = (rng.random((ny, nx)) > 0.04).astype(np.uint8)
+    p = SfftPlan(nx, ny, L, DK, DB)
+    p.set_template(dev(R), dev(mask))
+    Ds, cs = p.subtract_batch([dev(s) for s in Ss])
+    p.sync_status()
+    cs = cs.cpu().numpy()
+    for b in range(B):
+        p1, G, h, c, D = run_gpu(Ss[b], R, mask, L, DK, DB)
+        assert np.max(np.abs(c - cs[b])) <= 1e-12 * np.max(np.abs(c)), b
+        assert np.max(np.abs(D - Ds[b].cpu().numpy())) <= 1e-9 * 20.0, b
+        p1.destroy()
+    p.destroy()
