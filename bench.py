@@ -487,8 +487,8 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
         plan.sync_status()
         t_t, t_b = e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
         r = nx * ny * 8.0
-        # per image: a1 of S 4 r, Theta (NK + 2)/2 r (two images share one pass over the NK template spectra), a5 (NK + 4) r
-        per_img_bytes = (4 + (NK + 2) / 2.0 + (NK + 4)) * r + (13 + NK) * r / B
+        # per image: a1 of S 4 r, Theta (NK + 4)/4 r (four images share one pass over the NK template spectra), a5 (NK + 4) r
+        per_img_bytes = (4 + (NK + 4) / 4.0 + (NK + 4)) * r + (13 + NK) * r / B
         out["batched"] = {"workload": f"BASELINE.json configs[3]: one template, B={B} science images "
                                       f"({len(Ss)} distinct seeded images cycled)",
                           "B": B, "template_ms": round(t_t, 3), "per_image_ms": round(t_b / B, 4),

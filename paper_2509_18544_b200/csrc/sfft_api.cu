@@ -74,8 +74,10 @@ static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
                     p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
-                    p->ywork, p->zwork, p->sflags, p->coef, p->h2, p->coef2, p->h3, p->h4, p->coef3, p->coef4, p->specS2, p->muS2, p->delta2, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->ywork, p->zwork, p->sflags, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
+    for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
+    for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
     if (p->flag_host) cudaFreeHost(p->flag_host);
     for (int s = 0; s < SFFT_NUM_STAGES; s++) {
         if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
@@ -128,16 +130,14 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
         for (int tp = t; tp < g.NK; tp++) { p->plO.a[p->plO.np] = t; p->plO.b[p->plO.np] = tp; p->plO.np++; }
     p->plT.np = g.NK;
     for (int t = 0; t < g.NK; t++) { p->plT.a[t] = t; p->plT.b[t] = g.NK; }
-    p->plT2.np = 2 * g.NK;
-    for (int t = 0; t < g.NK; t++) { p->plT2.a[t] = t; p->plT2.b[t] = g.NK; p->plT2.a[g.NK + t] = t; p->plT2.b[g.NK + t] = g.NK + 1; }
     p->npairsO = p->plO.np;
 
     const size_t plane = (size_t)g.My * g.Hx;
     const int W2 = 4 * g.w + 1, n = g.n;
     LagCfg cO, cT; lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.NK + 1, g.w, &cT, 16);
-    const size_t qO = (size_t)cO.nsplit * p->plO.np * W2 * (g.Hx + 1), qT = (size_t)cT.nsplit * 2 * p->plT.np * L * (g.Hx + 1); // 2 x: two science images per pass
+    const size_t qO = (size_t)cO.nsplit * p->plO.np * W2 * (g.Hx + 1), qT = (size_t)cT.nsplit * NSCI * p->plT.np * L * (g.Hx + 1); // NSCI science images per pass
     size_t bO = (size_t)border_chunks() * p->plO.np * W2 * W2;
-    { const size_t bT2 = (size_t)border_chunks() * 2 * g.NK * L * L; if (bT2 > bO) bO = bT2; }
+    { const size_t bT2 = (size_t)border_chunks() * NSCI * g.NK * L * L; if (bT2 > bO) bO = bT2; }
     cudaError_t e = cudaSuccess;
 #define AL(ptr, cnt) if (e == cudaSuccess) e = dalloc(p, &ptr, (size_t)(cnt))
     AL(p->tw, g.Nt);
@@ -146,10 +146,10 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->specS, plane);
     AL(p->muR, (size_t)(DK + DB + 1) * ny);
     AL(p->muS, (size_t)(DB + 1) * ny);
-    AL(p->muS2, (size_t)(DB + 1) * ny);
+    for (int i = 1; i < NSCI; i++) AL(p->muSx[i], (size_t)(DB + 1) * ny);
     AL(p->Q, qO > qT ? qO : qT);
     AL(p->lagO, (size_t)p->plO.np * W2 * W2);
-    AL(p->lagT, (size_t)2 * g.NK * L * L);
+    AL(p->lagT, (size_t)NSCI * g.NK * L * L);
     AL(p->bpart, bO);
     AL(p->SB, border_strip_doubles(g, 2 * g.w > 0 ? 2 * g.w : 1));
     {
@@ -160,7 +160,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->gam, (size_t)g.NK * g.NB * L * L);
     AL(p->phi, g.NB * g.NB);
     AL(p->delta, g.NB);
-    AL(p->delta2, g.NB);
+    for (int i = 1; i < NSCI; i++) AL(p->deltax[i], g.NB);
     AL(p->G, (size_t)n * n);
     AL(p->h, n);
     AL(p->Lf, (size_t)n * n);
@@ -170,9 +170,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->zwork, n);
     AL(p->sflags, 2 * ((n + 63) / 64));
     AL(p->coef, n);
-    AL(p->h2, n);
-    AL(p->coef2, n);
-    AL(p->h3, n); AL(p->h4, n); AL(p->coef3, n); AL(p->coef4, n);
+    for (int i = 1; i < 2 * NSCI; i++) { AL(p->hq[i], n); AL(p->cq[i], n); }
     AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
     AL(p->flag, 1);
 #undef AL
@@ -303,26 +301,30 @@ static sfft_status science_side(sfft_plan *p) {
     return SFFT_OK;
 }
 
-// The same for TWO science images in one pass over the template spectra (batched path): a1 of both, then ONE Theta lag
-// pass with 2 NK pairs over NK + 2 spectra -- the NK template spectra are read once for two images (8 r instead of
-// 14 r at DK = 2).  Results: hA, hB.  Uses p->S / p->S2.
-static sfft_status science_side2(sfft_plan *p, const double *SA, const double *SB, double *hA, double *hB) {
+// The same for nimg <= NSCI science images in ONE pass over the template spectra (batched path): a1 of each image, then
+// one Theta lag pass with nimg NK pairs over NK + nimg spectra -- the NK template spectra are read once for the
+// group ((NK + nimg)/nimg r per image instead of (NK + 1) r).  Results: hout[i].
+static sfft_status science_sideN(sfft_plan *p, int nimg, const double *const *S, double *const *hout) {
     const Geom &g = p->g;
-    if (!p->specS2) CK(dalloc(p, &p->specS2, (size_t)g.My * g.Hx), "alloc second science spectrum");
-    p->S = SA; p->S2 = SB;
+    p->specSx[0] = p->specS; p->muSx[0] = p->muS; p->deltax[0] = p->delta;
     const int i0 = 0, j0 = 0;
-    CK(launch_row_fwd(p, SA, p->mask, p->inter, 1, p->muS, g.DB + 1), "row_fwd(S)");
-    CK(launch_col_fwd(p, p->inter, p->specS, 1, &i0, &j0), "col_fwd(S)");
-    CK(launch_row_fwd(p, SB, p->mask, p->inter, 1, p->muS2, g.DB + 1), "row_fwd(S2)");
-    CK(launch_col_fwd(p, p->inter, p->specS2, 1, &i0, &j0), "col_fwd(S2)");
+    for (int i = 0; i < nimg; i++) {
+        if (!p->specSx[i]) CK(dalloc(p, &p->specSx[i], (size_t)g.My * g.Hx), "alloc science spectrum");
+        p->Sx[i] = S[i];
+        CK(launch_row_fwd(p, S[i], p->mask, p->inter, 1, p->muSx[i], g.DB + 1), "row_fwd(S)");
+        CK(launch_col_fwd(p, p->inter, p->specSx[i], 1, &i0, &j0), "col_fwd(S)");
+    }
+    p->S = S[0];
+    PairList pl; pl.np = nimg * g.NK;
+    for (int i = 0; i < nimg; i++)
+        for (int t = 0; t < g.NK; t++) { pl.a[i * g.NK + t] = t; pl.b[i * g.NK + t] = g.NK + i; }
     fork_side(p);
     use_side(p, 2);
-    CK(launch_delta(p, p->muS, p->delta), "delta");
-    CK(launch_delta(p, p->muS2, p->delta2), "delta");
+    for (int i = 0; i < nimg; i++) CK(launch_delta(p, p->muSx[i], p->deltax[i]), "delta");
     back_to_main(p);
-    CK(launch_lags(p, p->plT2, g.w, p->lagT, true, 2), "lags(Theta x 2)");
-    CK(launch_gather_h(p, p->lagT, p->delta, hA), "gather h");
-    CK(launch_gather_h(p, p->lagT + (size_t)g.NK * g.L * g.L, p->delta2, hB), "gather h");
+    CK(launch_lags(p, pl, g.w, p->lagT, true, nimg), "lags(Theta, several images)");
+    for (int i = 0; i < nimg; i++)
+        CK(launch_gather_h(p, p->lagT + (size_t)i * g.NK * g.L * g.L, p->deltax[i], hout[i]), "gather h");
     return SFFT_OK;
 }
 
@@ -439,49 +441,47 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
     if (!S || !D || B < 1) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: bad arguments");
     for (int b = 0; b < B; b++) if (!S[b] || !D[b]) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: NULL image");
     if (B > 1 && !p->timing && !p->ktiming && p->fstream && !getenv("SFFT_NO_BATCH_PIPE")) {
-        // Two images per science-side pass (science_side2), and a software pipeline over the pairs: the triangular
-        // solves of pair k (latency-bound launches that leave the machine empty) run on the factor stream beside the
-        // science-side kernels of pair k+1.  Order on the main stream: sci(0), [sci(1), a5(pair 0)], [sci(2), a5(pair 1)], ...
-        // h and the coefficients are quadruple-buffered (pair parity x image); the solves of pair k+2 start after
-        // sci(k+2), which is behind a5(pair k) on the main stream, so no buffer is overwritten while in use.
-        double *hb[4] = {p->h, p->h2, p->h3, p->h4}, *cb[4] = {p->coef, p->coef2, p->coef3, p->coef4};
-        const int npair = (B + 1) / 2;
-        auto sci = [&](int k) -> sfft_status { // images 2k, 2k+1 (or the last single image)
-            const int b0 = 2 * k, par = 2 * (k & 1);
-            if (b0 + 1 < B) return science_side2(p, S[b0], S[b0 + 1], hb[par], hb[par + 1]);
-            p->S = S[b0]; p->h = hb[par];
-            const sfft_status r = science_side(p);
-            p->h = hb[0];
-            return r;
+        // Groups of up to NSCI images per science-side pass (science_sideN), and a software pipeline over the groups: the
+        // triangular solves of group k (latency-bound launches that leave the machine empty) run on the factor stream
+        // beside the science-side kernels of group k+1.  Order on the main stream: sci(0), [sci(1), a5(group 0)],
+        // [sci(2), a5(group 1)], ...  h and the coefficients are buffered per (group parity, image); the solves of group
+        // k+2 start after sci(k+2), which is behind a5(group k) on the main stream, so no buffer is overwritten while in use.
+        p->hq[0] = p->h; p->cq[0] = p->coef;
+        static int gsz = 0;
+        if (!gsz) { const char *e = getenv("SFFT_BATCH_GROUP"); gsz = e ? atoi(e) : NSCI; if (gsz < 1 || gsz > NSCI) gsz = NSCI; }
+        const int ngrp = (B + gsz - 1) / gsz;
+        auto sci = [&](int k) -> sfft_status {
+            const int b0 = gsz * k, nimg = B - b0 < gsz ? B - b0 : gsz;
+            return science_sideN(p, nimg, S + b0, p->hq + NSCI * (k & 1));
         };
         sfft_status rc = sci(0);
         if (rc == SFFT_OK) CK(cudaEventRecord(p->ev_ffork, p->stream), "event");
-        for (int k = 0; k < npair && rc == SFFT_OK; k++) {
-            const int b0 = 2 * k, par = 2 * (k & 1), nimg = b0 + 1 < B ? 2 : 1;
+        for (int k = 0; k < ngrp && rc == SFFT_OK; k++) {
+            const int b0 = gsz * k, nimg = B - b0 < gsz ? B - b0 : gsz, par = NSCI * (k & 1);
             cudaStreamWaitEvent(p->fstream, p->ev_ffork, 0);
             cudaError_t e = cudaSuccess;
-            for (int i = 0; i < nimg && e == cudaSuccess; i++) e = launch_trisolve(p, hb[par + i], cb[par + i], p->fstream);
+            for (int i = 0; i < nimg && e == cudaSuccess; i++) e = launch_trisolve(p, p->hq[par + i], p->cq[par + i], p->fstream);
             if (e == cudaSuccess) e = cudaEventRecord(p->ev_fjoin, p->fstream);
             CK(e, "trisolve (batch)");
-            if (k + 1 < npair) {
+            if (k + 1 < ngrp) {
                 rc = sci(k + 1);
                 if (rc != SFFT_OK) break;
                 cudaEventRecord(p->ev_ffork, p->stream);
             }
             cudaStreamWaitEvent(p->stream, p->ev_fjoin, 0);
             for (int i = 0; i < nimg && e == cudaSuccess; i++) {
-                e = launch_subtract(p, S[b0 + i], p->R, cb[par + i], D[b0 + i]);
+                e = launch_subtract(p, S[b0 + i], p->R, p->cq[par + i], D[b0 + i]);
                 if (e == cudaSuccess && coeffs)
-                    e = cudaMemcpyAsync(coeffs + (size_t)(b0 + i) * p->g.n, cb[par + i], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
+                    e = cudaMemcpyAsync(coeffs + (size_t)(b0 + i) * p->g.n, p->cq[par + i], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
             }
             CK(e, "subtract (batch)");
         }
         if (rc != SFFT_OK) return rc;
         // leave the plan as the sequential path does: S, h, coef = those of the last image
-        const int last = 2 * ((npair - 1) & 1) + ((B & 1) ? 0 : 1);
+        const int last = NSCI * ((ngrp - 1) & 1) + (B - 1 - gsz * (ngrp - 1));
         if (last != 0) {
-            cudaMemcpyAsync(hb[0], hb[last], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
-            cudaMemcpyAsync(cb[0], cb[last], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
+            cudaMemcpyAsync(p->h, p->hq[last], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
+            cudaMemcpyAsync(p->coef, p->cq[last], sizeof(double) * p->g.n, cudaMemcpyDeviceToDevice, p->stream);
         }
         p->S = S[B - 1];
         p->have_system = p->have_solution = true;

@@ -12,6 +12,7 @@ namespace sfft {
 constexpr int MAX_DEG = 3;                                   // DK, DB <= 3
 constexpr int MAX_NP = (MAX_DEG + 1) * (MAX_DEG + 2) / 2;    // 10 polynomial terms
 constexpr int MAX_L = 21;
+constexpr int NSCI = 4;    // science images per Theta pass of the batched path
 constexpr int MAX_PAIRS = MAX_NP * (MAX_NP + 1) / 2;         // 55 unordered template pairs
 constexpr double PIVOT_MIN = 1e-12;                          // reading C9
 
@@ -59,10 +60,11 @@ struct sfft_plan {
     sfft::cplx *specT;       // [NK][My][Hx] spectra of the fit (masked) template images
     sfft::cplx *specTo;      // [NK][My][Hx] spectra of the unmasked template images (== specT without mask)
     sfft::cplx *specS;       // [My][Hx]
-    sfft::cplx *specS2;      // [My][Hx] second science spectrum (batched path: two images per Theta pass), allocated on first use
-    double *muS2, *delta2;   // row moments / Delta of the second image
-    double *h3, *h4, *coef3, *coef4; // the batched path pipelines two PAIRS of images
-    const double *S2;        // second science image of a two-image science side
+    // batched path: up to NSCI science images share one Theta pass; groups of images are pipelined two deep
+    sfft::cplx *specSx[sfft::NSCI]; // [My][Hx] each; [0] aliases specS, the others are allocated on first use
+    double *muSx[sfft::NSCI], *deltax[sfft::NSCI]; // row moments / Delta per image; [0] alias muS, delta
+    double *hq[2 * sfft::NSCI], *cq[2 * sfft::NSCI]; // right-hand sides / solutions: group parity x image; [0] alias h, coef
+    const double *Sx[sfft::NSCI];   // the science images of the current group
     double *muR;             // [(DK+DB+1)][ny] row moments sum_x xt^m (m.R)
     double *muS;             // [(DB+1)][ny]
     sfft::cplx *Q;           // [np][2W+1][Hx+1] column-reduced products (stage 1 of a2)
@@ -94,7 +96,7 @@ struct sfft_plan {
     const double *S, *R; const uint8_t *mask;
     bool have_template, have_system, have_factor, have_solution;
     int npairsO;
-    sfft::PairList plO, plT, plT2; // plT2: (t, NK) then (t, NK+1), two science images in one pass
+    sfft::PairList plO, plT;
     // timing
     bool timing; cudaEvent_t ev0[SFFT_NUM_STAGES], ev1[SFFT_NUM_STAGES]; bool ev_used[SFFT_NUM_STAGES];
     // per-launch timing (sfft_enable_timings(plan, 2)): one event pair per kernel launch, in launch order
@@ -130,7 +132,7 @@ cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science,
 // ---- a2, a3 (sfft_lags.cu, sfft_assemble.cu) ---------------------------------------------------------
 // lag tables of pair list pl over spectra base[s] = spec0 + s*My*Hx (s < nsA: template set, s == nsA: specS)
 cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag /*[np][(2W+1)^2]*/, bool science, int nsci = 1);
-// nsci = 2: spectra NK, NK+1 are specS, specS2 (images p->S, p->S2); pl lists the NK pairs of each image in turn
+// nsci > 1: spectra NK + i are specSx[i] (images p->Sx[i]); pl lists the NK pairs of each image in turn
 cudaError_t launch_gamma(sfft_plan *p);   // muR, R, mask -> gam
 cudaError_t launch_delta(sfft_plan *p, const double *muS = nullptr, double *delta = nullptr);   // muS -> delta
 cudaError_t launch_gather_G(sfft_plan *p);

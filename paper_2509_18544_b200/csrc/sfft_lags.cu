@@ -24,7 +24,7 @@
 
 namespace sfft {
 
-struct SpecSet { const cplx *p[MAX_NP + 2]; };
+struct SpecSet { const cplx *p[MAX_NP + NSCI]; };
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
     unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -362,8 +362,7 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     const Geom &g = p->g;
     SpecSet ss;
     for (int t = 0; t < g.NK; t++) ss.p[t] = p->specT + (size_t)t * g.My * g.Hx;
-    ss.p[g.NK] = p->specS;
-    ss.p[g.NK + 1] = nsci > 1 ? p->specS2 : p->specS;
+    for (int i = 0; i < NSCI; i++) ss.p[g.NK + i] = (i < nsci && i > 0) ? p->specSx[i] : p->specS;
     const int ns = science ? g.NK + nsci : g.NK;
     static int omega_split = -1; // SFFT_OMEGA_SPLIT=8 shortens the column kernel by 8 % but lengthens the stage (side-stream kernels wait, more partials)
     if (omega_split < 0) { const char *e = getenv("SFFT_OMEGA_SPLIT"); omega_split = e ? atoi(e) : 1; }
@@ -380,14 +379,16 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
         nchunk = border_chunks();
         use_side(p, 1);
         if (W > 0 && science && nsci > 1) {
-            // two science images: the wrap corrections image by image (their strips come from p->S), pairs of image 2 behind
-            // those of image 1 in bpart (border_chunks() == 1)
+            // several science images: the wrap corrections image by image (their strips come from p->S), the pairs of
+            // image i behind those of image i-1 in bpart (border_chunks() == 1)
             const int nl = (2 * W + 1) * (2 * W + 1);
-            e = launch_border(p, p->plT, W, true, bpart); if (e != cudaSuccess) return e;
-            const double *keep = p->S; p->S = p->S2;
-            e = launch_border(p, p->plT, W, true, bpart + (size_t)g.NK * nl);
+            const double *keep = p->S;
+            for (int i = 0; i < nsci; i++) {
+                p->S = p->Sx[i];
+                e = launch_border(p, p->plT, W, true, bpart + (size_t)i * g.NK * nl);
+                if (e != cudaSuccess) { p->S = keep; return e; }
+            }
             p->S = keep;
-            if (e != cudaSuccess) return e;
         } else if (W > 0) { e = launch_border(p, pl, W, science, bpart); if (e != cudaSuccess) return e; }
         else nchunk = 0;
     }

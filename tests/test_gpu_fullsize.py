@@ -86,7 +86,11 @@ def test_config2_full_roman_size():
     Ds, cs = p.subtract_batch([dS] + [dev(s) for s in Ss[1:]])
     p.sync_status()
     cs = cs.cpu().numpy()
-    assert np.array_equal(cs[0], c) and np.array_equal(Ds[0].cpu().numpy(), D)
+    # batched vs single path: the same sums in a different split order (the batched path runs several science images
+    # through one Theta pass with its own launch shape), so agreement is at rounding level amplified by the system's
+    # conditioning -- bars an order tighter than the oracle-parity bars C12 / C13
+    assert np.max(np.abs(cs[0] - c)) <= 0.1 * TOL_C * np.max(np.abs(c))
+    assert np.max(np.abs(Ds[0].cpu().numpy() - D)) <= 0.1 * TOL_D * cfg["noise_rms"]
     rng = np.random.default_rng(77)
     for b in (1, 2):
         Db = Ds[b].cpu().numpy()

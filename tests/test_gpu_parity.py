@@ -200,7 +200,7 @@ def test_state_and_argument_errors():
 
 def test_batched_matches_single_and_oracle():
     """configs[3]'s structure at reduced size: one template, B science images; template-side work
-    once.  Each image must match the single-pair path bit for bit and the oracle to tolerance."""
+    once.  Each image must match the single-pair path to rounding level and the oracle to tolerance."""
     t = starfield.make_pair(3, nx=300, ny=260, n_stars=600)
     B, L, DK, DB = 3, 11, 2, 2
     Ss = [t["S"]] + [starfield.make_batch_science(t, b) for b in range(1, B)]
@@ -212,7 +212,9 @@ def test_batched_matches_single_and_oracle():
     cs = cs.cpu().numpy()
     for b in range(B):
         p1, G, h, c, D = run_gpu(Ss[b], t["R"], None, L, DK, DB)
-        assert np.array_equal(c, cs[b]) and np.array_equal(D, Ds[b].cpu().numpy())
+        # same sums, different split order (several images per Theta pass): rounding level, an order inside C12 / C13
+        assert np.max(np.abs(c - cs[b])) <= 0.1 * TOL_C * np.max(np.abs(c))
+        assert np.max(np.abs(D - Ds[b].cpu().numpy())) <= 0.1 * TOL_D * t["noise_rms"]
         G0, h0 = oracle.build_system(Ss[b], t["R"], None, L, DK, DB)
         c0 = oracle.solve(G0, h0)
         assert_coeffs(cs[b], c0, L * L * 6)
@@ -308,12 +310,12 @@ def test_stamp_mode_1000_cutout():
     full_parity(c["S"], c["R"], None, 11, 2, 2, c["noise_rms"])
 
 
-@pytest.mark.parametrize("B", [2, 4, 5])
-def test_batched_pairs_of_images_masked(B):
-    """The batched path takes the science images two at a time through one Theta pass (2 NK pairs over NK + 2 spectra)
-    and pipelines the pairs; even and odd batch sizes, a mask and a zero-padded frame, every image against the
-    single-pair path (same arithmetic per (pair, kx), so the bar is rounding level: 1e-12 relative on the
-    coefficients, 1e-9 of the noise RMS on D)."""
+@pytest.mark.parametrize("B", [2, 4, 5, 9])
+def test_batched_groups_of_images_masked(B):
+    """The batched path takes the science images up to four at a time through one Theta pass (4 NK pairs over NK + 4
+    spectra) and pipelines the groups; full and ragged groups, a mask and a zero-padded frame, every image against
+    the single-pair path (same sums in another split order, so the bar is rounding level: 1e-10 relative on the
+    coefficients, 1e-8 of the noise RMS on D)."""
     nx, ny, L, DK, DB = 100, 72, 5, 2, 1
     _, R = starfield.random_pair(nx, ny, seed=100)
     Ss = [starfield.random_pair(nx, ny, seed=101 + b)[0] for b in range(B)]
@@ -326,7 +328,7 @@ def test_batched_pairs_of_images_masked(B):
     cs = cs.cpu().numpy()
     for b in range(B):
         p1, G, h, c, D = run_gpu(Ss[b], R, mask, L, DK, DB)
-        assert np.max(np.abs(c - cs[b])) <= 1e-12 * np.max(np.abs(c)), b
-        assert np.max(np.abs(D - Ds[b].cpu().numpy())) <= 1e-9 * 20.0, b
+        assert np.max(np.abs(c - cs[b])) <= 1e-10 * np.max(np.abs(c)), b
+        assert np.max(np.abs(D - Ds[b].cpu().numpy())) <= 1e-8 * 20.0, b
         p1.destroy()
     p.destroy()
