@@ -125,9 +125,14 @@ sfft_status sfft_subtract_with(sfft_plan *plan, const double *S, const double *c
  * the Cholesky factor of a4.  Keeps the pointer R (see sfft_build_system). */
 sfft_status sfft_set_template(sfft_plan *plan, const double *R, const uint8_t *mask);
 
-/* For b = 0..B-1: a1 (science), Theta, Delta, h, two triangular solves, a5.
- * S, D: HOST arrays of B device pointers (ny*nx doubles each); coeffs: device B*n doubles
- * or NULL.  mask is the one given to sfft_set_template.  Errors: STATE, INVALID_ARG, CUDA. */
+/* For b = 0..B-1: a1 (science), Theta, Delta, h, two triangular solves, a5.  The images go
+ * through the Theta pass in groups of up to four (the template spectra are read once per group)
+ * and the groups are pipelined against the solves; every image's result equals the single-pair
+ * path's up to FP64 rounding.  The first batched call allocates up to three more science spectra
+ * (ny_pad * nx_pad/2 complex each).
+ * S, D: HOST arrays of B device pointers (ny*nx doubles each), all distinct from each other;
+ * coeffs: device B*n doubles or NULL.  mask is the one given to sfft_set_template.
+ * Errors: STATE, INVALID_ARG, CUDA. */
 sfft_status sfft_subtract_batch(sfft_plan *plan, const double *const *S, int B,
                                 double *const *D, double *coeffs);
 
