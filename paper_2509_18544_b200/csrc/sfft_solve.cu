@@ -321,10 +321,19 @@ __global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int 
         if (mode == 2) { bi++; bj++; }
     }
     const int i0 = t0 + bi * CB, j0 = t0 + bj * CB;
-    for (int e = threadIdx.x; e < CB * CB; e += blockDim.x) {
-        const int r = e / CB, c = e % CB;
-        As[r][c] = (i0 + r < n && c < bs) ? Lf[(size_t)(i0 + r) * n + k0 + c] : 0.0;
-        Bs[r][c] = (j0 + r < n && c < bs) ? Lf[(size_t)(j0 + r) * n + k0 + c] : 0.0;
+    {   // all 32 loads of a thread in flight before the first shared-memory store: one global round trip, not sixteen
+        double ta[16], tb[16];
+#pragma unroll
+        for (int i = 0; i < 16; i++) {
+            const int e = threadIdx.x + 256 * i, r = e >> 6, c = e & 63;
+            ta[i] = (i0 + r < n && c < bs) ? Lf[(size_t)(i0 + r) * n + k0 + c] : 0.0;
+            tb[i] = (j0 + r < n && c < bs) ? Lf[(size_t)(j0 + r) * n + k0 + c] : 0.0;
+        }
+#pragma unroll
+        for (int i = 0; i < 16; i++) {
+            const int e = threadIdx.x + 256 * i, r = e >> 6, c = e & 63;
+            As[r][c] = ta[i]; Bs[r][c] = tb[i];
+        }
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -347,14 +356,25 @@ __global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int 
 #pragma unroll
             for (int b = 0; b < 4; b++) dmma884(acc[a][b][0], acc[a][b][1], af[a], bf[b]);
     }
+    // read-modify-write of the 64 x 64 target tile: all reads first (the compiler must otherwise order each load behind
+    // the previous store to the same array), then the stores
+    double cur[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int b = 0; b < 4; b++) {
+            const int r = i0 + rw + 8 * a + fr, c = j0 + cw + 8 * b + 2 * fk;
+            cur[a][b][0] = (r < n && c < n && c <= r) ? Lf[(size_t)r * n + c] : 0.0;
+            cur[a][b][1] = (r < n && c + 1 < n && c + 1 <= r) ? Lf[(size_t)r * n + c + 1] : 0.0;
+        }
 #pragma unroll
     for (int a = 0; a < 2; a++)
 #pragma unroll
         for (int b = 0; b < 4; b++) {
             const int r = i0 + rw + 8 * a + fr, c = j0 + cw + 8 * b + 2 * fk;
             if (r < n) {
-                if (c < n && c <= r) Lf[(size_t)r * n + c] -= acc[a][b][0];
-                if (c + 1 < n && c + 1 <= r) Lf[(size_t)r * n + c + 1] -= acc[a][b][1];
+                if (c < n && c <= r) Lf[(size_t)r * n + c] = cur[a][b][0] - acc[a][b][0];
+                if (c + 1 < n && c + 1 <= r) Lf[(size_t)r * n + c + 1] = cur[a][b][1] - acc[a][b][1];
             }
         }
 }
