@@ -166,8 +166,8 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->Lf, (size_t)n * n);
     AL(p->dscale, n);
     AL(p->Linv, (size_t)((n + 63) / 64) * 64 * 64);
-    AL(p->ywork, n);
-    AL(p->zwork, n);
+    AL(p->ywork, 2 * (size_t)(((n + 63) / 64) * 64)); // flag-in-data exchange words of the triangular solves (two per element)
+    AL(p->zwork, 2 * (size_t)(((n + 63) / 64) * 64));
     AL(p->sflags, 2 * ((n + 63) / 64));
     AL(p->coef, n);
     for (int i = 1; i < 2 * NSCI; i++) { AL(p->hq[i], n); AL(p->cq[i], n); }
@@ -218,6 +218,8 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     e = cudaMemcpy(p->phi, phi, sizeof(double) * g.NB * g.NB, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemset(p->flag, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(p->sflags, 0, sizeof(int) * 2 * ((n + 63) / 64));
+    if (e == cudaSuccess) e = cudaMemset(p->ywork, 0, sizeof(double) * 2 * (size_t)(((n + 63) / 64) * 64)); // epoch 0 never matches a solve
+    if (e == cudaSuccess) e = cudaMemset(p->zwork, 0, sizeof(double) * 2 * (size_t)(((n + 63) / 64) * 64));
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { cudaGetLastError(); free_plan(p); return SFFT_ERR_CUDA; }
     p->launches = 1;
@@ -514,6 +516,7 @@ sfft_status sfft_sync_status(sfft_plan *p) {
     if (p->side) { CK(cudaStreamSynchronize(p->side), "sync side"); CK(cudaStreamSynchronize(p->sideB), "sync side"); CK(cudaStreamSynchronize(p->sideC), "sync side"); }
     if (p->have_factor) {
         CK(cudaMemcpy(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost), "read flag");
+        if (*p->flag_host == 3) return fail(p, SFFT_ERR_CUDA, "triangular solve: a solution block never arrived");
         if (*p->flag_host) return fail(p, SFFT_ERR_NOT_SPD, "pivot <= 1e-12: matrix not positive definite");
     }
     return SFFT_OK;

@@ -385,19 +385,34 @@ __global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int 
 // same from the last block up with L^T.  The critical path is the chain of 64 x 64 diagonal solves; the
 // off-diagonal products of the waiting CTAs run beside it.  flags[0..nblk) forward, [nblk..2 nblk) backward,
 // compared against `epoch` (incremented per call, so no reset is needed).
-__device__ __forceinline__ void wait_flag(const int *f, int epoch) {
-    if (threadIdx.x == 0) {
-        while (*((volatile const int *)f) != epoch) { }
-        __threadfence();
+// Inter-CTA exchange of the solution blocks in the style of a low-latency flag-in-data protocol: a double travels as two
+// 8-byte words (low half | epoch << 32), (high half | epoch << 32).  8-byte stores are atomic, so a reader that finds the
+// epoch of THIS solve in both words has the value: one L2 round trip per hop instead of flag poll + fence + data load
+// (the chain of 2 * nblk hops is the whole cost of the solve).  The epoch increments per call, so stale words never match.
+// A reader gives up after ~1e6 polls and raises *err (a lost block must not hang the device).
+__device__ __forceinline__ void ll_store(unsigned long long *buf, int i, double v, int epoch) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v), e = (unsigned long long)(unsigned)epoch << 32;
+    volatile unsigned long long *w = buf + 2 * (size_t)i;
+    w[0] = (b & 0xffffffffull) | e;
+    w[1] = (b >> 32) | e;
+}
+__device__ __forceinline__ double ll_load(const unsigned long long *buf, int i, int epoch, int *err) {
+    const volatile unsigned long long *w = buf + 2 * (size_t)i;
+    const unsigned long long e = (unsigned long long)(unsigned)epoch;
+    unsigned long long a = w[0], b = w[1];
+    int spins = 0;
+    while ((a >> 32) != e || (b >> 32) != e) {
+        if (++spins > (1 << 20)) { *err = 3; return 0.0; }
+        a = w[0]; b = w[1];
     }
-    __syncthreads();
+    return __longlong_as_double((long long)((a & 0xffffffffull) | (b << 32)));
 }
 
 __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict__ Lf, const double *__restrict__ Linv,
                                                       const double *__restrict__ dscale,
-                                                      const double *__restrict__ h, double *__restrict__ y,
-                                                      double *__restrict__ z, double *__restrict__ c, int n,
-                                                      int *flags, int epoch) {
+                                                      const double *__restrict__ h, unsigned long long *yl,
+                                                      unsigned long long *zl, double *__restrict__ c, int n,
+                                                      int *err, int epoch) {
     __shared__ double Ld[CB][CB + 1];
     __shared__ double vec[CB];
     __shared__ double blk[CB];
@@ -418,8 +433,7 @@ __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict_
             const double *row = Lf + (size_t)(k0 + r) * n + kb * CB;
             l0[q] = r < bs ? row[lane] : 0.0; l1[q] = r < bs ? row[lane + 32] : 0.0;
         }
-        wait_flag(flags + kb, epoch);
-        const double y0 = __ldcg(y + kb * CB + lane), y1 = __ldcg(y + kb * CB + lane + 32);
+        const double y0 = ll_load(yl, kb * CB + lane, epoch, err), y1 = ll_load(yl, kb * CB + lane + 32, epoch, err);
 #pragma unroll
         for (int q = 0; q < 8; q++) acc[q] = fma(l0[q], y0, fma(l1[q], y1, acc[q]));
     }
@@ -440,10 +454,8 @@ __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict_
         t += __shfl_xor_sync(0xffffffffu, t, 1);
         t += __shfl_xor_sync(0xffffffffu, t, 2);
         __syncthreads();
-        if (cq == 0) { blk[r] = t; if (r < bs) y[k0 + r] = t; }
-        __threadfence();
+        if (cq == 0) { blk[r] = t; ll_store(yl, k0 + r, r < bs ? t : 0.0, epoch); } // all 64 rows: readers take whole blocks
         __syncthreads();
-        if (tid == 0) atomicExch(flags + b, epoch);
     }
     // ---------------- backward: columns of this block; thread -> (col = tid % 64, slice = tid / 64)
     const int col = tid & (CB - 1), slice = tid >> 6;
@@ -456,8 +468,7 @@ __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict_
             const int i = slice + 4 * q;
             lv[q] = (i < ibs && col < bs) ? Lf[(size_t)(i0 + i) * n + k0 + col] : 0.0;
         }
-        wait_flag(flags + nblk + kb, epoch);
-        if (tid < CB) vec[tid] = tid < ibs ? __ldcg(z + i0 + tid) : 0.0;
+        if (tid < CB) vec[tid] = tid < ibs ? ll_load(zl, i0 + tid, epoch, err) : 0.0;
         __syncthreads();
 #pragma unroll
         for (int q = 0; q < 16; q++) s = fma(lv[q], vec[slice + 4 * q], s);
@@ -474,10 +485,10 @@ __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict_
         for (int q = 0; q < 16; q++) t = fma(Ld[4 * q + cq][cc], blk[4 * q + cq], t);
         t += __shfl_xor_sync(0xffffffffu, t, 1);
         t += __shfl_xor_sync(0xffffffffu, t, 2);
-        if (cq == 0 && cc < bs) { z[k0 + cc] = t; c[k0 + cc] = t * dscale[k0 + cc]; }
-        __threadfence();
-        __syncthreads();
-        if (tid == 0) atomicExch(flags + nblk + b, epoch);
+        if (cq == 0) {
+            if (cc < bs) c[k0 + cc] = t * dscale[k0 + cc];
+            ll_store(zl, k0 + cc, cc < bs ? t : 0.0, epoch);
+        }
     }
 }
 
@@ -531,9 +542,9 @@ cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream
     const int n = p->g.n, nblk = (n + CB - 1) / CB;
     p->solve_epoch++;
     const double *Lf = p->Lf, *Li = p->Linv, *ds = p->dscale;
-    double *y = p->ywork, *z = p->zwork;
-    int *flags = p->sflags, epoch = p->solve_epoch, nn = n;
-    void *args[] = {(void *)&Lf, (void *)&Li, (void *)&ds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&flags, (void *)&epoch};
+    unsigned long long *y = reinterpret_cast<unsigned long long *>(p->ywork), *z = reinterpret_cast<unsigned long long *>(p->zwork);
+    int *err = p->flag, epoch = p->solve_epoch, nn = n;
+    void *args[] = {(void *)&Lf, (void *)&Li, (void *)&ds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&err, (void *)&epoch};
     KLaunch kl(p, "trisolve");
     return cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, st ? st : p->stream);
 }
