@@ -74,7 +74,7 @@ static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
                     p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
-                    p->ywork, p->zwork, p->sflags, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->ywork, p->zwork, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
@@ -168,7 +168,6 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->Linv, (size_t)((n + 63) / 64) * 64 * 64);
     AL(p->ywork, 2 * (size_t)(((n + 63) / 64) * 64)); // flag-in-data exchange words of the triangular solves (two per element)
     AL(p->zwork, 2 * (size_t)(((n + 63) / 64) * 64));
-    AL(p->sflags, 2 * ((n + 63) / 64));
     AL(p->coef, n);
     for (int i = 1; i < 2 * NSCI; i++) { AL(p->hq[i], n); AL(p->cq[i], n); }
     AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
@@ -217,7 +216,6 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
             phi[s * g.NB + s2] = power_sum(nx, g.pi[s] + g.pi[s2]) * power_sum(ny, g.pj[s] + g.pj[s2]);
     e = cudaMemcpy(p->phi, phi, sizeof(double) * g.NB * g.NB, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemset(p->flag, 0, sizeof(int));
-    if (e == cudaSuccess) e = cudaMemset(p->sflags, 0, sizeof(int) * 2 * ((n + 63) / 64));
     if (e == cudaSuccess) e = cudaMemset(p->ywork, 0, sizeof(double) * 2 * (size_t)(((n + 63) / 64) * 64)); // epoch 0 never matches a solve
     if (e == cudaSuccess) e = cudaMemset(p->zwork, 0, sizeof(double) * 2 * (size_t)(((n + 63) / 64) * 64));
     if (e == cudaSuccess) e = cudaDeviceSynchronize();

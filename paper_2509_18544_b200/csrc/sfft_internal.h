@@ -84,7 +84,7 @@ struct sfft_plan {
     double *dscale;          // [n]   1/sqrt(G_ii)
     double *Linv;            // [nblk][64][64] inverses of the factor's diagonal blocks
     double *ywork, *zwork;   // [n] forward / backward substitution vectors
-    int *sflags; int solve_epoch; // [2*nblk] block-done flags of the cooperative triangular solve
+    int solve_epoch;         // epoch tag of the flag-in-data exchange words of the triangular solves (ywork, zwork), one per solve
     double *coef;            // [n]   solved coefficients
     sfft::cplx *E;           // [NK][L][Hx+1] kernel row tables for a5
     int *flag;               // device: 1 = pivot test failed

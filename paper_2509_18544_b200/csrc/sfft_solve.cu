@@ -381,10 +381,9 @@ __global__ void __launch_bounds__(256) syrk_kernel(double *__restrict__ Lf, int 
 
 // ---- triangular solves: one CTA per 64-row block, all co-resident (cooperative launch) -------------
 // c = D L^-T L^-1 D h.  Forward: CTA b accumulates L[b, kb] y_kb for kb = 0..b-1 as soon as block kb
-// publishes y_kb (flag in global memory), then solves its diagonal block and publishes y_b; backward the
-// same from the last block up with L^T.  The critical path is the chain of 64 x 64 diagonal solves; the
-// off-diagonal products of the waiting CTAs run beside it.  flags[0..nblk) forward, [nblk..2 nblk) backward,
-// compared against `epoch` (incremented per call, so no reset is needed).
+// publishes y_kb, then solves its diagonal block and publishes y_b; backward the same from the last block up
+// with L^T.  The critical path is the chain of 64 x 64 diagonal solves; the off-diagonal products of the
+// waiting CTAs run beside it.
 // Inter-CTA exchange of the solution blocks in the style of a low-latency flag-in-data protocol: a double travels as two
 // 8-byte words (low half | epoch << 32), (high half | epoch << 32).  8-byte stores are atomic, so a reader that finds the
 // epoch of THIS solve in both words has the value: one L2 round trip per hop instead of flag poll + fence + data load
@@ -507,7 +506,6 @@ cudaError_t launch_factor(sfft_plan *p) {
     // the panel kernel of k+1; the rest of the update runs on an auxiliary stream beside it.
     cudaStream_t aux = (p->ktiming || !p->fstream2 || getenv("SFFT_NO_LOOKAHEAD")) ? nullptr : p->fstream2;
     bool aux_busy = false;
-    const int inv_done = 0; // (inverting block kb on the auxiliary stream right after its panel delayed the look-ahead updates queued behind it)
     const size_t sm_panel = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_panel);
     for (int kb = 0; kb < nblk; kb++) {
@@ -533,7 +531,8 @@ cudaError_t launch_factor(sfft_plan *p) {
         aux_busy = true;
     }
     if (aux_busy) cudaStreamWaitEvent(st, p->ev_lookB, 0);
-    if (inv_done < nblk) { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk - inv_done, 256, 3 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n, inv_done); }
+    // (inverting block kb on the auxiliary stream right after its panel delayed the look-ahead updates queued behind it)
+    { KLaunch kl(p, "trinv"); trinv_kernel<<<nblk, 256, 3 * CB * (CB + 1) * sizeof(double), st>>>(p->Linv, n, 0); }
     cudaMemcpyAsync(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     return cudaGetLastError();
 }
