@@ -150,6 +150,36 @@ sfft_status sfft_subtract_batch(sfft_plan *plan, const double *const *S, int B,
  * Errors: INVALID_ARG (NULL or aliased pointers), CUDA. */
 sfft_status sfft_convolve_stamp(sfft_plan *plan, const double *img, const double *stamp, double *out);
 
+/* ---- f1: the decorrelation kernel (pipeline step 7: "Fit and apply the decorrelation kernel to
+ * the difference image.  Also apply the decorrelation kernel to the science PSF and cross-convolved science image")
+ * PAPER.md gives no formula; DESIGN.md section 13 lists the readings D1-D5 these two calls implement.  The kernel is
+ * APPLIED with sfft_convolve_stamp (to D, to the cross-convolved science image; to the science PSF on a small plan). -- */
+
+/* K_out[(v + w) * L + (u + w)] = sum_t a_{t,u,v} xt(x)^i yt(y)^j: the local matching kernel at pixel (x, y) of the
+ * frame (reading D2; xt, yt the centred coordinates of reading C3; x, y may be fractional or outside the frame: the
+ * polynomial is simply evaluated there).  coeffs: device, n doubles in the coefficient layout above, or NULL = the
+ * plan's current solution (STATE error if there is none).  K_out: device, L*L doubles.  Asynchronous on the plan's
+ * stream.  Errors: INVALID_ARG (NULL output, NaN position), STATE, CUDA. */
+sfft_status sfft_local_kernel(sfft_plan *plan, const double *coeffs, double x, double y, double *K_out);
+
+/* stamp_out = the central L x L taps (L the plan's) of the decorrelation kernel W,
+ *     W^(k) = sqrt(F(0) / F(k)),  F(k) = var_S |P_R^(k)|^2 + var_R |P_S^(k)|^2 |K^(k)|^2,
+ * transforms taken on an N x N periodic grid (readings D1, D3, D4): F is the noise power spectrum of
+ * D = S (*) P_R - (R (*) P_S) (*) K for white pixel noise of variance var_S in S and var_R in R; W is real and even,
+ * W^(0) = 1 (flux scale kept); the crop is not renormalised.
+ * K: device, Lk*Lk doubles (e.g. from sfft_local_kernel); psf_S, psf_R: device, Lp*Lp doubles each; all stamps in
+ * the tap layout stamp[(v + w) * P + (u + w)], P odd.  stamp_out: device, L*L doubles.
+ * N: any integer with max(Lk + Lp - 1, L) <= N <= 1024 (no power-of-two restriction: the transforms are pruned direct
+ * sums over the stamp taps); (N*N + 1) doubles of the plan's intermediate buffer serve as scratch, so the call-order
+ * rule of sfft_convolve_stamp applies (not between sfft_build_system and sfft_subtract).
+ * SYNCHRONISES the plan's stream (a per-frame set-up call) and returns INVALID_ARG if F is zero, negative or not finite
+ * at any grid frequency (the kernel is undefined there; stamp_out is then unspecified).
+ * Errors: INVALID_ARG (NULL pointers, even or non-positive stamp sizes, N out of range or larger than the scratch,
+ * negative / non-finite / both-zero variances, zero of F), CUDA. */
+sfft_status sfft_decorrelation_stamp(sfft_plan *plan, const double *K, int Lk, const double *psf_S,
+                                     const double *psf_R, int Lp, double var_S, double var_R, int N,
+                                     double *stamp_out);
+
 /* ---- host-buffer convenience (the end-to-end call bench.py times as `e2e`) ---------- */
 
 /* Whole single-pair path from HOST buffers: copies S, R (and mask, may be NULL) to plan-owned

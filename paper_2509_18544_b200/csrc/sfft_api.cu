@@ -419,6 +419,42 @@ sfft_status sfft_convolve_stamp(sfft_plan *p, const double *img, const double *s
     return SFFT_OK;
 }
 
+sfft_status sfft_local_kernel(sfft_plan *p, const double *coeffs, double x, double y, double *K_out) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!K_out) return fail(p, SFFT_ERR_INVALID_ARG, "local_kernel: NULL output");
+    if (!coeffs) {
+        if (!p->have_solution) return fail(p, SFFT_ERR_STATE, "local_kernel: no coefficients given and nothing solved yet");
+        coeffs = p->coef;
+    }
+    if (!(x == x) || !(y == y)) return fail(p, SFFT_ERR_INVALID_ARG, "local_kernel: position is NaN");
+    back_to_main(p);
+    const double xt = (2.0 * x + 1.0 - p->g.nx) / (double)p->g.nx, yt = (2.0 * y + 1.0 - p->g.ny) / (double)p->g.ny; // reading C3
+    CK(launch_local_kernel(p, coeffs, xt, yt, K_out), "local_kernel");
+    return SFFT_OK;
+}
+
+sfft_status sfft_decorrelation_stamp(sfft_plan *p, const double *K, int Lk, const double *psf_S, const double *psf_R,
+                                     int Lp, double var_S, double var_R, int N, double *stamp_out) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!K || !psf_S || !psf_R || !stamp_out) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: NULL pointer");
+    if (Lk < 1 || Lp < 1 || !(Lk & 1) || !(Lp & 1)) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: stamp sizes must be odd and >= 1");
+    if (N > 1024 || N < Lk + Lp - 1 || N < Lp || N < p->g.L) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: need max(Lk + Lp - 1, L) <= N <= 1024");
+    if (!(var_S >= 0.0) || !(var_R >= 0.0) || !(var_S + var_R > 0.0) || var_S + var_R > 1.7e308)
+        return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: variances must be finite, >= 0 and not both 0");
+    const size_t have = (size_t)(p->g.DK + 1) * p->g.ny * p->g.Hx * sizeof(cplx), need = ((size_t)N * N + 1) * sizeof(double);
+    if (need > have) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: N x N grid does not fit the plan's intermediate buffer");
+    join_factor(p);
+    back_to_main(p);
+    double *F = reinterpret_cast<double *>(p->inter);
+    int *bad = reinterpret_cast<int *>(F + (size_t)N * N);
+    CK(launch_decorr(p, K, Lk, psf_S, psf_R, Lp, var_S, var_R, N, F, bad, stamp_out), "decorrelation_stamp");
+    int bad_host = 0;
+    CK(cudaMemcpyAsync(&bad_host, bad, sizeof(int), cudaMemcpyDeviceToHost, p->stream), "decorrelation_stamp: read flag");
+    CK(cudaStreamSynchronize(p->stream), "decorrelation_stamp: sync");
+    if (bad_host) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: the noise power spectrum has a zero (or overflowed): the kernel is undefined");
+    return SFFT_OK;
+}
+
 sfft_status sfft_set_template(sfft_plan *p, const double *R, const uint8_t *mask) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (!R) return fail(p, SFFT_ERR_INVALID_ARG, "set_template: NULL image");

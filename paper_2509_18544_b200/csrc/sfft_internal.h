@@ -148,6 +148,12 @@ cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream
 cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D,
                             const cplx *spec = nullptr, int mode = 0);
 
+// ---- f1 (sfft_decorr.cu) -----------------------------------------------------------------
+cudaError_t launch_local_kernel(sfft_plan *p, const double *coef, double xt, double yt, double *K);
+// F: N*N doubles of scratch, bad: one int (raised when the noise power is not positive somewhere)
+cudaError_t launch_decorr(sfft_plan *p, const double *K, int Lk, const double *PS, const double *PR, int Lp,
+                          double varS, double varR, int N, double *F, int *bad, double *stamp);
+
 // ---- probes (sfft_probe.cu) -------------------------------------------------------------------
 cudaError_t run_probe_fp64(int kind, int iters, double *tflops);
 

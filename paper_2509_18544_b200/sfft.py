@@ -23,7 +23,8 @@ _STATUS = {0: "OK", -1: "INVALID_ARG", -2: "ALLOC", -3: "CUDA", -4: "STATE", -5:
 SYMBOLS = (
     "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
     "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_with",
-    "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_difference_host", "sfft_sync_status",
+    "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_local_kernel",
+    "sfft_decorrelation_stamp", "sfft_difference_host", "sfft_sync_status",
     "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
     "sfft_kernel_timing_get", "sfft_launch_count",
     "sfft_last_error", "sfft_version", "sfft_debug_read", "sfft_probe_fp64",
@@ -60,6 +61,9 @@ def load_library():
     lib.sfft_subtract.argtypes = [vp, dp, dp]
     lib.sfft_subtract_with.argtypes = [vp, dp, dp, dp]
     lib.sfft_convolve_stamp.argtypes = [vp, dp, dp, dp]
+    cd = ctypes.c_double
+    lib.sfft_local_kernel.argtypes = [vp, dp, cd, cd, dp]
+    lib.sfft_decorrelation_stamp.argtypes = [vp, dp, ci, dp, dp, ci, cd, cd, ci, dp]
     lib.sfft_set_template.argtypes = [vp, dp, dp]
     lib.sfft_subtract_batch.argtypes = [vp, ctypes.POINTER(vp), ci, ctypes.POINTER(vp), dp]
     lib.sfft_difference_host.argtypes = [vp, dp, dp, dp, dp, dp]
@@ -196,6 +200,27 @@ class SfftPlan:
     def cross_convolve(self, S, R, psf_S, psf_R):
         """Pipeline step 5: (S (*) psf_R, R (*) psf_S)."""
         return self.convolve_stamp(S, psf_R), self.convolve_stamp(R, psf_S)
+
+    # -- f1: decorrelation kernel (PAPER.md:88) ----------------------------------------------
+    def local_kernel(self, x, y, coeffs=None, out=None):
+        """K(u, v; x, y) as an L x L stamp; coeffs None = the plan's solution.  See sfft_local_kernel."""
+        if out is None:
+            out = torch.empty((self.L, self.L), dtype=torch.float64, device="cuda")
+        cptr = None if coeffs is None else _dev_f64(coeffs, (self.n,), "coeffs")
+        self._ck(self._lib.sfft_local_kernel(self._h, cptr, float(x), float(y),
+                                             _dev_f64(out, (self.L, self.L), "out")), "sfft_local_kernel")
+        return out
+
+    def decorrelation_stamp(self, K, psf_S, psf_R, var_S, var_R, N, out=None):
+        """The L x L crop of the decorrelation kernel (L the plan's); see sfft_decorrelation_stamp."""
+        Lk, Lp = int(K.shape[0]), int(psf_S.shape[0])
+        if out is None:
+            out = torch.empty((self.L, self.L), dtype=torch.float64, device="cuda")
+        self._ck(self._lib.sfft_decorrelation_stamp(
+            self._h, _dev_f64(K, (Lk, Lk), "K"), Lk, _dev_f64(psf_S, (Lp, Lp), "psf_S"),
+            _dev_f64(psf_R, (Lp, Lp), "psf_R"), Lp, float(var_S), float(var_R), int(N),
+            _dev_f64(out, (self.L, self.L), "out")), "sfft_decorrelation_stamp")
+        return out
 
     # -- batched --------------------------------------------------------------------------
     def set_template(self, R, mask=None):
