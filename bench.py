@@ -15,7 +15,8 @@ Extra objects on the JSON line: `roofline` (dominant kernel, timed live with CUD
 the library's per-launch timers on the plan's stream), `path_roofline` (the metric's "% of HBM
 roofline": 34 r of algorithmic bytes over the a1+a2+a3+a5 time), `stages_ms`, `kernels_ms`,
 `batched` (configs[3]: template-side work once, per-science-image throughput), `cross_convolve`
-(f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `stamp_mode`
+(f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `decorrelate`
+(f1: decorrelation stamp build + one application), `stamp_mode`
 (f4: the path on a 1000 x 1000 cut-out), `cpu_baseline`
 (the oracle on this box's host cores, bounded sample), `clocks`.
 
@@ -432,6 +433,54 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
                                                 "pairs_per_s_full_frame_est": round(1.0 / (2 * t_cpu * (nx * ny) / (crop * crop)), 4)}}
     except Exception as ex:  # pragma: no cover
         out["cross_convolve"] = {"error": str(ex)}
+
+    # f1: the decorrelation kernel from a local kernel stamp and the two PSF stamps on an
+    # N = 64 grid (sfft_decorrelation_stamp synchronises: host clock), then applied to a frame (8 r, like one
+    # cross-convolution).  K is a fixed synthetic stamp so that the oracle sees no CUDA-path value.
+    try:
+        import oracle
+        from oracle import decorrelation as _deco
+        import time as _time
+        L = cfg["L"]
+        w = (L - 1) // 2
+        yy, xx = np.mgrid[-w:w + 1, -w:w + 1]
+
+        def _g(sg, dx=0.0):
+            st = np.exp(-0.5 * ((xx - dx) ** 2 + yy * yy) / (sg * sg)); return st / st.sum()
+        Kst, pS, pR = 1.05 * _g(0.6, 0.1), _g(1.0), _g(0.85)
+        vS, vR, Ng = 64.0, 64.0 / 9.0, 64
+        dK, dpS, dpR = (torch.from_numpy(a).cuda() for a in (Kst, pS, pR))
+        dW = torch.empty((L, L), dtype=torch.float64, device="cuda")
+        oW = torch.empty_like(dS)
+        for _ in range(3):
+            plan.decorrelation_stamp(dK, dpS, dpR, vS, vR, Ng, dW)
+            plan.convolve_stamp(dS, dW, oW)
+        torch.cuda.synchronize()
+        t0 = _time.perf_counter()
+        for _ in range(K):
+            plan.decorrelation_stamp(dK, dpS, dpR, vS, vR, Ng, dW)
+        ms_build = (_time.perf_counter() - t0) * 1e3 / K
+        stream = torch.cuda.current_stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            plan.convolve_stamp(dS, dW, oW)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_apply = e0.elapsed_time(e1) / K
+        W0 = _deco.decorrelation_stamp(Kst, pS, pR, vS, vR, Ng, L)
+        crop = 1022 if ny >= 1022 and nx >= 1022 else min(nx, ny)
+        ref = oracle.convolve_stamp(pair["S"][:crop, :crop], W0)
+        got = oW[:crop - w, :crop - w].cpu().numpy()[w:, w:]
+        r = nx * ny * 8.0
+        out["decorrelate"] = {"workload": f"decorrelation stamp {L} x {L} on a {Ng} x {Ng} grid, applied to one {nx} x {ny} frame (PAPER.md:88)",
+                              "stamp_build_ms_host_clock": round(ms_build, 4), "apply_ms": round(ms_apply, 4),
+                              "apply_achieved_gbs": round(8 * r / ms_apply / 1e6, 1),
+                              "apply_frac_of_measured_hbm": round(8 * r / ms_apply / 1e6 / peak, 4),
+                              "oracle_check_stamp_max_abs_err": float(np.max(np.abs(dW.cpu().numpy() - W0))),
+                              "oracle_check_image_max_abs_err": float(np.max(np.abs(got - ref[w:crop - w, w:crop - w])))}
+    except Exception as ex:  # pragma: no cover
+        out["decorrelate"] = {"error": str(ex)}
 
     # f4: "decrease the processed stamp size ... down to a minimum size of 1000 x 1000 px": the same path
     # on a contiguous 1000 x 1000 cut-out of the pair (a second, small plan; same L, DK, DB).

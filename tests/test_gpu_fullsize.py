@@ -148,3 +148,32 @@ def test_cross_convolution_at_4088_sampled():
         assert np.max(np.abs(out[ys, xs] - ref)) <= TOL_CONV * np.max(np.abs(img)) * np.abs(st).sum()
         assert abs(out.sum() - img.sum() * st.sum()) <= 1e-10 * np.abs(img).sum() * np.abs(st).sum()
     p.destroy()
+
+
+def test_decorrelation_at_4088_sampled():
+    """f1 in the configuration bench.py times: an 11 x 11 decorrelation stamp on a 64 x 64 grid, built on
+    the full-frame plan and applied to the 4088 x 4088 science frame; the stamp against the oracle tap by tap, the
+    decorrelated frame on sampled pixels the oracle computes one by one, and the flux scale sum(out) = sum(img) sum(W)."""
+    from oracle import decorrelation as deco
+    from test_gpu_parity import TOL_CONV, _psf_stamp
+    cfg = starfield.make_pair(2)
+    S = cfg["S"]
+    ny, nx = S.shape
+    P, w, N = 11, 5, 64
+    K, psfS, psfR = 1.05 * _psf_stamp(P, 23, 0.6), _psf_stamp(P, 21, 1.0), _psf_stamp(P, 22, 0.85)
+    vS, vR = 64.0, 64.0 / 9.0
+    p = SfftPlan(nx, ny, P, 2, 2)
+    W = p.decorrelation_stamp(dev(K), dev(psfS), dev(psfR), vS, vR, N)
+    out = p.convolve_stamp(dev(S), W).cpu().numpy()
+    W = W.cpu().numpy()
+    W0 = deco.decorrelation_stamp(K, psfS, psfR, vS, vR, N, P)
+    F = deco.noise_power(K, psfS, psfR, vS, vR, N)
+    assert np.max(np.abs(W - W0)) <= 1e-13 * np.sqrt(F[0, 0] / F.min())
+    rng = np.random.default_rng(19)
+    xs = rng.integers(0, nx, 600); ys = rng.integers(0, ny, 600)
+    xs[:6] = [0, nx - 1, 0, nx - 1, w - 1, nx - w]
+    ys[:6] = [0, 0, ny - 1, ny - 1, ny // 2, 5]
+    ref = oracle.convolve_stamp_at(S, W0, xs, ys)
+    assert np.max(np.abs(out[ys, xs] - ref)) <= TOL_CONV * np.max(np.abs(S)) * np.abs(W0).sum()
+    assert abs(out.sum() - S.sum() * W0.sum()) <= 1e-10 * np.abs(S).sum() * np.abs(W0).sum()
+    p.destroy()
