@@ -150,6 +150,26 @@ sfft_status sfft_subtract_batch(sfft_plan *plan, const double *const *S, int B,
  * Errors: INVALID_ARG (NULL or aliased pointers), CUDA. */
 sfft_status sfft_convolve_stamp(sfft_plan *plan, const double *img, const double *stamp, double *out);
 
+/* ---- f3: alignment / resampling onto the science grid (pipeline step 4: "Align the reference image,
+ * reference PSF, and reference detection mask to the science image").  PAPER.md names neither the
+ * geometric model nor the interpolant; DESIGN.md section 14 lists the readings A1-A4 implemented here. ---------- */
+
+/* out(x, y) = interpolant of img at xs = (M[0] x + M[1] y) + M[2], ys = (M[3] x + M[4] y) + M[5]  (the affine map from
+ * an OUTPUT pixel to SOURCE pixel coordinates, pixel centres at integers, FP64, evaluated in this order without fused
+ * multiply-add).  img, out: device, ny*nx doubles, row-major, the plan's frame size, must not alias.  M: HOST, 6 doubles
+ * (read before the call returns).  method: 0 = nearest (pixel floor(xs + 0.5), floor(ys + 0.5)); 1 = bilinear;
+ * 3 = Lanczos-3, k(t) = sinc(t) sinc(t/3), |t| < 3, the 6 weights of each axis divided by their sum.  An output pixel
+ * whose footprint (taps floor(xs)-a+1 .. floor(xs)+a on each axis, a = 1 / 3; the one pixel for nearest) is not entirely
+ * inside the frame is set to `fill` (any double, NaN allowed).  Touches no plan workspace (callable at any point of the
+ * call sequence); asynchronous on the plan's stream.  The plan's L, DK, DB are irrelevant.
+ * Errors: INVALID_ARG (NULL or aliased pointers, non-finite M, unknown method), CUDA. */
+sfft_status sfft_resample_affine(sfft_plan *plan, const double *img, const double *M, int method, double fill,
+                                 double *out);
+
+/* The same geometry for a detection mask: nearest neighbour on uint8 (device, ny*nx), pixels from outside = fill
+ * (0..255).  Errors: INVALID_ARG, CUDA. */
+sfft_status sfft_resample_affine_mask(sfft_plan *plan, const uint8_t *mask, const double *M, int fill, uint8_t *out);
+
 /* ---- f1: the decorrelation kernel (pipeline step 7: "Fit and apply the decorrelation kernel to
  * the difference image.  Also apply the decorrelation kernel to the science PSF and cross-convolved science image")
  * PAPER.md gives no formula; DESIGN.md section 13 lists the readings D1-D5 these two calls implement.  The kernel is

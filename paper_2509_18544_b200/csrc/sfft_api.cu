@@ -419,6 +419,34 @@ sfft_status sfft_convolve_stamp(sfft_plan *p, const double *img, const double *s
     return SFFT_OK;
 }
 
+static bool affine_ok(const double *M) {
+    if (!M) return false;
+    for (int i = 0; i < 6; i++) if (!(M[i] - M[i] == 0.0)) return false; // NaN or infinite
+    return true;
+}
+
+sfft_status sfft_resample_affine(sfft_plan *p, const double *img, const double *M, int method, double fill, double *out) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!img || !out) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine: NULL pointer");
+    if (img == out) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine: in-place operation is not supported");
+    if (!affine_ok(M)) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine: the matrix must be 6 finite numbers");
+    if (method != 0 && method != 1 && method != 3) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine: method must be 0 (nearest), 1 (bilinear) or 3 (Lanczos-3)");
+    back_to_main(p);
+    CK(launch_resample(p, img, M, method, fill, out), "resample_affine");
+    return SFFT_OK;
+}
+
+sfft_status sfft_resample_affine_mask(sfft_plan *p, const uint8_t *mask, const double *M, int fill, uint8_t *out) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!mask || !out) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine_mask: NULL pointer");
+    if (mask == out) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine_mask: in-place operation is not supported");
+    if (!affine_ok(M)) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine_mask: the matrix must be 6 finite numbers");
+    if (fill < 0 || fill > 255) return fail(p, SFFT_ERR_INVALID_ARG, "resample_affine_mask: fill must be 0..255");
+    back_to_main(p);
+    CK(launch_resample_mask(p, mask, M, fill, out), "resample_affine_mask");
+    return SFFT_OK;
+}
+
 sfft_status sfft_local_kernel(sfft_plan *p, const double *coeffs, double x, double y, double *K_out) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (!K_out) return fail(p, SFFT_ERR_INVALID_ARG, "local_kernel: NULL output");

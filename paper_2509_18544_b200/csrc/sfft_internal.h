@@ -154,6 +154,11 @@ cudaError_t launch_local_kernel(sfft_plan *p, const double *coef, double xt, dou
 cudaError_t launch_decorr(sfft_plan *p, const double *K, int Lk, const double *PS, const double *PR, int Lp,
                           double varS, double varR, int N, double *F, int *bad, double *stamp);
 
+// ---- f3 (sfft_align.cu) ------------------------------------------------------------------
+// M: 6 host doubles (output pixel -> source position); method 0 nearest, 1 bilinear, 3 Lanczos-3
+cudaError_t launch_resample(sfft_plan *p, const double *img, const double *M, int method, double fill, double *out);
+cudaError_t launch_resample_mask(sfft_plan *p, const uint8_t *mask, const double *M, int fill, uint8_t *out);
+
 // ---- probes (sfft_probe.cu) -------------------------------------------------------------------
 cudaError_t run_probe_fp64(int kind, int iters, double *tflops);
 

@@ -23,7 +23,7 @@ _STATUS = {0: "OK", -1: "INVALID_ARG", -2: "ALLOC", -3: "CUDA", -4: "STATE", -5:
 SYMBOLS = (
     "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
     "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_subtract", "sfft_subtract_with",
-    "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_local_kernel",
+    "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_resample_affine", "sfft_resample_affine_mask", "sfft_local_kernel",
     "sfft_decorrelation_stamp", "sfft_difference_host", "sfft_sync_status",
     "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
     "sfft_kernel_timing_get", "sfft_launch_count",
@@ -62,6 +62,8 @@ def load_library():
     lib.sfft_subtract_with.argtypes = [vp, dp, dp, dp]
     lib.sfft_convolve_stamp.argtypes = [vp, dp, dp, dp]
     cd = ctypes.c_double
+    lib.sfft_resample_affine.argtypes = [vp, dp, ctypes.POINTER(cd), ci, cd, dp]
+    lib.sfft_resample_affine_mask.argtypes = [vp, dp, ctypes.POINTER(cd), ci, dp]
     lib.sfft_local_kernel.argtypes = [vp, dp, cd, cd, dp]
     lib.sfft_decorrelation_stamp.argtypes = [vp, dp, ci, dp, dp, ci, cd, cd, ci, dp]
     lib.sfft_set_template.argtypes = [vp, dp, dp]
@@ -200,6 +202,25 @@ class SfftPlan:
     def cross_convolve(self, S, R, psf_S, psf_R):
         """Pipeline step 5: (S (*) psf_R, R (*) psf_S)."""
         return self.convolve_stamp(S, psf_R), self.convolve_stamp(R, psf_S)
+
+    # -- f3: alignment onto the science grid (PAPER.md:85) ------------------------------------
+    def resample_affine(self, img, M, method=3, fill=0.0, out=None):
+        """out(x, y) = img interpolated at (M0 x + M1 y + M2, M3 x + M4 y + M5); see sfft_resample_affine."""
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        Mc = (ctypes.c_double * 6)(*[float(m) for m in M])
+        self._ck(self._lib.sfft_resample_affine(self._h, _dev_f64(img, self.shape, "img"), Mc, int(method), float(fill),
+                                                _dev_f64(out, self.shape, "out")), "sfft_resample_affine")
+        return out
+
+    def resample_affine_mask(self, mask, M, fill=0, out=None):
+        """Nearest-neighbour resampling of a uint8 mask with the same geometry; see sfft_resample_affine_mask."""
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.uint8, device="cuda")
+        Mc = (ctypes.c_double * 6)(*[float(m) for m in M])
+        self._ck(self._lib.sfft_resample_affine_mask(self._h, _dev_mask(mask, self.shape), Mc, int(fill),
+                                                     _dev_mask(out, self.shape)), "sfft_resample_affine_mask")
+        return out
 
     # -- f1: decorrelation kernel (PAPER.md:88) ----------------------------------------------
     def local_kernel(self, x, y, coeffs=None, out=None):

@@ -177,3 +177,28 @@ def test_decorrelation_at_4088_sampled():
     assert np.max(np.abs(out[ys, xs] - ref)) <= TOL_CONV * np.max(np.abs(S)) * np.abs(W0).sum()
     assert abs(out.sum() - S.sum() * W0.sum()) <= 1e-10 * np.abs(S).sum() * np.abs(W0).sum()
     p.destroy()
+
+
+def test_alignment_at_4088_sampled():
+    """f3 in the configuration bench.py times: Lanczos-3 resampling of the 4088 x 4088 template under a
+    small rotation + shift, on sampled output pixels (the oracle evaluated on a crop around each would need the whole
+    frame, so the oracle runs once on the full frame: a few seconds of numpy), and the mask bit-exact everywhere."""
+    from oracle import alignment as al
+    cfg = starfield.make_pair(2)
+    R = cfg["R"]
+    ny, nx = R.shape
+    cx, cy, th = (nx - 1) / 2.0, (ny - 1) / 2.0, 2e-4
+    c, s = np.cos(th), np.sin(th)
+    M = [c, -s, cx - c * cx + s * cy + 0.37, s, c, cy - s * cx - c * cy - 0.21]
+    p = SfftPlan(nx, ny, 11, 2, 2)
+    out = p.resample_affine(dev(R), M, method=3, fill=float("nan")).cpu().numpy()
+    ref = al.resample_affine(R, M, al.LANCZOS3, np.nan)
+    assert np.array_equal(np.isnan(out), np.isnan(ref))
+    ok = ~np.isnan(ref)
+    assert ok.mean() > 0.99
+    assert np.max(np.abs(out[ok] - ref[ok])) <= 1e-12 * np.max(np.abs(R))
+    rng = np.random.default_rng(23)
+    m = (rng.random((ny, nx)) > 0.02).astype(np.uint8)
+    mo = p.resample_affine_mask(dev(m), M, fill=0).cpu().numpy()
+    assert np.array_equal(mo, al.resample_affine_mask(m, M, fill=0))
+    p.destroy()
