@@ -16,7 +16,8 @@ the library's per-launch timers on the plan's stream), `path_roofline` (the metr
 roofline": 34 r of algorithmic bytes over the a1+a2+a3+a5 time), `stages_ms`, `kernels_ms`,
 `batched` (configs[3]: template-side work once, per-science-image throughput), `cross_convolve`
 (f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `decorrelate`
-(f1: decorrelation stamp build + one application), `stamp_mode`
+(f1: decorrelation stamp build + one application), `align` (f3: affine resampling of one
+frame and its mask), `stamp_mode`
 (f4: the path on a 1000 x 1000 cut-out), `cpu_baseline`
 (the oracle on this box's host cores, bounded sample), `clocks`.
 
@@ -433,6 +434,49 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
                                                 "pairs_per_s_full_frame_est": round(1.0 / (2 * t_cpu * (nx * ny) / (crop * crop)), 4)}}
     except Exception as ex:  # pragma: no cover
         out["cross_convolve"] = {"error": str(ex)}
+
+    # f3: Lanczos-3 resampling of the template under a small rotation + shift (2 r of
+    # algorithmic bytes: the frame read once, written once) and the nearest-neighbour mask.  Oracle check on the
+    # top-left crop (same pixel coordinates, so every pixel whose footprint lies inside the crop must agree).
+    try:
+        from oracle import alignment as _al
+        cx, cy, th = (nx - 1) / 2.0, (ny - 1) / 2.0, 2e-4
+        co, si = float(np.cos(th)), float(np.sin(th))
+        Maff = [co, -si, cx - co * cx + si * cy + 0.37, si, co, cy - si * cx - co * cy - 0.21]
+        oA = torch.empty_like(dR)
+        dM = (torch.rand((ny, nx), device="cuda") > 0.02).to(torch.uint8)
+        oM = torch.empty_like(dM)
+        res = {}
+        for name, fn in (("lanczos3", lambda: plan.resample_affine(dR, Maff, 3, float("nan"), oA)),
+                         ("bilinear", lambda: plan.resample_affine(dR, Maff, 1, float("nan"), oA)),
+                         ("mask_nearest", lambda: plan.resample_affine_mask(dM, Maff, 0, oM))):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            stream = torch.cuda.current_stream()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(K):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            res[name] = e0.elapsed_time(e1) / K
+        plan.resample_affine(dR, Maff, 3, float("nan"), oA)
+        crop = 1022 if ny >= 1022 and nx >= 1022 else min(nx, ny)
+        ref = _al.resample_affine(pair["R"][:crop, :crop], Maff, _al.LANCZOS3, np.nan)
+        got = oA[:crop, :crop].cpu().numpy()
+        okm = ~np.isnan(ref) & ~np.isnan(got)
+        r = nx * ny * 8.0
+        out["align"] = {"workload": f"affine resampling of one {nx} x {ny} frame, rotation 2e-4 rad + sub-pixel shift (PAPER.md:85)",
+                        "lanczos3_ms": round(res["lanczos3"], 4), "bilinear_ms": round(res["bilinear"], 4),
+                        "mask_nearest_ms": round(res["mask_nearest"], 4),
+                        "lanczos3_achieved_gbs": round(2 * r / res["lanczos3"] / 1e6, 1),
+                        "lanczos3_frac_of_measured_hbm": round(2 * r / res["lanczos3"] / 1e6 / peak, 4),
+                        "bilinear_frac_of_measured_hbm": round(2 * r / res["bilinear"] / 1e6 / peak, 4),
+                        "oracle_check_pixels": int(okm.sum()),
+                        "oracle_check_max_abs_err": float(np.max(np.abs(got[okm] - ref[okm])))}
+    except Exception as ex:  # pragma: no cover
+        out["align"] = {"error": str(ex)}
 
     # f1: the decorrelation kernel from a local kernel stamp and the two PSF stamps on an
     # N = 64 grid (sfft_decorrelation_stamp synchronises: host clock), then applied to a frame (8 r, like one
