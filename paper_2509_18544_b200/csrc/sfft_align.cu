@@ -3,7 +3,8 @@
 //     xs = (M0 x + M1 y) + M2,  ys = (M3 x + M4 y) + M5      (FP64, this order, no fused multiply-add: the integer
 // decisions floor(xs), floor(xs + 0.5) and the footprint test are then the same bits as in the oracle).
 // One thread per output pixel, 32 x 8 pixel CTAs: the 2a x 2a footprints of neighbouring pixels overlap, so the source
-// is read from HBM about once (through L1/L2) and the kernel is bound by 1 r read + 1 r written.
+// is read from HBM once (through L1/L2: ncu 134 MB read at 4088^2); nearest and bilinear are bound by 1 r read + 1 r
+// written, Lanczos-3 by the FP64 instructions of its 12 weights and 36 taps per pixel.
 // With f = xs - floor(xs) and tap offsets k = -2..3:
 //     sin(pi (f - k)) = (-1)^k sin(pi f),   sin(pi (f - k)/3) = sin(pi f/3) cos(k pi/3) - cos(pi f/3) sin(k pi/3).
 #include "sfft_internal.h"
@@ -18,29 +19,32 @@ __device__ __forceinline__ void source_pos(const Affine &A, int x, int y, double
 }
 
 // Weights PROPORTIONAL to k(f - k), k = -2..3, k(t) = sinc(t) sinc(t/3): the caller divides by their sum (reading A2), so
-// the factors common to the six taps -- 3/pi^2 and |sin(pi f)| -- are dropped:  w_k = (-1)^k sin(pi (f - k)/3) / (f - k)^2.
-// One sincospi and ONE division per axis (the six 1/t^2 come from prefix products of the t^2 and the reciprocal of their
-// product); the kernel is bound by FP64 instruction issue, not by HBM, so this is what its time is made of.
+// every factor common to the six taps is dropped -- 3/pi^2, |sin(pi f)| and 1/prod_j (f - j)^2:
+//     w_k = (-1)^k sin(pi (f - k)/3) prod_{j != k} (f - j)^2.
+// One sincospi and no division per axis (prefix / suffix products of the t^2); ncu shows the kernel bound by FP64
+// instruction issue, not by HBM (profiles/r01o_align_ncu.md), so this is what its time is made of.
 __device__ __forceinline__ void lanczos3_weights(double f, double w[6]) {
     const double H = 0.86602540378443864676372317075294;    // sqrt(3)/2
     const double ck[6] = {-0.5, 0.5, 1.0, 0.5, -0.5, -1.0}, sk[6] = {-H, -H, 0.0, H, H, 0.0};
-    if (f < 1e-30) { // on a pixel centre (sin(pi f) = 0 kills every other tap); also keeps 1/f^2 finite
+    if (f == 0.0) { // on a pixel centre sin(pi f) = 0 kills every other tap (and the products below would all vanish)
 #pragma unroll
         for (int q = 0; q < 6; q++) w[q] = q == 2 ? 1.0 : 0.0;
         return;
     }
     double s3, c3;
     sincospi(f * (1.0 / 3.0), &s3, &c3);
-    double u[6], pre[6];
+    double u[6], pre[6], suf[6];
 #pragma unroll
-    for (int q = 0; q < 6; q++) { const double t = f - (double)(q - 2); u[q] = t * t; pre[q] = q ? pre[q - 1] * u[q] : u[q]; }
-    double inv = 1.0 / pre[5];
+    for (int q = 0; q < 6; q++) { const double t = f - (double)(q - 2); u[q] = t * t; }
+    pre[0] = 1.0; suf[5] = 1.0;
 #pragma unroll
-    for (int q = 5; q >= 0; q--) {
-        const double r = q ? inv * pre[q - 1] : inv; // 1 / u[q]
-        inv *= u[q];
+    for (int q = 1; q < 6; q++) pre[q] = pre[q - 1] * u[q - 1];
+#pragma unroll
+    for (int q = 4; q >= 0; q--) suf[q] = suf[q + 1] * u[q + 1];
+#pragma unroll
+    for (int q = 0; q < 6; q++) {
         const double b = s3 * ck[q] - c3 * sk[q];     // sin(pi (f - k)/3)
-        w[q] = ((q & 1) ? -b : b) * r;
+        w[q] = ((q & 1) ? -b : b) * (pre[q] * suf[q]);
     }
 }
 
