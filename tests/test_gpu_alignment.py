@@ -112,3 +112,18 @@ def test_resample_errors():
     with pytest.raises(SfftError):
         p.resample_affine_mask(m, [1, 0, 0, 0, 1, 0], fill=300)
     p.destroy()
+
+
+def test_psf_stamp_is_resampled_on_a_plan_of_its_own_size():
+    """Reading A4: the reference PSF (a 25 x 25 stamp) is aligned like an image, on a plan of the stamp's size."""
+    P = 25
+    yy, xx = np.mgrid[0:P, 0:P] - (P - 1) / 2.0
+    psf = np.exp(-0.5 * ((xx / 1.6) ** 2 + (yy / 2.1) ** 2)); psf /= psf.sum()
+    M = _rot(0.3, 1.0, 1.0, 0.25, -0.4, P, P)
+    p = SfftPlan(P, P, 1, 0, 0)
+    for method in (al.BILINEAR, al.LANCZOS3):
+        out = p.resample_affine(dev(psf), M, method=method, fill=0.0).cpu().numpy()
+        ref = al.resample_affine(psf, M, method, 0.0)
+        assert np.array_equal(out == 0.0, ref == 0.0)
+        assert np.max(np.abs(out - ref)) <= TOL_RS * psf.max()
+    p.destroy()

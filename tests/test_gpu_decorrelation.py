@@ -124,3 +124,23 @@ def test_decorrelation_stamp_errors():
     ref = np.zeros((5, 5)); ref[2, 2] = 1.0
     assert np.max(np.abs(W - ref)) < 1e-15
     p.destroy()
+
+
+def test_decorrelated_science_psf_on_a_small_plan():
+    """"Also apply the decorrelation kernel to the science PSF": a 25 x 25 PSF stamp convolved with the
+    11 x 11 decorrelation stamp on a plan of the stamp's size (circular at 25 x 25, like any frame: reading C6)."""
+    P, L, N = 25, 11, 64
+    yy, xx = np.mgrid[0:P, 0:P] - (P - 1) / 2.0
+    psf_img = np.exp(-0.5 * ((xx / 1.1) ** 2 + (yy / 1.3) ** 2)); psf_img /= psf_img.sum()
+    K, PS, PR = _stamp(L, 7, 0.7), _stamp(L, 8, 0.9), _stamp(L, 9, 0.8)
+    big = SfftPlan(128, 128, L, 0, 0)          # the stamp is built once on the frame's plan (its scratch holds N x N) ...
+    W = big.decorrelation_stamp(dev(K), dev(PS), dev(PR), 9.0, 1.0, N)
+    p = SfftPlan(P, P, L, 0, 0)                # ... and applied to the PSF on a plan of the PSF stamp's size
+    with pytest.raises(SfftError):
+        p.decorrelation_stamp(dev(K), dev(PS), dev(PR), 9.0, 1.0, N)   # 64 x 64 does not fit a 25 x 25 plan's scratch
+    out = p.convolve_stamp(dev(psf_img), W).cpu().numpy()
+    W0 = deco.decorrelation_stamp(K, PS, PR, 9.0, 1.0, N, L)
+    ref = oracle.convolve_stamp(psf_img, W0)
+    assert np.max(np.abs(out - ref)) <= 1e-12 * np.abs(W0).sum() * psf_img.max()
+    assert abs(out.sum() - W0.sum()) <= 1e-12 * np.abs(W0).sum()     # a unit-flux PSF keeps the stamp's flux scale
+    p.destroy(); big.destroy()
