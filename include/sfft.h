@@ -109,6 +109,15 @@ sfft_status sfft_build_system(sfft_plan *plan, const double *S, const double *R,
  * next sfft_subtract with a host coefficient read).  Errors: STATE, CUDA. */
 sfft_status sfft_solve(sfft_plan *plan);
 
+/* f4 variant ("constant-photometric-ratio constraint (drops the sum-flux freedom of higher-order
+ * terms)"; reading R1 of DESIGN.md section 15): sfft_solve, then the solution is replaced by the least-squares solution
+ * subject to  sum_{u,v} a_{t,u,v} = 0  for every polynomial term t = 1..NK-1, so that the flux scaling sum_{u,v} K(u,v;x,y)
+ * is the same everywhere on the frame (term t = 0 and the background stay free).  Uses the factor of sfft_solve: NK-1
+ * more pairs of triangular solves and an (NK-1) x (NK-1) Schur system.  DK = 0: identical to sfft_solve.  Allocates
+ * 2 (NK-1) n doubles of plan workspace on first use.  sfft_subtract then uses the constrained coefficients.
+ * Errors: those of sfft_solve; ALLOC / CUDA. */
+sfft_status sfft_solve_constant_ratio(sfft_plan *plan);
+
 /* a5: D (device, ny*nx) = S - sum_t T_t (*) K_t - B using the solved coefficients;
  * coeffs (device, n doubles) receives them, or NULL.  Errors: STATE, INVALID_ARG, CUDA. */
 sfft_status sfft_subtract(sfft_plan *plan, double *D, double *coeffs);

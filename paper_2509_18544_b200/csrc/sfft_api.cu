@@ -74,7 +74,7 @@ static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
                     p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
-                    p->ywork, p->zwork, p->coef, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->ywork, p->zwork, p->coef, p->ratioEZ, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
@@ -373,6 +373,19 @@ sfft_status sfft_solve(sfft_plan *p) {
         CK(launch_trisolve(p, p->h, p->coef), "trisolve");
     }
     p->have_solution = true;
+    return SFFT_OK;
+}
+
+sfft_status sfft_solve_constant_ratio(sfft_plan *p) {
+    sfft_status st = sfft_solve(p);
+    if (st != SFFT_OK) return st;
+    const int m = p->g.NK - 1;
+    if (m < 1) return SFFT_OK; // DK = 0: nothing to constrain
+    if (!p->ratioEZ) CK(dalloc(p, &p->ratioEZ, (size_t)2 * m * p->g.n), "alloc constant-ratio workspace");
+    {
+        StageTimer tm(p, SFFT_STAGE_A4_SOLVE);
+        CK(launch_constant_ratio(p, p->ratioEZ, p->ratioEZ + (size_t)m * p->g.n, p->coef), "constant_ratio");
+    }
     return SFFT_OK;
 }
 

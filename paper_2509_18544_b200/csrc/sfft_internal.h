@@ -86,6 +86,7 @@ struct sfft_plan {
     double *ywork, *zwork;   // [n] forward / backward substitution vectors
     int solve_epoch;         // epoch tag of the flag-in-data exchange words of the triangular solves (ywork, zwork), one per solve
     double *coef;            // [n]   solved coefficients
+    double *ratioEZ;         // [2][NK-1][n] indicator right-hand sides and their solves (sfft_solve_constant_ratio; allocated on first use)
     sfft::cplx *E;           // [NK][L][Hx+1] kernel row tables for a5
     int *flag;               // device: 1 = pivot test failed
     int *flag_host;          // pinned mirror
@@ -153,6 +154,10 @@ cudaError_t launch_local_kernel(sfft_plan *p, const double *coef, double xt, dou
 // F: N*N doubles of scratch, bad: one int (raised when the noise power is not positive somewhere)
 cudaError_t launch_decorr(sfft_plan *p, const double *K, int Lk, const double *PS, const double *PR, int Lp,
                           double varS, double varR, int N, double *F, int *bad, double *stamp);
+
+// ---- f4 constant photometric ratio (sfft_ratio.cu) ---------------------------------------
+// c: free solution in, constrained solution out; E, Z: [NK-1][n] scratch each
+cudaError_t launch_constant_ratio(sfft_plan *p, double *E, double *Z, double *c);
 
 // ---- f3 (sfft_align.cu) ------------------------------------------------------------------
 // M: 6 host doubles (output pixel -> source position); method 0 nearest, 1 bilinear, 3 Lanczos-3
