@@ -17,7 +17,7 @@ roofline": 34 r of algorithmic bytes over the a1+a2+a3+a5 time), `stages_ms`, `k
 `batched` (configs[3]: template-side work once, per-science-image throughput), `cross_convolve`
 (f2: both PSF cross-convolutions of the pair, device time, 16 r of algorithmic bytes), `decorrelate`
 (f1: decorrelation stamp build + one application), `align` (f3: affine resampling of one
-frame and its mask), `stamp_mode`
+frame and its mask), `constant_ratio` (f4: the step under the constant-photometric-ratio constraint), `stamp_mode`
 (f4: the path on a 1000 x 1000 cut-out), `cpu_baseline`
 (the oracle on this box's host cores, bounded sample), `clocks`.
 
@@ -525,6 +525,33 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
                               "oracle_check_image_max_abs_err": float(np.max(np.abs(got - ref[w:crop - w, w:crop - w])))}
     except Exception as ex:  # pragma: no cover
         out["decorrelate"] = {"error": str(ex)}
+
+    # f4 variant: the same step with the constant-photometric-ratio solve (NK - 1 more triangular solves).
+    try:
+        oD = torch.empty_like(dS); oc = torch.empty(plan.n, dtype=torch.float64, device="cuda")
+
+        def rstep():
+            plan.build_system(dS, dR); plan.solve_constant_ratio(); plan.subtract(oD, oc)
+        for _ in range(3):
+            rstep()
+        plan.sync_status()
+        stream = torch.cuda.current_stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            rstep()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        plan.sync_status()
+        rms_ = e0.elapsed_time(e1) / K
+        LLb = cfg["L"] ** 2
+        sums = [float(oc[t * LLb:(t + 1) * LLb].sum()) for t in range(NK)]
+        out["constant_ratio"] = {"workload": "the headline step with sfft_solve_constant_ratio instead of sfft_solve",
+                                 "ms_per_step": round(rms_, 4), "images_per_s": round(1e3 / rms_, 1),
+                                 "tap_sums_per_term": sums}
+        step()                                   # leave the plan with the free solution
+    except Exception as ex:  # pragma: no cover
+        out["constant_ratio"] = {"error": str(ex)}
 
     # f4: "decrease the processed stamp size ... down to a minimum size of 1000 x 1000 px": the same path
     # on a contiguous 1000 x 1000 cut-out of the pair (a second, small plan; same L, DK, DB).
