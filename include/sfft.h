@@ -118,6 +118,13 @@ sfft_status sfft_solve(sfft_plan *plan);
  * Errors: those of sfft_solve; ALLOC / CUDA. */
 sfft_status sfft_solve_constant_ratio(sfft_plan *plan);
 
+/* The same constraint as a plan mode (on != 0): from now on EVERY solve of the plan -- sfft_solve, the per-image solves of
+ * sfft_subtract_batch, sfft_difference_host -- is followed by the constant-ratio correction.  The NK-1 auxiliary solves
+ * depend on the factor only: in this mode they are enqueued right behind the factorisation (on the plan's factor stream,
+ * beside the science-side kernels; once per template in the batched path) and each solve then costs one small
+ * correction kernel more.  Default: off.  Coefficients already solved are not changed.  Errors: INVALID_ARG (NULL plan). */
+sfft_status sfft_set_constant_ratio(sfft_plan *plan, int on);
+
 /* a5: D (device, ny*nx) = S - sum_t T_t (*) K_t - B using the solved coefficients;
  * coeffs (device, n doubles) receives them, or NULL.  Errors: STATE, INVALID_ARG, CUDA. */
 sfft_status sfft_subtract(sfft_plan *plan, double *D, double *coeffs);

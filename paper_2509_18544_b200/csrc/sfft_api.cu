@@ -250,6 +250,21 @@ const char *sfft_last_error(const sfft_plan *p) { return p ? p->err : "null plan
 // stage sequencing
 // ------------------------------------------------------------------------------------------
 
+// f4, constant photometric ratio: z_k = G^-1 e_k behind the factorisation on stream st (kept while the factor lives)
+static cudaError_t ratio_Z(sfft_plan *p, cudaStream_t st) {
+    const int m = p->g.NK - 1;
+    if (m < 1) { p->have_ratioZ = true; return cudaSuccess; }
+    if (!p->ratioEZ) { cudaError_t e = dalloc(p, &p->ratioEZ, (size_t)2 * m * p->g.n); if (e != cudaSuccess) return e; }
+    cudaError_t e = launch_ratio_Z(p, p->ratioEZ, p->ratioEZ + (size_t)m * p->g.n, st);
+    if (e == cudaSuccess) p->have_ratioZ = true;
+    return e;
+}
+static cudaError_t ratio_apply(sfft_plan *p, double *c, cudaStream_t st) {
+    const int m = p->g.NK - 1;
+    if (m < 1) return cudaSuccess;
+    return launch_ratio_apply(p, p->ratioEZ + (size_t)m * p->g.n, c, st);
+}
+
 // a1 (template), Omega, Gamma, G.  Needs p->R, p->mask set.
 static sfft_status template_side(sfft_plan *p) {
     const Geom &g = p->g;
@@ -345,6 +360,8 @@ sfft_status sfft_build_system(sfft_plan *p, const double *S, const double *R, co
         {
             StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
             CK(launch_factor(p), "factor");
+            p->have_ratioZ = false;
+            if (p->ratio_mode) CK(ratio_Z(p, p->cur), "constant-ratio solves");
         }
         back_to_main(p);
         p->have_factor = true;
@@ -366,27 +383,31 @@ sfft_status sfft_solve(sfft_plan *p) {
     if (!p->have_factor) {
         StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
         CK(launch_factor(p), "factor");
-        p->have_factor = true;
+        p->have_factor = true; p->have_ratioZ = false;
     }
     {
         StageTimer tm(p, SFFT_STAGE_A4_SOLVE);
+        if (p->ratio_mode && !p->have_ratioZ) CK(ratio_Z(p, p->stream), "constant-ratio solves");
         CK(launch_trisolve(p, p->h, p->coef), "trisolve");
+        if (p->ratio_mode) CK(ratio_apply(p, p->coef, p->stream), "constant-ratio correction");
     }
     p->have_solution = true;
     return SFFT_OK;
 }
 
-sfft_status sfft_solve_constant_ratio(sfft_plan *p) {
-    sfft_status st = sfft_solve(p);
-    if (st != SFFT_OK) return st;
-    const int m = p->g.NK - 1;
-    if (m < 1) return SFFT_OK; // DK = 0: nothing to constrain
-    if (!p->ratioEZ) CK(dalloc(p, &p->ratioEZ, (size_t)2 * m * p->g.n), "alloc constant-ratio workspace");
-    {
-        StageTimer tm(p, SFFT_STAGE_A4_SOLVE);
-        CK(launch_constant_ratio(p, p->ratioEZ, p->ratioEZ + (size_t)m * p->g.n, p->coef), "constant_ratio");
-    }
+sfft_status sfft_set_constant_ratio(sfft_plan *p, int on) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    p->ratio_mode = on != 0;
     return SFFT_OK;
+}
+
+sfft_status sfft_solve_constant_ratio(sfft_plan *p) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    const bool saved = p->ratio_mode;
+    p->ratio_mode = true;
+    const sfft_status st = sfft_solve(p);
+    p->ratio_mode = saved;
+    return st;
 }
 
 sfft_status sfft_subtract(sfft_plan *p, double *D, double *coeffs) {
@@ -507,6 +528,8 @@ sfft_status sfft_set_template(sfft_plan *p, const double *R, const uint8_t *mask
     {
         StageTimer tm(p, SFFT_STAGE_A4_FACTOR);
         CK(launch_factor(p), "factor");
+        p->have_ratioZ = false;
+        if (p->ratio_mode) CK(ratio_Z(p, p->cur), "constant-ratio solves");
     }
     p->have_template = true; p->have_factor = true;
     return SFFT_OK;
@@ -531,13 +554,17 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
             const int b0 = gsz * k, nimg = B - b0 < gsz ? B - b0 : gsz;
             return science_sideN(p, nimg, S + b0, p->hq + NSCI * (k & 1));
         };
+        if (p->ratio_mode && !p->have_ratioZ) CK(ratio_Z(p, p->stream), "constant-ratio solves");
         sfft_status rc = sci(0);
         if (rc == SFFT_OK) CK(cudaEventRecord(p->ev_ffork, p->stream), "event");
         for (int k = 0; k < ngrp && rc == SFFT_OK; k++) {
             const int b0 = gsz * k, nimg = B - b0 < gsz ? B - b0 : gsz, par = NSCI * (k & 1);
             cudaStreamWaitEvent(p->fstream, p->ev_ffork, 0);
             cudaError_t e = cudaSuccess;
-            for (int i = 0; i < nimg && e == cudaSuccess; i++) e = launch_trisolve(p, p->hq[par + i], p->cq[par + i], p->fstream);
+            for (int i = 0; i < nimg && e == cudaSuccess; i++) {
+                e = launch_trisolve(p, p->hq[par + i], p->cq[par + i], p->fstream);
+                if (e == cudaSuccess && p->ratio_mode) e = ratio_apply(p, p->cq[par + i], p->fstream);
+            }
             if (e == cudaSuccess) e = cudaEventRecord(p->ev_fjoin, p->fstream);
             CK(e, "trisolve (batch)");
             if (k + 1 < ngrp) {
@@ -571,7 +598,9 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
         p->have_system = true;
         {
             StageTimer tm(p, SFFT_STAGE_A4_SOLVE);
+            if (p->ratio_mode && !p->have_ratioZ) CK(ratio_Z(p, p->stream), "constant-ratio solves");
             CK(launch_trisolve(p, p->h, p->coef), "trisolve");
+            if (p->ratio_mode) CK(ratio_apply(p, p->coef, p->stream), "constant-ratio correction");
         }
         p->have_solution = true;
         {

@@ -96,6 +96,8 @@ struct sfft_plan {
     // state
     const double *S, *R; const uint8_t *mask;
     bool have_template, have_system, have_factor, have_solution;
+    bool ratio_mode;         // sfft_set_constant_ratio: every solve is followed by the constant-ratio correction
+    bool have_ratioZ;        // ratioEZ holds the z_k of the current factor
     int npairsO;
     sfft::PairList plO, plT;
     // timing
@@ -156,8 +158,10 @@ cudaError_t launch_decorr(sfft_plan *p, const double *K, int Lk, const double *P
                           double varS, double varR, int N, double *F, int *bad, double *stamp);
 
 // ---- f4 constant photometric ratio (sfft_ratio.cu) ---------------------------------------
-// c: free solution in, constrained solution out; E, Z: [NK-1][n] scratch each
-cudaError_t launch_constant_ratio(sfft_plan *p, double *E, double *Z, double *c);
+// E, Z: [NK-1][n] each: indicator right-hand sides and z_k = G^-1 e_k (factor only); apply: c free solution in,
+// constrained solution out
+cudaError_t launch_ratio_Z(sfft_plan *p, double *E, double *Z, cudaStream_t st);
+cudaError_t launch_ratio_apply(sfft_plan *p, const double *Z, double *c, cudaStream_t st);
 
 // ---- f3 (sfft_align.cu) ------------------------------------------------------------------
 // M: 6 host doubles (output pixel -> source position); method 0 nearest, 1 bilinear, 3 Lanczos-3

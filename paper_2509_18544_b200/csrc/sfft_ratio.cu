@@ -58,16 +58,25 @@ __global__ void __launch_bounds__(256) ratio_apply_kernel(const double *__restri
     }
 }
 
-// E, Z: [m][n] each (plan-owned).  c holds the free solution on entry and the constrained one on return.
-cudaError_t launch_constant_ratio(sfft_plan *p, double *E, double *Z, double *c) {
+// E, Z: [m][n] each (plan-owned).  z_k = G^-1 e_k on stream st: they depend on the factor only, so the caller runs them
+// right behind the factorisation (beside the science-side kernels) and keeps them for as long as the factor lives.
+cudaError_t launch_ratio_Z(sfft_plan *p, double *E, double *Z, cudaStream_t st) {
     const int n = p->g.n, LL = p->g.L * p->g.L, m = p->g.NK - 1;
     if (m < 1) return cudaSuccess;
-    { KLaunch kl(p, "ratio_rhs"); ratio_rhs_kernel<<<dim3((n + 255) / 256, m), 256, 0, p->stream>>>(E, n, LL); }
+    { KLaunch kl(p, "ratio_rhs"); ratio_rhs_kernel<<<dim3((n + 255) / 256, m), 256, 0, st>>>(E, n, LL); }
     for (int k = 0; k < m; k++) {
-        cudaError_t e = launch_trisolve(p, E + (size_t)k * n, Z + (size_t)k * n);
+        cudaError_t e = launch_trisolve(p, E + (size_t)k * n, Z + (size_t)k * n, st);
         if (e != cudaSuccess) return e;
     }
-    { KLaunch kl(p, "ratio_apply"); ratio_apply_kernel<<<1, 256, 0, p->stream>>>(Z, c, n, LL, m); }
+    return cudaGetLastError();
+}
+
+// c holds the free solution on entry and the constrained one on return
+cudaError_t launch_ratio_apply(sfft_plan *p, const double *Z, double *c, cudaStream_t st) {
+    const int n = p->g.n, LL = p->g.L * p->g.L, m = p->g.NK - 1;
+    if (m < 1) return cudaSuccess;
+    KLaunch kl(p, "ratio_apply");
+    ratio_apply_kernel<<<1, 256, 0, st>>>(Z, c, n, LL, m);
     return cudaGetLastError();
 }
 

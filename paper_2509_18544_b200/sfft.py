@@ -22,7 +22,7 @@ _STATUS = {0: "OK", -1: "INVALID_ARG", -2: "ALLOC", -3: "CUDA", -4: "STATE", -5:
 # every symbol include/sfft.h declares (tests check the library exports all of them)
 SYMBOLS = (
     "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
-    "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_solve_constant_ratio", "sfft_subtract", "sfft_subtract_with",
+    "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_solve_constant_ratio", "sfft_set_constant_ratio", "sfft_subtract", "sfft_subtract_with",
     "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_resample_affine", "sfft_resample_affine_mask", "sfft_local_kernel",
     "sfft_decorrelation_stamp", "sfft_difference_host", "sfft_sync_status",
     "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
@@ -59,6 +59,7 @@ def load_library():
     lib.sfft_build_system.argtypes = [vp, dp, dp, dp]
     lib.sfft_solve.argtypes = [vp]
     lib.sfft_solve_constant_ratio.argtypes = [vp]
+    lib.sfft_set_constant_ratio.argtypes = [vp, ci]
     lib.sfft_subtract.argtypes = [vp, dp, dp]
     lib.sfft_subtract_with.argtypes = [vp, dp, dp, dp]
     lib.sfft_convolve_stamp.argtypes = [vp, dp, dp, dp]
@@ -172,6 +173,10 @@ class SfftPlan:
 
     def solve(self):
         self._ck(self._lib.sfft_solve(self._h), "sfft_solve")
+
+    def set_constant_ratio(self, on=True):
+        """Plan mode: every solve (single, batched, host path) under the constant-ratio constraint (f4)."""
+        self._ck(self._lib.sfft_set_constant_ratio(self._h, 1 if on else 0), "sfft_set_constant_ratio")
 
     def solve_constant_ratio(self):
         """sfft_solve under the constant-photometric-ratio constraint (f4); see sfft_solve_constant_ratio."""
