@@ -531,7 +531,8 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
         oD = torch.empty_like(dS); oc = torch.empty(plan.n, dtype=torch.float64, device="cuda")
 
         def rstep():
-            plan.build_system(dS, dR); plan.solve_constant_ratio(); plan.subtract(oD, oc)
+            plan.build_system(dS, dR); plan.solve(); plan.subtract(oD, oc)
+        plan.set_constant_ratio(True)            # plan mode: the auxiliary solves run behind the factor, beside the science side
         for _ in range(3):
             rstep()
         plan.sync_status()
@@ -546,11 +547,13 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
         rms_ = e0.elapsed_time(e1) / K
         LLb = cfg["L"] ** 2
         sums = [float(oc[t * LLb:(t + 1) * LLb].sum()) for t in range(NK)]
-        out["constant_ratio"] = {"workload": "the headline step with sfft_solve_constant_ratio instead of sfft_solve",
+        plan.set_constant_ratio(False)
+        out["constant_ratio"] = {"workload": "the headline step in the sfft_set_constant_ratio(1) plan mode",
                                  "ms_per_step": round(rms_, 4), "images_per_s": round(1e3 / rms_, 1),
                                  "tap_sums_per_term": sums}
         step()                                   # leave the plan with the free solution
     except Exception as ex:  # pragma: no cover
+        plan.set_constant_ratio(False)
         out["constant_ratio"] = {"error": str(ex)}
 
     # f4: "decrease the processed stamp size ... down to a minimum size of 1000 x 1000 px": the same path
@@ -614,6 +617,24 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
                           "B": B, "template_ms": round(t_t, 3), "per_image_ms": round(t_b / B, 4),
                           "images_per_s": round(B * 1e3 / (t_t + t_b), 1),
                           "frac_of_measured_hbm": round(per_img_bytes / ((t_t + t_b) / B) / 1e6 / peak, 4)}
+        # the same batch in the constant-photometric-ratio plan mode (f4): auxiliary solves once per template
+        try:
+            plan.set_constant_ratio(True)
+            plan.set_template(dR); plan.subtract_batch(S_list[:2], D_arg[:2], cb[:2].contiguous())
+            torch.cuda.synchronize()
+            e[0].record(stream)
+            plan.set_template(dR)
+            e[1].record(stream)
+            plan.subtract_batch(S_list, D_arg, cb)
+            e[2].record(stream)
+            torch.cuda.synchronize()
+            plan.sync_status()
+            t_t2, t_b2 = e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
+            out["batched"]["constant_ratio_mode"] = {"template_ms": round(t_t2, 3), "per_image_ms": round(t_b2 / B, 4),
+                                                     "images_per_s": round(B * 1e3 / (t_t2 + t_b2), 1)}
+        except Exception as ex:  # pragma: no cover
+            out["batched"]["constant_ratio_mode"] = {"error": str(ex)}
+        plan.set_constant_ratio(False)
     return out
 
 
