@@ -74,7 +74,7 @@ static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
                     p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
-                    p->ywork, p->zwork, p->coef, p->ratioEZ, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->ywork, p->zwork, p->coef, p->ratioEZ, p->ratioW, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
@@ -96,6 +96,8 @@ static void free_plan(sfft_plan *p) {
     if (p->ev_copy) cudaEventDestroy(p->ev_copy);
     if (p->ev_fjoin) cudaEventDestroy(p->ev_fjoin);
     if (p->fstream2) cudaStreamDestroy(p->fstream2);
+    for (int k = 0; k < MAX_NP - 2; k++) { if (p->rstream[k]) cudaStreamDestroy(p->rstream[k]); if (p->ev_rjoin[k]) cudaEventDestroy(p->ev_rjoin[k]); }
+    if (p->ev_rfork) cudaEventDestroy(p->ev_rfork);
     if (p->ev_lookP) cudaEventDestroy(p->ev_lookP);
     if (p->ev_lookB) cudaEventDestroy(p->ev_lookB);
     for (int k = 0; k < MAX_KREC; k++)
@@ -255,7 +257,20 @@ static cudaError_t ratio_Z(sfft_plan *p, cudaStream_t st) {
     const int m = p->g.NK - 1;
     if (m < 1) { p->have_ratioZ = true; return cudaSuccess; }
     if (!p->ratioEZ) { cudaError_t e = dalloc(p, &p->ratioEZ, (size_t)2 * m * p->g.n); if (e != cudaSuccess) return e; }
-    cudaError_t e = launch_ratio_Z(p, p->ratioEZ, p->ratioEZ + (size_t)m * p->g.n, st);
+    if (m > 1 && !p->ratioW) { // first use: exchange words (epoch 0 never matches a solve), streams and events of the parallel solves
+        const size_t cnt = (size_t)(m - 1) * 4 * (size_t)(((p->g.n + 63) / 64) * 64);
+        cudaError_t e = dalloc(p, &p->ratioW, cnt);
+        if (e == cudaSuccess) e = cudaMemsetAsync(p->ratioW, 0, cnt * sizeof(double), st); // ordered before the fork event of the solves
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_rfork, cudaEventDisableTiming);
+        for (int k = 0; k < m - 1 && e == cudaSuccess; k++) {
+            int lo = 0, hi = 0;
+            cudaDeviceGetStreamPriorityRange(&lo, &hi);
+            e = cudaStreamCreateWithPriority(&p->rstream[k], cudaStreamNonBlocking, hi); // like the factor stream: latency chains go first
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_rjoin[k], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return e;
+    }
+    cudaError_t e = launch_ratio_Z(p, p->ratioEZ, p->ratioEZ + (size_t)m * p->g.n, st, p->ratioW);
     if (e == cudaSuccess) p->have_ratioZ = true;
     return e;
 }

@@ -98,6 +98,8 @@ struct sfft_plan {
     bool have_template, have_system, have_factor, have_solution;
     bool ratio_mode;         // sfft_set_constant_ratio: every solve is followed by the constant-ratio correction
     bool have_ratioZ;        // ratioEZ holds the z_k of the current factor
+    double *ratioW;          // [NK-2][2][2*ceil64(n)] exchange words of the auxiliary solves 2..NK-1, which run beside the first
+    cudaStream_t rstream[sfft::MAX_NP - 2]; cudaEvent_t ev_rfork, ev_rjoin[sfft::MAX_NP - 2];
     int npairsO;
     sfft::PairList plO, plT;
     // timing
@@ -143,7 +145,7 @@ cudaError_t launch_gather_h(sfft_plan *p, const double *lagT = nullptr, const do
 
 // ---- a4 (sfft_solve.cu) ------------------------------------------------------------------
 cudaError_t launch_factor(sfft_plan *p);                      // G -> dscale, Lf, flag
-cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream_t st = nullptr); // c = D (L^-T (L^-1 (D h))); st: default the plan's stream
+cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream_t st = nullptr, double *work = nullptr); // c = D (L^-T (L^-1 (D h))); st: default the plan's stream; work: own exchange words [2][2*ceil64(n)] (zeroed once) for a solve that runs beside another one, default the plan's
 
 // ---- a5 (sfft_subtract.cu) ---------------------------------------------------------------
 // spec: the NK spectra to convolve (default: the plan's unmasked template spectra); mode 0: D = S - M - B,
@@ -160,7 +162,7 @@ cudaError_t launch_decorr(sfft_plan *p, const double *K, int Lk, const double *P
 // ---- f4 constant photometric ratio (sfft_ratio.cu) ---------------------------------------
 // E, Z: [NK-1][n] each: indicator right-hand sides and z_k = G^-1 e_k (factor only); apply: c free solution in,
 // constrained solution out
-cudaError_t launch_ratio_Z(sfft_plan *p, double *E, double *Z, cudaStream_t st);
+cudaError_t launch_ratio_Z(sfft_plan *p, double *E, double *Z, cudaStream_t st, double *W);
 cudaError_t launch_ratio_apply(sfft_plan *p, const double *Z, double *c, cudaStream_t st);
 
 // ---- f3 (sfft_align.cu) ------------------------------------------------------------------

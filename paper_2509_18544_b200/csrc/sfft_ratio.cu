@@ -60,13 +60,22 @@ __global__ void __launch_bounds__(256) ratio_apply_kernel(const double *__restri
 
 // E, Z: [m][n] each (plan-owned).  z_k = G^-1 e_k on stream st: they depend on the factor only, so the caller runs them
 // right behind the factorisation (beside the science-side kernels) and keeps them for as long as the factor lives.
-cudaError_t launch_ratio_Z(sfft_plan *p, double *E, double *Z, cudaStream_t st) {
+// The m solves are independent: solve 0 stays on st with the plan's exchange words, solves 1..m-1 run beside it on the
+// plan's auxiliary streams with exchange words of their own (W; each is a 12-CTA latency chain, so five in parallel take
+// about as long as one).  In per-launch timing mode everything stays on st.
+cudaError_t launch_ratio_Z(sfft_plan *p, double *E, double *Z, cudaStream_t st, double *W) {
     const int n = p->g.n, LL = p->g.L * p->g.L, m = p->g.NK - 1;
     if (m < 1) return cudaSuccess;
+    const size_t wsz = 2 * (size_t)(((n + 63) / 64) * 64);
+    const bool par = W && !p->ktiming && p->rstream[0];
     { KLaunch kl(p, "ratio_rhs"); ratio_rhs_kernel<<<dim3((n + 255) / 256, m), 256, 0, st>>>(E, n, LL); }
+    if (par) cudaEventRecord(p->ev_rfork, st);
     for (int k = 0; k < m; k++) {
-        cudaError_t e = launch_trisolve(p, E + (size_t)k * n, Z + (size_t)k * n, st);
+        cudaStream_t sk = (par && k > 0) ? p->rstream[k - 1] : st;
+        if (par && k > 0) cudaStreamWaitEvent(sk, p->ev_rfork, 0);
+        cudaError_t e = launch_trisolve(p, E + (size_t)k * n, Z + (size_t)k * n, sk, (par && k > 0) ? W + (size_t)(k - 1) * 2 * wsz : nullptr);
         if (e != cudaSuccess) return e;
+        if (par && k > 0) { cudaEventRecord(p->ev_rjoin[k - 1], sk); cudaStreamWaitEvent(st, p->ev_rjoin[k - 1], 0); }
     }
     return cudaGetLastError();
 }

@@ -537,11 +537,12 @@ cudaError_t launch_factor(sfft_plan *p) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream_t st) {
+cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream_t st, double *work) {
     const int n = p->g.n, nblk = (n + CB - 1) / CB;
     p->solve_epoch++;
     const double *Lf = p->Lf, *Li = p->Linv, *ds = p->dscale;
-    unsigned long long *y = reinterpret_cast<unsigned long long *>(p->ywork), *z = reinterpret_cast<unsigned long long *>(p->zwork);
+    const size_t wsz = 2 * (size_t)(((n + 63) / 64) * 64); // exchange words of one substitution (sfft_plan_create)
+    unsigned long long *y = reinterpret_cast<unsigned long long *>(work ? work : p->ywork), *z = reinterpret_cast<unsigned long long *>(work ? work + wsz : p->zwork);
     int *err = p->flag, epoch = p->solve_epoch, nn = n;
     void *args[] = {(void *)&Lf, (void *)&Li, (void *)&ds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&err, (void *)&epoch};
     KLaunch kl(p, "trisolve");
