@@ -76,10 +76,15 @@ enum {
     SFFT_NUM_STAGES = 8
 };
 
+#define SFFT_MAX_SIDE 4096
+
 /* Create a plan for nx x ny frames, L x L kernel (L odd, 1 <= L <= 21), polynomial degrees
- * DK, DB (0 <= DK, DB <= 3).  Requires 2L-1 <= nx, ny <= 8192.  Frames are zero-padded
- * internally to the next powers of two (>= 64); any nx, ny in range is supported,
- * including 256, 1024 and 4088.  Allocates every workspace; uses the
+ * DK, DB (0 <= DK, DB <= 3).  Requires 2L-1 <= nx, ny <= SFFT_MAX_SIDE (4096: the Roman
+ * detector frame is 4088 x 4088).  Frames are zero-padded internally to powers
+ * of two (at least 1024 x 512) and the sums that wrap differently on the padded grid are
+ * corrected exactly, so any nx, ny in range is supported, including 256, 1024 and 4088.
+ * Allocates every workspace (nothing is allocated later except the second set of template
+ * spectra on the first call with a mask and the host-path staging buffers); uses the
  * current CUDA device and the legacy default stream until sfft_plan_set_stream.
  * Errors: INVALID_ARG, ALLOC, CUDA (no usable device). */
 sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int DB);
@@ -257,7 +262,7 @@ const char *sfft_last_error(const sfft_plan *plan);
 const char *sfft_version(void);
 
 /* Test hook: copies an internal device array to a HOST buffer (synchronises).
- *   which = 0: template spectrum t=idx  (My x Hx complex128, column 0 = DC + i*Nyquist packed)
+ *   which = 0: template spectrum t=idx  (My x (Hx+1) complex128, row-major [ky][kx], kx = 0..Hx = Mx/2)
  *           1: science spectrum
  *           2: Omega lag table of pair idx ((4w+1)^2 doubles, [dv+2w][du+2w])
  *           3: Theta lag table of t=idx (L*L doubles)

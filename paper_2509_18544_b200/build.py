@@ -16,9 +16,8 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libsfft.so"
-SOURCES = ["sfft_api.cu", "sfft_fwd.cu", "sfft_lags.cu", "sfft_border.cu", "sfft_assemble.cu", "sfft_solve.cu",
-           "sfft_subtract.cu", "sfft_colpipe.cu", "sfft_decorr.cu", "sfft_align.cu", "sfft_ratio.cu",
-           "sfft_probe.cu"]
+SOURCES = ["sfft_api.cu", "sfft_rows.cu", "sfft_cols.cu", "sfft_lags.cu", "sfft_border.cu", "sfft_assemble.cu",
+           "sfft_solve.cu", "sfft_subtract.cu", "sfft_decorr.cu", "sfft_align.cu", "sfft_ratio.cu", "sfft_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

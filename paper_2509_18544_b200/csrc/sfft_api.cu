@@ -73,12 +73,13 @@ struct StageTimer {
 static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
-                    p->Q, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
+                    p->Q, p->phO, p->phT, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
                     p->ywork, p->zwork, p->coef, p->ratioEZ, p->ratioW, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
     if (p->flag_host) cudaFreeHost(p->flag_host);
+    lags_free(p);
     for (int s = 0; s < SFFT_NUM_STAGES; s++) {
         if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
         if (p->ev1[s]) cudaEventDestroy(p->ev1[s]);
@@ -113,7 +114,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     if (!out) return SFFT_ERR_INVALID_ARG;
     *out = nullptr;
     if (L < 1 || L > MAX_L || !(L & 1) || DK < 0 || DK > MAX_DEG || DB < 0 || DB > MAX_DEG) return SFFT_ERR_INVALID_ARG;
-    if (nx < 2 * L - 1 || ny < 2 * L - 1 || nx > 8192 || ny > 8192) return SFFT_ERR_INVALID_ARG;
+    if (nx < 2 * L - 1 || ny < 2 * L - 1 || nx > SFFT_MAX_SIDE || ny > SFFT_MAX_SIDE) return SFFT_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return SFFT_ERR_CUDA; }
     sfft_plan *p = new (std::nothrow) sfft_plan();
@@ -122,7 +123,9 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     Geom &g = p->g;
     g.nx = nx; g.ny = ny; g.L = L; g.w = (L - 1) / 2; g.DK = DK; g.DB = DB;
     g.NK = (DK + 1) * (DK + 2) / 2; g.NB = (DB + 1) * (DB + 2) / 2; g.n = L * L * g.NK + g.NB;
-    g.Mx = next_pow2(nx, 64); g.My = next_pow2(ny, 64); g.Hx = g.Mx / 2;
+    // zero-padded FFT grid: powers of two, at least 1024 x 512 (the transforms run 16 values per thread in groups of
+    // at least one warp; a small frame only pays a few MB of padding, the wrap corrections make any padding exact)
+    g.Mx = next_pow2(nx, 1024); g.My = next_pow2(ny, 512); g.Hx = g.Mx / 2;
     g.log2Hx = ilog2(g.Hx); g.log2My = ilog2(g.My);
     g.Nt = g.Mx > g.My ? g.Mx : g.My;
     for (int t = 0; t < MAX_NP; t++) poly_index(t, &g.pi[t], &g.pj[t]);
@@ -134,22 +137,39 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     for (int t = 0; t < g.NK; t++) { p->plT.a[t] = t; p->plT.b[t] = g.NK; }
     p->npairsO = p->plO.np;
 
-    const size_t plane = (size_t)g.My * g.Hx;
+    const size_t iplane = (size_t)g.My * g.Hx, splane = (size_t)g.My * (g.Hx + 1);
     const int W2 = 4 * g.w + 1, n = g.n;
-    LagCfg cO, cT; lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &cO); lagcol_config(g, p->plT.np, g.NK + 1, g.w, &cT, 16);
-    const size_t qO = (size_t)cO.nsplit * p->plO.np * W2 * (g.Hx + 1), qT = (size_t)cT.nsplit * NSCI * p->plT.np * L * (g.Hx + 1); // NSCI science images per pass
+    {   // experiment knobs: the environment is read here and nowhere else
+        Knobs &k = p->knob;
+        k.no_side = getenv("SFFT_NO_SIDE") != nullptr;
+        k.no_factor_overlap = getenv("SFFT_NO_FACTOR_OVERLAP") != nullptr;
+        k.no_batch_pipe = getenv("SFFT_NO_BATCH_PIPE") != nullptr;
+        k.no_lookahead = getenv("SFFT_NO_LOOKAHEAD") != nullptr;
+        const char *e = getenv("SFFT_BATCH_GROUP"); k.batch_group = e ? atoi(e) : NSCI;
+        if (k.batch_group < 1 || k.batch_group > NSCI) k.batch_group = NSCI;
+        e = getenv("SFFT_FACTOR_SMS"); k.factor_sms = e ? atoi(e) : 12;
+        int dev = 0; cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || p->sms <= 0) p->sms = 148;
+    }
+    // lag-pass launch shapes first: they size Q
+    lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &p->cfgO);
+    for (int k = 1; k <= NSCI; k++) lagcol_config(g, k * g.NK, g.NK + k, g.w, &p->cfgT[k - 1]);
     size_t bO = (size_t)border_chunks() * p->plO.np * W2 * W2;
     { const size_t bT2 = (size_t)border_chunks() * NSCI * g.NK * L * L; if (bT2 > bO) bO = bT2; }
     cudaError_t e = cudaSuccess;
 #define AL(ptr, cnt) if (e == cudaSuccess) e = dalloc(p, &ptr, (size_t)(cnt))
     AL(p->tw, g.Nt);
-    AL(p->inter, (size_t)(DK + 1) * g.ny * g.Hx);
-    AL(p->specT, g.NK * plane);
-    AL(p->specS, plane);
+    AL(p->inter, (size_t)(DK + 1) * iplane);
+    AL(p->specT, g.NK * splane);
+    AL(p->specS, splane);
+    p->specSx[0] = p->specS;
+    for (int i = 1; i < NSCI; i++) AL(p->specSx[i], splane); // batched path: up to NSCI science spectra per Theta pass
     AL(p->muR, (size_t)(DK + DB + 1) * ny);
     AL(p->muS, (size_t)(DB + 1) * ny);
     for (int i = 1; i < NSCI; i++) AL(p->muSx[i], (size_t)(DB + 1) * ny);
-    AL(p->Q, qO > qT ? qO : qT);
+    AL(p->Q, lag_q_elems(p));
+    AL(p->phO, (size_t)(g.My / 16) * p->cfgO.WB);
+    AL(p->phT, (size_t)(g.My / 16) * p->cfgT[0].WB);
     AL(p->lagO, (size_t)p->plO.np * W2 * W2);
     AL(p->lagT, (size_t)NSCI * g.NK * L * L);
     AL(p->bpart, bO);
@@ -173,19 +193,18 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     AL(p->coef, n);
     for (int i = 1; i < 2 * NSCI; i++) { AL(p->hq[i], n); AL(p->cq[i], n); }
     AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
-    AL(p->flag, 1);
+    AL(p->flag, 2);   // [0] pivot test failed (factorisation), [1] triangular-solve error
 #undef AL
     p->specTo = p->specT;
-    if (e == cudaSuccess) e = cudaMallocHost((void **)&p->flag_host, sizeof(int));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&p->flag_host, 2 * sizeof(int));
     if (e != cudaSuccess) {
         const bool oom = (e == cudaErrorMemoryAllocation);
         cudaGetLastError(); free_plan(p);
         return oom ? SFFT_ERR_ALLOC : SFFT_ERR_CUDA;
     }
-    *p->flag_host = 0;
+    p->flag_host[0] = p->flag_host[1] = 0;
     for (int s = 0; s < SFFT_NUM_STAGES; s++) { cudaEventCreate(&p->ev0[s]); cudaEventCreate(&p->ev1[s]); }
     p->stream = 0; p->cur = 0;
-    p->no_side = getenv("SFFT_NO_SIDE") != nullptr;
     cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
     cudaStreamCreateWithFlags(&p->sideB, cudaStreamNonBlocking);
     cudaStreamCreateWithFlags(&p->sideC, cudaStreamNonBlocking);
@@ -211,13 +230,17 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     cudaEventCreateWithFlags(&p->ev_lookP, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_lookB, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
+    e = rows_init();
+    if (e == cudaSuccess) e = cols_init();
+    if (e == cudaSuccess) e = lags_init(p);   // tensor maps over the spectra, phase tables (after the twiddles)
+    if (e != cudaSuccess) { cudaGetLastError(); free_plan(p); return SFFT_ERR_CUDA; }
     // Phi (pin P7): closed form, mask independent
     double phi[MAX_NP * MAX_NP];
     for (int s = 0; s < g.NB; s++)
         for (int s2 = 0; s2 < g.NB; s2++)
             phi[s * g.NB + s2] = power_sum(nx, g.pi[s] + g.pi[s2]) * power_sum(ny, g.pj[s] + g.pj[s2]);
     e = cudaMemcpy(p->phi, phi, sizeof(double) * g.NB * g.NB, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemset(p->flag, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(p->flag, 0, 2 * sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(p->ywork, 0, sizeof(double) * 2 * (size_t)(((n + 63) / 64) * 64)); // epoch 0 never matches a solve
     if (e == cudaSuccess) e = cudaMemset(p->zwork, 0, sizeof(double) * 2 * (size_t)(((n + 63) / 64) * 64));
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -285,8 +308,8 @@ static sfft_status template_side(sfft_plan *p) {
     const Geom &g = p->g;
     {
         StageTimer tm(p, SFFT_STAGE_A1_TEMPLATE);
-        if (p->mask && p->specTo == p->specT) { // the subtraction needs spectra of the UNMASKED template (C7)
-            CK(dalloc(p, &p->specTo, (size_t)g.NK * g.My * g.Hx), "alloc unmasked spectra");
+        if (p->mask && p->specTo == p->specT) { // the subtraction needs spectra of the UNMASKED template (C7): allocated with the first mask
+            CK(dalloc(p, &p->specTo, (size_t)g.NK * g.My * (g.Hx + 1)), "alloc unmasked spectra");
         }
         if (p->mask) {
             CK(launch_row_fwd(p, p->R, nullptr, p->inter, g.DK + 1, nullptr, 0), "row_fwd(R unmasked)");
@@ -336,10 +359,9 @@ static sfft_status science_side(sfft_plan *p) {
 // group ((NK + nimg)/nimg r per image instead of (NK + 1) r).  Results: hout[i].
 static sfft_status science_sideN(sfft_plan *p, int nimg, const double *const *S, double *const *hout) {
     const Geom &g = p->g;
-    p->specSx[0] = p->specS; p->muSx[0] = p->muS; p->deltax[0] = p->delta;
+    p->muSx[0] = p->muS; p->deltax[0] = p->delta;
     const int i0 = 0, j0 = 0;
     for (int i = 0; i < nimg; i++) {
-        if (!p->specSx[i]) CK(dalloc(p, &p->specSx[i], (size_t)g.My * g.Hx), "alloc science spectrum");
         p->Sx[i] = S[i];
         CK(launch_row_fwd(p, S[i], p->mask, p->inter, 1, p->muSx[i], g.DB + 1), "row_fwd(S)");
         CK(launch_col_fwd(p, p->inter, p->specSx[i], 1, &i0, &j0), "col_fwd(S)");
@@ -368,7 +390,7 @@ sfft_status sfft_build_system(sfft_plan *p, const double *S, const double *R, co
     p->have_template = p->have_system = p->have_factor = p->have_solution = false;
     sfft_status st = template_side(p);
     if (st != SFFT_OK) return st;
-    if (!p->ktiming && p->fstream && !getenv("SFFT_NO_FACTOR_OVERLAP")) {
+    if (!p->ktiming && p->fstream && !p->knob.no_factor_overlap) {
         // G depends on the template only: factor it (a4) on its own stream while the science side (a1, Theta)
         // runs on the caller's stream; sfft_solve joins.
         fork_factor(p);
@@ -518,7 +540,7 @@ sfft_status sfft_decorrelation_stamp(sfft_plan *p, const double *K, int Lk, cons
     if (N > 1024 || N < Lk + Lp - 1 || N < Lp || N < p->g.L) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: need max(Lk + Lp - 1, L) <= N <= 1024");
     if (!(var_S >= 0.0) || !(var_R >= 0.0) || !(var_S + var_R > 0.0) || var_S + var_R > 1.7e308)
         return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: variances must be finite, >= 0 and not both 0");
-    const size_t have = (size_t)(p->g.DK + 1) * p->g.ny * p->g.Hx * sizeof(cplx), need = ((size_t)N * N + 1) * sizeof(double);
+    const size_t have = (size_t)(p->g.DK + 1) * p->g.My * p->g.Hx * sizeof(cplx), need = ((size_t)N * N + 1) * sizeof(double);
     if (need > have) return fail(p, SFFT_ERR_INVALID_ARG, "decorrelation_stamp: N x N grid does not fit the plan's intermediate buffer");
     join_factor(p);
     back_to_main(p);
@@ -555,15 +577,15 @@ sfft_status sfft_subtract_batch(sfft_plan *p, const double *const *S, int B, dou
     if (!p->have_template || !p->have_factor) return fail(p, SFFT_ERR_STATE, "subtract_batch before set_template");
     if (!S || !D || B < 1) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: bad arguments");
     for (int b = 0; b < B; b++) if (!S[b] || !D[b]) return fail(p, SFFT_ERR_INVALID_ARG, "subtract_batch: NULL image");
-    if (B > 1 && !p->timing && !p->ktiming && p->fstream && !getenv("SFFT_NO_BATCH_PIPE")) {
+    join_factor(p); // the factor may come from sfft_build_system's overlap path and still be in flight on the factor stream
+    if (B > 1 && !p->timing && !p->ktiming && p->fstream && !p->knob.no_batch_pipe) {
         // Groups of up to NSCI images per science-side pass (science_sideN), and a software pipeline over the groups: the
         // triangular solves of group k (latency-bound launches that leave the machine empty) run on the factor stream
         // beside the science-side kernels of group k+1.  Order on the main stream: sci(0), [sci(1), a5(group 0)],
         // [sci(2), a5(group 1)], ...  h and the coefficients are buffered per (group parity, image); the solves of group
         // k+2 start after sci(k+2), which is behind a5(group k) on the main stream, so no buffer is overwritten while in use.
         p->hq[0] = p->h; p->cq[0] = p->coef;
-        static int gsz = 0;
-        if (!gsz) { const char *e = getenv("SFFT_BATCH_GROUP"); gsz = e ? atoi(e) : NSCI; if (gsz < 1 || gsz > NSCI) gsz = NSCI; }
+        const int gsz = p->knob.batch_group;
         const int ngrp = (B + gsz - 1) / gsz;
         auto sci = [&](int k) -> sfft_status {
             const int b0 = gsz * k, nimg = B - b0 < gsz ? B - b0 : gsz;
@@ -634,9 +656,12 @@ sfft_status sfft_sync_status(sfft_plan *p) {
     CK(cudaStreamSynchronize(p->stream), "sync");
     if (p->side) { CK(cudaStreamSynchronize(p->side), "sync side"); CK(cudaStreamSynchronize(p->sideB), "sync side"); CK(cudaStreamSynchronize(p->sideC), "sync side"); }
     if (p->have_factor) {
-        CK(cudaMemcpy(p->flag_host, p->flag, sizeof(int), cudaMemcpyDeviceToHost), "read flag");
-        if (*p->flag_host == 3) return fail(p, SFFT_ERR_CUDA, "triangular solve: a solution block never arrived");
-        if (*p->flag_host) return fail(p, SFFT_ERR_NOT_SPD, "pivot <= 1e-12: matrix not positive definite");
+        CK(cudaMemcpy(p->flag_host, p->flag, 2 * sizeof(int), cudaMemcpyDeviceToHost), "read flag");
+        if (p->flag_host[1]) {   // the coefficients of that solve are NaN (sfft_solve.cu: ll_load); clear so the plan stays usable
+            CK(cudaMemset(p->flag + 1, 0, sizeof(int)), "clear solve flag");
+            return fail(p, SFFT_ERR_CUDA, "triangular solve: a solution block never arrived");
+        }
+        if (p->flag_host[0]) return fail(p, SFFT_ERR_NOT_SPD, "pivot <= 1e-12: matrix not positive definite");
     }
     return SFFT_OK;
 }
@@ -724,12 +749,12 @@ sfft_status sfft_get_timings(sfft_plan *p, float *ms, int n_stages) {
 sfft_status sfft_debug_read(sfft_plan *p, int which, int idx, void *host_dst, size_t nbytes) {
     if (!p || !host_dst) return SFFT_ERR_INVALID_ARG;
     const Geom &g = p->g;
-    const size_t plane = (size_t)g.My * g.Hx * sizeof(cplx);
+    const size_t plane = (size_t)g.My * (g.Hx + 1) * sizeof(cplx);
     const int W2 = 4 * g.w + 1, LL = g.L * g.L;
     const void *src = nullptr; size_t sz = 0;
     double dims[2] = {(double)g.Mx, (double)g.My};
     switch (which) {
-    case 0: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->specT + (size_t)idx * g.My * g.Hx; sz = plane; break;
+    case 0: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->specT + (size_t)idx * g.My * (g.Hx + 1); sz = plane; break;
     case 1: src = p->specS; sz = plane; break;
     case 2: if (idx < 0 || idx >= p->npairsO) return SFFT_ERR_INVALID_ARG; src = p->lagO + (size_t)idx * W2 * W2; sz = sizeof(double) * W2 * W2; break;
     case 3: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->lagT + (size_t)idx * LL; sz = sizeof(double) * LL; break;
@@ -741,13 +766,13 @@ sfft_status sfft_debug_read(sfft_plan *p, int which, int idx, void *host_dst, si
     }
     if (nbytes != sz) return fail(p, SFFT_ERR_INVALID_ARG, "debug_read: size mismatch");
     CK(cudaStreamSynchronize(p->stream), "sync");
-    if (which <= 1) { // spectra are tile-major on the device (spec_idx): hand them out as [My][Hx]
+    if (which <= 1) { // spectra are column-major on the device (plane_idx): hand them out as [My][Hx+1]
         cplx *tmp = (cplx *)malloc(sz);
         if (!tmp) return fail(p, SFFT_ERR_ALLOC, "debug_read: host allocation failed");
         cudaError_t e = cudaMemcpy(tmp, src, sz, cudaMemcpyDeviceToHost);
         if (e == cudaSuccess)
             for (int ky = 0; ky < g.My; ky++)
-                for (int kx = 0; kx < g.Hx; kx++) ((cplx *)host_dst)[(size_t)ky * g.Hx + kx] = tmp[spec_idx(ky, kx, g.My)];
+                for (int kx = 0; kx <= g.Hx; kx++) ((cplx *)host_dst)[(size_t)ky * (g.Hx + 1) + kx] = tmp[plane_idx(ky, kx, g.My)];
         free(tmp);
         CK(e, "debug copy");
         return SFFT_OK;

@@ -1,20 +1,19 @@
-// sfft_fft.cuh -- register/shared-memory Stockham FFT building blocks (FP64 complex).
+// sfft_fft.cuh -- building blocks of the FP64 Stockham FFTs of libsfft (steps a1 and a5) and of the
+// asynchronous staging (bulk copies completing on mbarriers) that feeds the column and lag kernels.
 //
-// One power-of-two FFT of length N (32 <= N <= 8192) is computed by T = N/16 threads.
-// Every thread holds 16 complex values v[0..15] in registers.  "Canonical" register
-// layout: thread j holds elements j + q*T, q = 0..15.  A pass of radix R (16, or the
-// remaining factor 2/4/8 in the last pass) does 16/R butterflies per thread straight from
-// the canonical layout, scatters the results into shared memory at the Stockham
-// (autosort) positions, and after a barrier the next pass reloads the canonical layout.
-// The last pass leaves its results canonical in registers (natural order: v[q] is
-// element j + q*T), so the caller stores them wherever it wants (global memory for
-// column passes, shared memory for the real<->complex untangle of row passes).
+// One power-of-two transform of length N (512 <= N <= 4096) is computed by T = N/16 threads, 16 complex
+// values per thread in registers.  "Canonical" register layout: thread j holds elements j + q T,
+// q = 0..15.  A Stockham (autosort) pass of radix R (R | 16) does 16/R butterflies per thread straight from
+// the canonical layout -- butterfly jb = j + b T takes elements jb + m N/R, m < R -- and scatters the results
+// into a shared-memory exchange buffer at position (jb div Ns) Ns R + (jb mod Ns) + m Ns, Ns = product of the
+// radices of the earlier passes; after a barrier the next pass reloads the canonical layout.  The last pass
+// leaves natural order in registers (v[q] = element j + q T).
 //
-// Shared-memory indices are padded by one element per 16 (phys = i + i/16) so that the
-// stride-16 scatter of the first pass is bank-conflict free for 16-byte accesses.
-//
-// The functions are __host__ __device__ so that the index arithmetic can be exercised on
-// the CPU by tests (tests/test_fft_host.py builds a host emulation of the passes).
+// Exchange buffers hold 16-byte elements at XOR-swizzled positions (no padding: the column kernels need the
+// 64 KB of a 4096-point column to be exactly 64 KB so that two workers and their staging rings fit one SM):
+//   swz<LR0>(i) = i ^ ((i >> LR0) & (2^LR0 - 1)),  2^LR0 = radix of the FIRST pass,
+// which spreads the stride-R scatter of the first pass over all banks; every later pass and every canonical
+// reload touches runs of >= 8 consecutive elements, which a constant XOR only permutes.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -36,15 +35,13 @@ SFFT_HD cplx cscale(cplx a, double s) { return mk(a.x * s, a.y * s); }
 // multiply by DIR*i  (W4 = exp(DIR*2*pi*i/4))
 template <int DIR> SFFT_HD cplx mul_w4(cplx a) { return DIR > 0 ? mk(-a.y, a.x) : mk(a.y, -a.x); }
 
-// Spectra are stored TILE-MAJOR: column tiles of 2 adjacent kx, rows contiguous inside a tile,
-//   element (ky, kx) of a My x Hx spectrum  ->  ((kx >> 1) * My + ky) * 2 + (kx & 1).
-// The column pass then writes (and the subtraction reads) whole 128-byte lines -- scattered 32-byte
-// sector stores of the row-major layout ran at a quarter of the line-store rate -- and the lag pass
-// still finds the two columns of a tile in one 32-byte sector.
-SFFT_HD size_t spec_idx(int ky, int kx, int My) { return ((size_t)(kx >> 1) * My + ky) * 2 + (kx & 1); }
+// Planes (row-transformed intermediates and spectra) are stored COLUMN-MAJOR: element (ky, kx) of a plane with
+// My rows at kx * My + ky, so a column is one contiguous run (bulk copies, coalesced 16-byte accesses along ky).
+// Intermediates have Hx columns (column 0 = X[0] + i X[Hx], both real along x); spectra have Hx + 1 true columns
+// kx = 0..Hx (the forward column pass separates the packed column once, sfft_cols.cu).
+SFFT_HD size_t plane_idx(int ky, int kx, int My) { return (size_t)kx * My + ky; }
 
-SFFT_HD int pad16(int i) { return i + (i >> 4); }
-SFFT_HD int padded_len(int N) { return N + (N >> 4); }
+template <int LR0> SFFT_HD int swz(int i) { return i ^ ((i >> LR0) & ((1 << LR0) - 1)); }
 
 template <int DIR> SFFT_HD void dft2(cplx &a0, cplx &a1) {
     cplx t = a0; a0 = cadd(t, a1); a1 = csub(t, a1);
@@ -134,179 +131,117 @@ template <int R> SFFT_HD void twiddle_powers(cplx *x, cplx w1) {
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// Generic form: E values per thread (E = 8 or 16), T = N/E threads per transform.  Canonical layout:
-// thread j holds elements j + q*T, q = 0..E-1.  Shared-memory indices are padded by one element per E
-// (phys = i + i/E) so that the stride-E scatter of the first pass is bank-conflict free.
-// ---------------------------------------------------------------------------------------------
-template <int E> SFFT_HD int padE(int i) { return i + i / E; }
-template <int E> SFFT_HD int padded_lenE(int N) { return N + N / E; }
+__host__ __device__ constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
 
-// One Stockham pass of radix R (R divides E) on the canonical registers of thread j.
-//   Ns = product of the radices of earlier passes (log2Ns given), tw[k] = exp(-2 pi i k/Nt).
-// STORE: results go to shared memory s (padded) at their autosort positions; otherwise (last pass)
-// they stay canonical in v.
-template <int E, int R, int DIR, bool STORE>
-SFFT_HD void fft_passE(cplx *v, cplx *s, int j, int T, int log2Ns, const cplx *tw, int Nt) {
-    constexpr int NBF = E / R; // butterflies per thread
-    constexpr int LOG2R = (R == 16) ? 4 : (R == 8) ? 3 : (R == 4) ? 2 : 1;
-    const int Ns = 1 << log2Ns;
+#ifdef __CUDACC__
+// ---------------------------------------------------------------------------------------------
+// passes (device).  X: exchange buffer of 16-byte elements; IL rows are interleaved element by element
+// (IL = 2 in the row kernels, where lane parity selects one of two image rows; 1 in the column kernels),
+// r = this thread's row.  tw[k] = exp(-2 pi i k / Nt), Nt >= N a power of two.
+// ---------------------------------------------------------------------------------------------
+
+// twiddle (by w^m, w = exp(DIR 2 pi i (jb mod Ns) / (Ns R))) and DFT of one radix-R butterfly
+template <int R, int DIR>
+__device__ __forceinline__ void bfly(cplx *x, int jb, int log2Ns, const cplx *__restrict__ tw, int Nt) {
+    constexpr int LOG2R = ilog2c(R);
+    if (log2Ns > 0) {
+        cplx w1 = tw[(size_t)(jb & ((1 << log2Ns) - 1)) * (Nt >> (log2Ns + LOG2R))];
+        if (DIR > 0) w1.y = -w1.y;
+        twiddle_powers<R>(x, w1);
+    }
+    dftR<R, DIR>(x);
+}
+
+// the same with the butterfly's base twiddle given (persistent kernels keep it in a register: for a pass with one
+// butterfly per thread it depends on the thread only)
+template <int R, int DIR>
+__device__ __forceinline__ void bfly_w(cplx *x, cplx w1) {
+    if (DIR > 0) w1.y = -w1.y;
+    twiddle_powers<R>(x, w1);
+    dftR<R, DIR>(x);
+}
+
+// exchange-buffer position of output m of butterfly jb
+template <int R, int LR0>
+__device__ __forceinline__ int out_pos(int jb, int m, int log2Ns) {
+    constexpr int LOG2R = ilog2c(R);
+    const int base = ((jb >> log2Ns) << (log2Ns + LOG2R)) + (jb & ((1 << log2Ns) - 1));
+    return swz<LR0>(base + (m << log2Ns));
+}
+
+// radix-R pass from the canonical registers into the exchange buffer (caller: barrier before and after)
+template <int R, int DIR, int LR0, int IL>
+__device__ __forceinline__ void pass_store(const cplx (&v)[16], cplx *X, int r, int j, int T, int log2Ns,
+                                           const cplx *__restrict__ tw, int Nt) {
+    constexpr int NBF = 16 / R;
 #pragma unroll
     for (int b = 0; b < NBF; b++) {
         cplx x[R];
 #pragma unroll
         for (int m = 0; m < R; m++) x[m] = v[b + m * NBF];
         const int jb = j + b * T;
-        const int k = jb & (Ns - 1);
-        if (log2Ns > 0) {
-            cplx w1 = tw[(size_t)k * (Nt >> (log2Ns + LOG2R))];
-            if (DIR > 0) w1.y = -w1.y;
-            twiddle_powers<R>(x, w1);
-        }
-        dftR<R, DIR>(x);
-        if (STORE) {
-            const int base = ((jb >> log2Ns) << (log2Ns + LOG2R)) + k;
+        bfly<R, DIR>(x, jb, log2Ns, tw, Nt);
 #pragma unroll
-            for (int m = 0; m < R; m++) s[padE<E>(base + (m << log2Ns))] = x[m];
-        } else {
-#pragma unroll
-            for (int m = 0; m < R; m++) v[b + m * NBF] = x[m];
-        }
+        for (int m = 0; m < R; m++) X[(size_t)out_pos<R, LR0>(jb, m, log2Ns) * IL + r] = x[m];
     }
 }
 
-template <int E> SFFT_HD void fft_load_canonicalE(cplx *v, const cplx *s, int j, int T) {
+template <int LR0, int IL>
+__device__ __forceinline__ void load_canonical(cplx (&v)[16], const cplx *X, int r, int j, int T) {
 #pragma unroll
-    for (int q = 0; q < E; q++) v[q] = s[padE<E>(j + q * T)];
+    for (int q = 0; q < 16; q++) v[q] = X[(size_t)swz<LR0>(j + q * T) * IL + r];
 }
 
-#ifdef __CUDACC__
-// Whole FFT of length N = 2^log2N >= 2E for the T = N/E threads of one transform inside a CTA in which
-// EVERY thread calls this with the same N (barriers are CTA-wide).  v canonical in, canonical out.
-// LOG2N_CT != 0 fixes the length at compile time (the hot sizes): every shift, mask, padded index and
-// twiddle stride below then folds to a constant and the passes unroll, which removes most of the
-// integer instructions that otherwise outnumber the FP64 ones.
-template <int DIR, int E, int LOG2N_CT = 0>
-__device__ __forceinline__ void fft_blockE(cplx *v, cplx *s, int log2N_rt, int j, const cplx *tw, int Nt) {
-    constexpr int LOG2E = (E == 16) ? 4 : 3;
-    const int log2N = LOG2N_CT ? LOG2N_CT : log2N_rt;
-    const int T = 1 << (log2N - LOG2E);
-    __syncthreads();
-    fft_passE<E, E, DIR, true>(v, s, j, T, 0, tw, Nt);
-    __syncthreads();
-    fft_load_canonicalE<E>(v, s, j, T);
-    if (LOG2N_CT) {
-        // up to two more full-radix passes (N <= E^4), all bounds known
-        if (LOG2E + LOG2E < log2N) {
-            __syncthreads();
-            fft_passE<E, E, DIR, true>(v, s, j, T, LOG2E, tw, Nt);
-            __syncthreads();
-            fft_load_canonicalE<E>(v, s, j, T);
-        }
-        if (3 * LOG2E < log2N) {
-            __syncthreads();
-            fft_passE<E, E, DIR, true>(v, s, j, T, 2 * LOG2E, tw, Nt);
-            __syncthreads();
-            fft_load_canonicalE<E>(v, s, j, T);
-        }
-        const int log2Ns = (3 * LOG2E < log2N) ? 3 * LOG2E : (2 * LOG2E < log2N) ? 2 * LOG2E : LOG2E;
-        switch (log2N - log2Ns) {
-        case 4: if (E >= 16) fft_passE<E, (E >= 16 ? 16 : E), DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-        case 3: fft_passE<E, 8, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-        case 2: fft_passE<E, 4, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-        default: fft_passE<E, 2, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-        }
-        return;
-    }
-    int log2Ns = LOG2E;
-#pragma unroll 1
-    while (log2Ns + LOG2E < log2N) {
-        __syncthreads();
-        fft_passE<E, E, DIR, true>(v, s, j, T, log2Ns, tw, Nt);
-        __syncthreads();
-        fft_load_canonicalE<E>(v, s, j, T);
-        log2Ns += LOG2E;
-    }
-    switch (log2N - log2Ns) {
-    case 4: if (E >= 16) fft_passE<E, (E >= 16 ? 16 : E), DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    case 3: fft_passE<E, 8, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    case 2: fft_passE<E, 4, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    default: fft_passE<E, 2, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    }
-}
-#endif
-
-// One Stockham pass of radix R on the canonical registers of thread j.
-//   N = FFT length, T = N/16, Ns = product of the radices of earlier passes (log2Ns given),
-//   tw[k] = exp(-2 pi i k / Nt) (Nt >= N, power of two).
-// If STORE, results go to shared memory s (padded) at their autosort positions (the caller
-// puts a barrier before -- all threads must have finished reading s -- and after);
-// otherwise (last pass, Ns*R == N) they stay canonical in v.
-template <int R, int DIR, bool STORE>
-SFFT_HD void fft_pass(cplx *v, cplx *s, int j, int T, int log2Ns, const cplx *tw, int Nt) {
-    constexpr int NB = 16 / R; // butterflies per thread
-    constexpr int LOG2R = (R == 16) ? 4 : (R == 8) ? 3 : (R == 4) ? 2 : 1;
-    const int Ns = 1 << log2Ns;
+// last pass (Ns R = N): results stay in the registers, natural order v[q] = element j + q T
+template <int R, int DIR>
+__device__ __forceinline__ void pass_regs(cplx (&v)[16], int j, int T, int log2Ns, const cplx *__restrict__ tw, int Nt) {
+    constexpr int NBF = 16 / R;
 #pragma unroll
-    for (int b = 0; b < NB; b++) {
+    for (int b = 0; b < NBF; b++) {
         cplx x[R];
 #pragma unroll
-        for (int m = 0; m < R; m++) x[m] = v[b + m * NB];
-        const int jb = j + b * T;
-        const int k = jb & (Ns - 1);
-        if (log2Ns > 0) {
-            // exp(DIR * 2 pi i k / (Ns R)) from the table of exp(-2 pi i ./Nt)
-            cplx w1 = tw[(size_t)k * (Nt >> (log2Ns + LOG2R))];
-            if (DIR > 0) w1.y = -w1.y;
-            twiddle_powers<R>(x, w1);
-        }
-        dftR<R, DIR>(x);
-        if (STORE) {
-            const int base = ((jb >> log2Ns) << (log2Ns + LOG2R)) + k;
+        for (int m = 0; m < R; m++) x[m] = v[b + m * NBF];
+        bfly<R, DIR>(x, j + b * T, log2Ns, tw, Nt);
 #pragma unroll
-            for (int m = 0; m < R; m++) s[pad16(base + (m << log2Ns))] = x[m];
-        } else {
-#pragma unroll
-            for (int m = 0; m < R; m++) v[b + m * NB] = x[m];
-        }
+        for (int m = 0; m < R; m++) v[b + m * NBF] = x[m];
     }
 }
 
-SFFT_HD void fft_load_canonical(cplx *v, const cplx *s, int j, int T) {
-#pragma unroll
-    for (int q = 0; q < 16; q++) v[q] = s[pad16(j + q * T)];
+// ---------------------------------------------------------------------------------------------
+// asynchronous staging: bulk global -> shared copies (TMA engine, SASS UBLKCP) completing on an mbarrier,
+// and named barriers for thread groups smaller than the CTA
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *b, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
-
-#ifdef __CUDACC__
-// Whole FFT for the T = N/16 threads of one transform inside a CTA in which EVERY thread
-// calls this function with the same N (all barriers are CTA-wide).  v: canonical input,
-// on return canonical output (natural order).  s: this transform's shared-memory region of
-// padded_len(N) elements.
-template <int DIR>
-__device__ __forceinline__ void fft_block(cplx *v, cplx *s, int log2N, int j, const cplx *tw, int Nt) {
-    const int T = 1 << (log2N - 4);
-    int log2Ns = 0;
-    // first pass: radix 16, no twiddles
-    __syncthreads();
-    fft_pass<16, DIR, true>(v, s, j, T, 0, tw, Nt);
-    __syncthreads();
-    fft_load_canonical(v, s, j, T);
-    log2Ns = 4;
-#pragma unroll 1
-    while (log2Ns + 4 < log2N) {
-        __syncthreads();
-        fft_pass<16, DIR, true>(v, s, j, T, log2Ns, tw, Nt);
-        __syncthreads();
-        fft_load_canonical(v, s, j, T);
-        log2Ns += 4;
-    }
-    switch (log2N - log2Ns) {
-    case 4: fft_pass<16, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    case 3: fft_pass<8, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    case 2: fft_pass<4, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    default: fft_pass<2, DIR, false>(v, s, j, T, log2Ns, tw, Nt); break;
-    }
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// one arrival that also announces `bytes` of asynchronous copies to come (0: a plain arrival)
+__device__ __forceinline__ void mbar_expect(unsigned long long *b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(unsigned long long *b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity) {
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n"
+                 ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+// bytes: a multiple of 16; both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+// writes of this thread to shared memory become visible to the asynchronous (bulk copy) proxy
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// barrier `id` (1..15) over `count` threads (a multiple of 32); id 0 is __syncthreads()
+__device__ __forceinline__ void group_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 #endif
 
 } // namespace sfft

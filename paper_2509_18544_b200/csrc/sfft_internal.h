@@ -36,6 +36,20 @@ struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of
     int a[MAX_PAIRS], b[MAX_PAIRS];
 };
 
+// launch shape of stage 1 of a lag pass (sfft_lags.cu), fixed at plan creation
+struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split, nst; size_t smem; };
+struct LagMaps;             // TMA tensor maps of a lag pass (sfft_lags.cu)
+
+// Experiment knobs (environment variables SFFT_*), read ONCE at sfft_plan_create: nothing on the hot path calls getenv
+struct Knobs {
+    bool no_side;           // SFFT_NO_SIDE: keep the small kernels on the caller's stream
+    bool no_factor_overlap; // SFFT_NO_FACTOR_OVERLAP: factor inside sfft_solve instead of beside the science side
+    bool no_batch_pipe;     // SFFT_NO_BATCH_PIPE: sequential batched path
+    bool no_lookahead;      // SFFT_NO_LOOKAHEAD: trailing updates of the Cholesky on the chain's own stream
+    int batch_group;        // SFFT_BATCH_GROUP: science images per Theta pass (1..NSCI)
+    int factor_sms;         // SFFT_FACTOR_SMS: SMs the persistent column kernels leave to a factorisation running beside them
+};
+
 } // namespace sfft
 
 struct sfft_plan {
@@ -52,22 +66,27 @@ struct sfft_plan {
     cudaEvent_t ev_lookP, ev_lookB;
     cudaStream_t cstream;    // plan-owned copy stream: sfft_difference_host uploads S here while the template side computes
     cudaEvent_t ev_copy; bool science_waits_copy;
-    bool no_side;            // SFFT_NO_SIDE: keep the small kernels on the caller's stream (experiments)
+    sfft::Knobs knob;        // experiment knobs, read once at plan creation
+    int sms;                 // multiprocessors of the plan's device
     bool factor_pending;     // factor kernels are enqueued on fstream and not yet joined into `stream`
     // device workspaces
     sfft::cplx *tw;          // [Nt]
-    sfft::cplx *inter;       // [(DK+1)][ny][Hx] row-transformed intermediates (a1) / a5 intermediate
-    sfft::cplx *specT;       // [NK][My][Hx] spectra of the fit (masked) template images
-    sfft::cplx *specTo;      // [NK][My][Hx] spectra of the unmasked template images (== specT without mask)
-    sfft::cplx *specS;       // [My][Hx]
+    // planes are column-major (sfft_fft.cuh: plane_idx): intermediates [Hx][My] (column 0 packed), spectra [Hx+1][My]
+    sfft::cplx *inter;       // [(DK+1)][Hx][My] row-transformed intermediates (a1) / a5 intermediate
+    sfft::cplx *specT;       // [NK][Hx+1][My] spectra of the fit (masked) template images
+    sfft::cplx *specTo;      // [NK][Hx+1][My] spectra of the unmasked template images (allocated with the first mask)
+    sfft::cplx *specS;       // [Hx+1][My]
     // batched path: up to NSCI science images share one Theta pass; groups of images are pipelined two deep
-    sfft::cplx *specSx[sfft::NSCI]; // [My][Hx] each; [0] aliases specS, the others are allocated on first use
+    sfft::cplx *specSx[sfft::NSCI]; // [Hx+1][My] each; [0] aliases specS
     double *muSx[sfft::NSCI], *deltax[sfft::NSCI]; // row moments / Delta per image; [0] alias muS, delta
     double *hq[2 * sfft::NSCI], *cq[2 * sfft::NSCI]; // right-hand sides / solutions: group parity x image; [0] alias h, coef
     const double *Sx[sfft::NSCI];   // the science images of the current group
     double *muR;             // [(DK+DB+1)][ny] row moments sum_x xt^m (m.R)
     double *muS;             // [(DB+1)][ny]
-    sfft::cplx *Q;           // [np][2W+1][Hx+1] column-reduced products (stage 1 of a2)
+    sfft::cplx *Q;           // [split][np][2W+1][Hx+1] column-reduced products (stage 1 of a2)
+    sfft::cplx *phO, *phT;   // phase tables of the lag passes (sfft_lags.cu: lag_phase_kernel)
+    sfft::LagCfg cfgO, cfgT[sfft::NSCI]; // launch shapes: Omega; Theta with 1..NSCI science images
+    sfft::LagMaps *mapsO, *mapsT;        // their tensor maps (host copies, passed to the kernels by value)
     double *lagO;            // [npairs][(4w+1)^2]
     double *lagT;            // [NK][L*L]
     double *bpart;           // [np][(2W+1)^2] native-grid wrap corrections X_N - X_M
@@ -112,32 +131,33 @@ struct sfft_plan {
 
 namespace sfft {
 
-// ---- a1 (sfft_fwd.cu) ---------------------------------------------------------------
-// rows: img (ny x nx real, optional mask) -> inter[i] (ny x Hx packed), i = 0..NI-1, weights xt^i;
+// ---- a1, a5 transforms (sfft_rows.cu, sfft_cols.cu) -------------------------------------------
+cudaError_t rows_init();   // kernel attributes of the current device (plan creation)
+cudaError_t cols_init();
+// rows: img (ny x nx real, optional mask) -> inter[i] ([Hx][My]), i = 0..NI-1, weights xt^i;
 // also row moments mu[m][y] = sum_x xt^m (m.img), m = 0..NMOM-1.
 cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI,
                            double *mu, int NMOM);
-// columns: inter[ii[k]] * yt^jj[k] -> spec[k] (My x Hx), k = 0..ns-1
+// columns: FFT_y(yt^jj[k] * inter[ii[k]]) -> spec[k] ([Hx+1][My]), k = 0..ns-1
 cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj);
+// inter = IFFT_y(sum_t spec_t K^_t(coef))
+cudaError_t launch_col_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter);
+// mode 0: D = S - M - B; mode 1: D = +M
+cudaError_t launch_row_inv(sfft_plan *p, const cplx *inter, const double *S, const double *coef, double *D, int mode);
 
-struct ColJobs { int ns; int ii[MAX_NP]; int jj[MAX_NP]; };   // column-pass outputs: spec[k] = FFT_y(yt^jj[k] * inter[ii[k]])
-bool colpipe_ok(const Geom &g);
-cudaError_t launch_colpipe_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj, int nsrc);
-cudaError_t launch_colpipe_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter);
-
-struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split; };
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, int min_split = 1, int reserve = 0);
-int theta_reserve();
-int theta_min_split();
 int border_chunks();
 int border_linpair_chunks();
 size_t border_lp_doubles(const Geom &g, int W, int EB);
 size_t border_strip_doubles(const Geom &g, int W);
 cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science, double *bpart);
 // ---- a2, a3 (sfft_lags.cu, sfft_assemble.cu) ---------------------------------------------------------
-// lag tables of pair list pl over spectra base[s] = spec0 + s*My*Hx (s < nsA: template set, s == nsA: specS)
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c);
+cudaError_t lags_init(sfft_plan *p);   // launch shapes, tensor maps, phase tables (plan creation, after the spectra exist)
+void lags_free(sfft_plan *p);
+size_t lag_q_elems(const sfft_plan *p);
+// lag tables of pair list pl over the template spectra (index < NK) and, for science passes, specSx[i] (index NK + i)
 cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag /*[np][(2W+1)^2]*/, bool science, int nsci = 1);
-// nsci > 1: spectra NK + i are specSx[i] (images p->Sx[i]); pl lists the NK pairs of each image in turn
+// nsci > 1: pl lists the NK pairs of each image in turn (images p->Sx[i])
 cudaError_t launch_gamma(sfft_plan *p);   // muR, R, mask -> gam
 cudaError_t launch_delta(sfft_plan *p, const double *muS = nullptr, double *delta = nullptr);   // muS -> delta
 cudaError_t launch_gather_G(sfft_plan *p);
@@ -191,19 +211,19 @@ struct KLaunch {
 // side stream: fork = side waits for everything enqueued on the main stream so far; join = main waits for side.
 // In per-launch timing mode everything stays on the main stream so that kernel times do not overlap.
 inline void fork_side(sfft_plan *p) {
-    if (p->ktiming || !p->side || p->no_side) return;
+    if (p->ktiming || !p->side || p->knob.no_side) return;
     cudaEventRecord(p->ev_fork, p->stream);
     cudaStreamWaitEvent(p->side, p->ev_fork, 0); cudaStreamWaitEvent(p->sideB, p->ev_fork, 0); cudaStreamWaitEvent(p->sideC, p->ev_fork, 0);
     p->cur = p->side;
 }
 inline void use_side(sfft_plan *p, int k) { // after fork_side: enqueue on side stream k (0, 1, 2)
-    if (p->ktiming || !p->side || p->no_side) return;
+    if (p->ktiming || !p->side || p->knob.no_side) return;
     p->cur = k == 0 ? p->side : k == 1 ? p->sideB : p->sideC;
 }
 inline void back_to_main(sfft_plan *p) { p->cur = p->stream; }
 inline void join_side(sfft_plan *p) {
     p->cur = p->stream;
-    if (p->ktiming || !p->side || p->no_side) return;
+    if (p->ktiming || !p->side || p->knob.no_side) return;
     cudaEventRecord(p->ev_join, p->side); cudaStreamWaitEvent(p->stream, p->ev_join, 0);
     cudaEventRecord(p->ev_joinB, p->sideB); cudaStreamWaitEvent(p->stream, p->ev_joinB, 0);
     cudaEventRecord(p->ev_joinC, p->sideC); cudaStreamWaitEvent(p->stream, p->ev_joinC, 0);

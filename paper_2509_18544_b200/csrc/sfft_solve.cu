@@ -401,7 +401,7 @@ __device__ __forceinline__ double ll_load(const unsigned long long *buf, int i, 
     unsigned long long a = w[0], b = w[1];
     int spins = 0;
     while ((a >> 32) != e || (b >> 32) != e) {
-        if (++spins > (1 << 20)) { *err = 3; return 0.0; }
+        if (++spins > (1 << 20)) { *err = 3; return __longlong_as_double(0x7ff8000000000000LL); } // poison: a lost block must not yield plausible coefficients
         a = w[0]; b = w[1];
     }
     return __longlong_as_double((long long)((a & 0xffffffffull) | (b << 32)));
@@ -504,7 +504,7 @@ cudaError_t launch_factor(sfft_plan *p) {
     cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * CB * (CB + 1) * sizeof(double)));
     // Look-ahead: panel k+1 needs only the first block column of panel k's trailing update.  That part is fused into
     // the panel kernel of k+1; the rest of the update runs on an auxiliary stream beside it.
-    cudaStream_t aux = (p->ktiming || !p->fstream2 || getenv("SFFT_NO_LOOKAHEAD")) ? nullptr : p->fstream2;
+    cudaStream_t aux = (p->ktiming || !p->fstream2 || p->knob.no_lookahead) ? nullptr : p->fstream2;
     bool aux_busy = false;
     const size_t sm_panel = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_panel);
@@ -543,7 +543,7 @@ cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream
     const double *Lf = p->Lf, *Li = p->Linv, *ds = p->dscale;
     const size_t wsz = 2 * (size_t)(((n + 63) / 64) * 64); // exchange words of one substitution (sfft_plan_create)
     unsigned long long *y = reinterpret_cast<unsigned long long *>(work ? work : p->ywork), *z = reinterpret_cast<unsigned long long *>(work ? work + wsz : p->zwork);
-    int *err = p->flag, epoch = p->solve_epoch, nn = n;
+    int *err = p->flag + 1, epoch = p->solve_epoch, nn = n; // flag[0]: pivot test of the factorisation, flag[1]: solve errors
     void *args[] = {(void *)&Lf, (void *)&Li, (void *)&ds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&err, (void *)&epoch};
     KLaunch kl(p, "trisolve");
     return cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, st ? st : p->stream);

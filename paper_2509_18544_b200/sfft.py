@@ -324,7 +324,7 @@ class SfftPlan:
             return Mx, My
         w, L = (self.L - 1) // 2, self.L
         NK, NB = (self.DK + 1) * (self.DK + 2) // 2, (self.DB + 1) * (self.DB + 2) // 2
-        shapes = {0: ((My, Mx // 2), np.complex128), 1: ((My, Mx // 2), np.complex128),
+        shapes = {0: ((My, Mx // 2 + 1), np.complex128), 1: ((My, Mx // 2 + 1), np.complex128),
                   2: ((4 * w + 1, 4 * w + 1), np.float64), 3: ((L, L), np.float64),
                   4: ((NK, NB, L, L), np.float64), 5: ((NB, NB), np.float64), 6: ((NB,), np.float64)}
         shp, dt = shapes[which]

@@ -86,6 +86,70 @@ def test_parity_small(nx, ny, L, DK, DB, masked):
     full_parity(S, R, mask, L, DK, DB, noise_rms=20.0)
 
 
+# L >= 13 takes the wide-lag instances of the a2 kernels (lag bound 2w > 20 in the Omega pass: split lag halves /
+# the widest row-reduction instance), which configs[0..3] never reach (L <= 11).  Element by element against the oracle.
+@pytest.mark.parametrize("nx,ny,L,DK,DB,masked", [
+    (96, 80, 13, 1, 1, False),
+    (128, 100, 21, 0, 0, False),
+    (100, 90, 15, 2, 1, True),      # non power of two, masked, 21 template pairs
+    (75, 131, 17, 1, 2, False),     # odd sizes, nx != ny
+    (64, 64, 21, 1, 0, False),      # power of two, the largest kernel the library takes
+])
+def test_parity_wide_kernels(nx, ny, L, DK, DB, masked):
+    S, R = starfield.random_pair(nx, ny, seed=1000 + nx + ny + L)
+    mask = None
+    if masked:
+        rng = np.random.default_rng(15)
+        mask = (rng.random((ny, nx)) > 0.05).astype(np.uint8)
+        mask[:2, 5:30] = 0
+    full_parity(S, R, mask, L, DK, DB, noise_rms=20.0)
+
+
+@pytest.mark.parametrize("nx,ny", [(72, 4096), (4096, 72)])
+def test_longest_sides(nx, ny):
+    """The longest side the library takes (include/sfft.h: SFFT_MAX_SIDE = 4096): no padding along it, 1024 / 512
+    padded points along the short one, wrap corrections on the short side only."""
+    S, R = starfield.random_pair(nx, ny, seed=nx + ny)
+    full_parity(S, R, None, 5, 1, 1, noise_rms=20.0)
+
+
+def test_sides_above_the_limit_are_rejected():
+    for nx, ny in ((4097, 64), (64, 5000)):
+        with pytest.raises(SfftError):
+            SfftPlan(nx, ny, 3, 0, 0)
+
+
+def test_masked_then_unmasked_pair_on_one_plan():
+    """A plan used with a mask keeps a second set of (unmasked) template spectra for the subtraction (reading C7);
+    the next pair WITHOUT a mask, and another template, must not convolve the stale set."""
+    nx, ny, L, DK, DB = 100, 72, 5, 1, 1
+    S1, R1 = starfield.random_pair(nx, ny, seed=201)
+    S2, R2 = starfield.random_pair(nx, ny, seed=202)
+    rng = np.random.default_rng(3)
+    mask = (rng.random((ny, nx)) > 0.05).astype(np.uint8)
+    p = SfftPlan(nx, ny, L, DK, DB)
+    nker = L * L * 3
+    for S, R, m in ((S1, R1, mask), (S2, R2, None), (S1, R1, mask), (S2, R1, None)):
+        p.build_system(dev(S), dev(R), dev(m) if m is not None else None)
+        p.solve()
+        D, c = p.subtract()
+        p.sync_status()
+        G0, h0 = oracle.build_system(S, R, m, L, DK, DB)
+        c0 = oracle.solve(G0, h0)
+        assert_coeffs(c.cpu().numpy(), c0, nker)
+        D0 = oracle.subtract(S, R, L, DK, DB, c0)
+        assert np.max(np.abs(D.cpu().numpy() - D0)) <= TOL_D * 20.0
+    # the batched calls after a masked single pair
+    p.set_template(dev(R2))
+    Ds, cs = p.subtract_batch([dev(S2), dev(S1)])
+    p.sync_status()
+    for S, D in ((S2, Ds[0]), (S1, Ds[1])):
+        G0, h0 = oracle.build_system(S, R2, None, L, DK, DB)
+        D0 = oracle.subtract(S, R2, L, DK, DB, oracle.solve(G0, h0))
+        assert np.max(np.abs(D.cpu().numpy() - D0)) <= TOL_D * 20.0
+    p.destroy()
+
+
 def test_masked_pair_on_the_pipelined_column_path():
     """600 x 520 pads to 1024 x 1024: the persistent column kernels (My >= 512), tile-major spectra,
     a mask (separate unmasked template spectra for the subtraction, reading C7) and wrap corrections."""
@@ -111,19 +175,22 @@ def test_tall_frame_on_the_compile_time_4096_column_path():
 
 
 def test_debug_read_spectrum_layout():
-    """The test hook hands spectra out as [My][Hx] whatever the device layout is: compare the template
-    spectrum t = 0 (no weight) with numpy's rfft2 of the zero-padded frame."""
+    """The test hook hands spectra out as [My][Hx+1] (kx = 0..Mx/2) whatever the device layout is: compare the
+    template spectra (weights xt^i yt^j) with numpy's rfft2 of the zero-padded weighted frames -- this pins the row and
+    column transforms, the untangle and the separation of the packed column kx = 0 / Mx/2 on their own."""
     S, R = starfield.random_pair(96, 80, seed=5)
     p = SfftPlan(96, 80, 3, 1, 0)
     p.build_system(dev(S), dev(R))
     Mx, My = p.debug_read(7)
-    spec = p.debug_read(0, 0)
-    pad = np.zeros((My, Mx)); pad[:80, :96] = R
-    ref = np.fft.rfft2(pad)
-    assert np.max(np.abs(spec[:, 1:] - ref[:, 1:Mx // 2])) <= 1e-9 * np.max(np.abs(ref))
-    # column 0 is packed: FFT_y(X[.,0] + i X[.,Hx]) (both real along x)
-    packed = np.fft.fft(np.fft.ifft(ref[:, 0]).real + 1j * np.fft.ifft(ref[:, Mx // 2]).real)
-    assert np.max(np.abs(spec[:, 0] - packed)) <= 1e-9 * np.max(np.abs(ref))
+    for t in range(3):
+        i, j = oracle.poly_index(t)
+        spec = p.debug_read(0, t)
+        pad = np.zeros((My, Mx)); pad[:80, :96] = oracle.weighted_image(R, None, i, j)
+        ref = np.fft.rfft2(pad)
+        assert spec.shape == ref.shape
+        assert np.max(np.abs(spec - ref)) <= 1e-9 * np.max(np.abs(ref)), t
+    pad = np.zeros((My, Mx)); pad[:80, :96] = S
+    assert np.max(np.abs(p.debug_read(1) - np.fft.rfft2(pad))) <= 1e-9 * np.max(np.abs(pad)) * 80 * 96
     p.destroy()
 
 
