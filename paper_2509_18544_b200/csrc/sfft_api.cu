@@ -79,7 +79,7 @@ static void free_plan(sfft_plan *p) {
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
     if (p->flag_host) cudaFreeHost(p->flag_host);
-    lags_free(p);
+    lags_free(p); rows_free(p);
     for (int s = 0; s < SFFT_NUM_STAGES; s++) {
         if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
         if (p->ev1[s]) cudaEventDestroy(p->ev1[s]);
@@ -230,7 +230,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     cudaEventCreateWithFlags(&p->ev_lookP, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_lookB, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
-    e = rows_init();
+    e = rows_init(p);
     if (e == cudaSuccess) e = cols_init();
     if (e == cudaSuccess) e = lags_init(p);   // tensor maps over the spectra, phase tables (after the twiddles)
     if (e != cudaSuccess) { cudaGetLastError(); free_plan(p); return SFFT_ERR_CUDA; }

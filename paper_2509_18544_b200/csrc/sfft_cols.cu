@@ -111,7 +111,9 @@ col_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, unsigned
     const cplx w2 = tw[(size_t)(j & 15) * (Nt >> 8)];
     const cplx w3 = C::R3 == 16 ? tw[(size_t)(j & 255) * (Nt >> 12)] : mk(1.0, 0.0);
     int s = 0;
+    const int j_outer_ = j; // (see the note at opaque_index)
     for (int n = 0; n < nitems; n++) {
+        const int j = opaque_index(j_outer_);
         const int col = wid + (n / njobs) * nw, k = n % njobs;
         const int jp = (int)(jpack >> (4 * k)) & 3;
         cplx v[16];
@@ -216,7 +218,9 @@ col_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, cplx 
     const cplx w3 = C::R3 == 16 ? tw[(size_t)(j & 255) * (Nt >> 12)] : mk(1.0, 0.0);
     const int twsy = Nt / N;
     int s = 0;
+    const int j_outer_ = j; // (see the note at opaque_index)
     for (int n = 0; n < ncol; n++) {
+        const int j = opaque_index(j_outer_);
         const int col = wid + n * nw, nv = col == 0 ? 2 * NK : NK;
         group_sync(bar_id, T); // the previous column's last exchange has been read: X is free for the taps
         for (int e = j; e < nv * L; e += T) {

@@ -207,6 +207,11 @@ __device__ __forceinline__ void pass_regs(cplx (&v)[16], int j, int T, int log2N
     }
 }
 
+// The persistent kernels derive ~50 shared-memory addresses from the thread index.  They are loop invariant, so the
+// compiler hoists them out of the item loop and keeps them in registers across it -- next to 16 complex values that is
+// what spilled.  An index laundered through an empty asm per item is recomputed where it is used instead.
+__device__ __forceinline__ int opaque_index(int j) { asm volatile("" : "+r"(j)); return j; }
+
 // ---------------------------------------------------------------------------------------------
 // asynchronous staging: bulk global -> shared copies (TMA engine, SASS UBLKCP) completing on an mbarrier,
 // and named barriers for thread groups smaller than the CTA

@@ -39,6 +39,9 @@ struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of
 // launch shape of stage 1 of a lag pass (sfft_lags.cu), fixed at plan creation
 struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split, nst; size_t smem; };
 struct LagMaps;             // TMA tensor maps of a lag pass (sfft_lags.cu)
+} // namespace sfft
+struct CUtensorMap_st;      // <cuda.h>: CUtensorMap
+namespace sfft {
 
 // Experiment knobs (environment variables SFFT_*), read ONCE at sfft_plan_create: nothing on the hot path calls getenv
 struct Knobs {
@@ -87,6 +90,7 @@ struct sfft_plan {
     sfft::cplx *phO, *phT;   // phase tables of the lag passes (sfft_lags.cu: lag_phase_kernel)
     sfft::LagCfg cfgO, cfgT[sfft::NSCI]; // launch shapes: Omega; Theta with 1..NSCI science images
     sfft::LagMaps *mapsO, *mapsT;        // their tensor maps (host copies, passed to the kernels by value)
+    CUtensorMap_st *mapI;                // tensor map of the a5 intermediate (sfft_rows.cu)
     double *lagO;            // [npairs][(4w+1)^2]
     double *lagT;            // [NK][L*L]
     double *bpart;           // [np][(2W+1)^2] native-grid wrap corrections X_N - X_M
@@ -132,7 +136,8 @@ struct sfft_plan {
 namespace sfft {
 
 // ---- a1, a5 transforms (sfft_rows.cu, sfft_cols.cu) -------------------------------------------
-cudaError_t rows_init();   // kernel attributes of the current device (plan creation)
+cudaError_t rows_init(sfft_plan *p);   // kernel attributes of the current device, tensor map of the a5 intermediate (plan creation)
+void rows_free(sfft_plan *p);
 cudaError_t cols_init();
 // rows: img (ny x nx real, optional mask) -> inter[i] ([Hx][My]), i = 0..NI-1, weights xt^i;
 // also row moments mu[m][y] = sum_x xt^m (m.img), m = 0..NMOM-1.

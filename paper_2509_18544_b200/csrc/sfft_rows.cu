@@ -14,16 +14,30 @@
 // registers, without the extra shared-memory round trip of a separate untangle step (the row passes were bound
 // by the shared-memory pipe: profiles/r01l_ncu_summary.md).  The inverse kernel mirrors this: tangle in
 // registers, then radix 8 (butterflies A, B), radix Hx/128, radix 16, and the fused D = S - M - B.
+#include <cuda.h>
+#include <new>
+#include <type_traits>
 #include "sfft_internal.h"
 
 namespace sfft {
 
 constexpr int ROW_THREADS = 256;
 
+constexpr int ROW_RING = 3;
+
+// A WORKER is the group of 2 T threads of one row pair; a CTA holds RP = 256 / (2 T) workers, two CTAs share an SM.
+// Workers are persistent: they loop over row pairs, and the input of the next steps is in flight (bulk copies
+// completing on mbarriers, one elected thread) while the current pair is transformed.
 template <int LOG2H> struct RowCfg {
     static constexpr int Hx = 1 << LOG2H, T = Hx / 16, GT = 2 * T, RP = ROW_THREADS / GT;
     static constexpr int R2 = Hx / 128;                       // middle radix: 4, 8 or 16
-    static constexpr size_t SMEM = (size_t)RP * 2 * Hx * sizeof(cplx);
+    static constexpr int QP = 8 * T;                          // pixels of a quarter row (Mx / 4)
+    static constexpr int FSLOT = 2 * QP + 16;                 // forward ring slot in doubles: two quarter rows, the second
+                                                              // skewed by 64 B (+ pad to 128 B) against bank conflicts
+    static constexpr int ISLOT = 2 * (Hx / 8) * 2;            // inverse ring slot in cplx: two TMA boxes {2 rows x Hx/8 kx}
+    static constexpr size_t XBYTES = (size_t)RP * 2 * Hx * sizeof(cplx);
+    static constexpr size_t SMEM_F = XBYTES + (size_t)RP * ROW_RING * FSLOT * sizeof(double);
+    static constexpr size_t SMEM_I = XBYTES + (size_t)RP * ROW_RING * ISLOT * sizeof(cplx);
 };
 
 __device__ __forceinline__ double ipow_small(double b, int e) {
@@ -67,80 +81,131 @@ __device__ __forceinline__ void tangle(cplx XA, cplx XB, cplx u, cplx &Zk, cplx 
 // ------------------------------------------------------------------------------------------ forward
 // rows: img (ny x nx real, optional mask) -> inter[i] (Hx columns x My, column-major), i = 0..NI-1, weights xt^i;
 // also row moments mu[m][y] = sum_x xt^m (m.img), m = 0..NMOM-1 (for Gamma / Delta).
-// grid = ceil(ny / (2 RP)); block 256 = RP row pairs of 2 T threads; dynamic smem RowCfg::SMEM
-template <int LOG2H>
+// grid: persistent, <= 2 CTAs per SM; block 256 = RP workers of 2 T threads; dynamic smem RowCfg::SMEM_F.
+// BULK (even nx, 16-byte aligned image): the two rows arrive quarter by quarter through a 3-slot ring of bulk copies
+// (every weight i re-reads the pair from L2); otherwise plain loads.
+template <int LOG2H, bool BULK, bool MASK>
 __global__ void __launch_bounds__(ROW_THREADS, 2)
 row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask, cplx *__restrict__ inter, int NI,
                double *__restrict__ mu, int NMOM, Geom g, const cplx *__restrict__ tw) {
     using C = RowCfg<LOG2H>;
-    constexpr int Hx = C::Hx, T = C::T, GT = C::GT, TP = 2 * T; // TP = Hx/8: butterflies of the last pass
+    constexpr int Hx = C::Hx, T = C::T, GT = C::GT, TP = 2 * T, QP = C::QP; // TP = Hx/8: butterflies of the last pass
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ double wpart[ROW_THREADS / 32][2][8];
+    __shared__ unsigned long long full[C::RP * ROW_RING];
     const int grp = threadIdx.x / GT, t = threadIdx.x - grp * GT, r = t & 1, j = t >> 1, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * 2 * Hx;
-    const int y = (blockIdx.x * C::RP + grp) * 2 + r, nx = g.nx, ny = g.ny, My = g.My, Nt = g.Nt;
-    const bool live = y < ny;
+    // warp partials of the row moments [warp of the worker][row][m]: they live in the exchange buffer, which is idle
+    // during the load phase (two CTAs per SM leave no room for another static array)
+    double (*wpart)[2][8] = reinterpret_cast<double (*)[2][8]>(X);
+    double *ring = reinterpret_cast<double *>(smem_raw + C::XBYTES) + (size_t)grp * ROW_RING * C::FSLOT;
+    unsigned long long *bar = full + grp * ROW_RING;
+    if (BULK && t == 0) {
+        for (int k = 0; k < ROW_RING; k++) mbar_init(&bar[k], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int nx = g.nx, ny = g.ny, My = g.My, Nt = g.Nt, npairs = (ny + 1) >> 1;
+    const int wid = blockIdx.x * C::RP + grp, nw = gridDim.x * C::RP;
+    const int nmine = wid < npairs ? (npairs - wid + nw - 1) / nw : 0;
+    const int nitems = nmine * NI, nsteps = nitems * 4;
     const double inv_nx = 1.0 / (double)nx;
-    const size_t rowoff = (size_t)y * nx;
-    const bool vec = ((nx & 1) == 0) && (((size_t)img & 15) == 0);
-    const int A = j, B = j == 0 ? T : TP - j;
-    const cplx wA = tw[(size_t)A * (Nt >> LOG2H)], wB = tw[(size_t)B * (Nt >> LOG2H)]; // exp(-2 pi i jb/Hx)
-    const cplx uA = tw[(size_t)A * (Nt >> (LOG2H + 1))], uT = tw[(size_t)T * (Nt >> (LOG2H + 1))]; // exp(-2 pi i k/Mx)
-
-    for (int i = 0; i < NI; i++) {
-        cplx v[16];
-        double mom[8];
-#pragma unroll
-        for (int m = 0; m < 8; m++) mom[m] = 0.0;
-#pragma unroll
-        for (int q = 0; q < 16; q++) {
-            const int x0 = 2 * (j + q * T);
-            double a = 0.0, b = 0.0;
-            if (live) {
-                if (vec) { // even nx, 16-byte aligned image: one 16-byte load per pixel pair
-                    if (x0 < nx) { const double2 ab = *reinterpret_cast<const double2 *>(img + rowoff + x0); a = ab.x; b = ab.y; }
-                } else {
-                    if (x0 < nx) a = img[rowoff + x0];
-                    if (x0 + 1 < nx) b = img[rowoff + x0 + 1];
-                }
-                if (mask) {
-                    if (x0 < nx && !mask[rowoff + x0]) a = 0.0;
-                    if (x0 + 1 < nx && !mask[rowoff + x0 + 1]) b = 0.0;
-                }
-            }
-            const double xa = (2.0 * x0 + 1.0 - nx) * inv_nx, xb = (2.0 * x0 + 3.0 - nx) * inv_nx;
-            if (i == 0 && NMOM > 0) {
-                double pa = a, pb = b;
-#pragma unroll
-                for (int m = 0; m < 8; m++)
-                    if (m < NMOM) { mom[m] += pa + pb; pa *= xa; pb *= xb; }
-            }
-            v[q] = mk(a * ipow_small(xa, i), b * ipow_small(xb, i));
+    auto issue = [&](int s) { // one thread: quarter Q of both rows of item n into slot s % RING
+        const int n = s >> 2, Q = s & 3, slot = s % ROW_RING;
+        const int y0 = 2 * (wid + (n / NI) * nw);
+        int px = nx - Q * QP; px = px < 0 ? 0 : (px > QP ? QP : px);
+        const unsigned bytes = (unsigned)px * 8u;
+        const bool two = y0 + 1 < ny;
+        mbar_expect(&bar[slot], two ? 2u * bytes : bytes);
+        if (bytes) {
+            double *dst = ring + (size_t)slot * C::FSLOT;
+            const double *src = img + (size_t)y0 * nx + Q * QP;
+            bulk_g2s(dst, src, bytes, &bar[slot]);
+            if (two) bulk_g2s(dst + QP + 8, src + nx, bytes, &bar[slot]);
         }
-        if (i == 0 && NMOM > 0) {
-            // deterministic reduction over the T threads of each row: lanes of equal parity inside a warp, then warps
+    };
+    if (BULK && t == 0)
+        for (int s = 0; s < ROW_RING && s < nsteps; s++) issue(s);
+
+    int s = 0;
+    const int j_outer_ = j; // (see the note at opaque_index)
+    for (int n = 0; n < nitems; n++) {
+        const int j = opaque_index(j_outer_);
+        // xt of the thread's pixel pairs: pixel 2 (j + q T) has xt = xa0 + q xstep, its neighbour xt + xpix
+        const double xa0 = (4.0 * j + 1.0 - nx) * inv_nx, xstep = 4.0 * T * inv_nx, xpix = 2.0 * inv_nx;
+        const int A = j, B = j == 0 ? T : TP - j;
+        const int i = n % NI, y = 2 * (wid + (n / NI) * nw) + r;
+        const bool live = y < ny;
+        const size_t rowoff = (size_t)y * nx;
+        cplx v[16];
+        // weight xt^i as the one-hot cubic c0 + x (c1 + x (c2 + x c3)): three fused multiply-adds, no branches on i
+        const double c0 = i == 0 ? 1.0 : 0.0, c1 = i == 1 ? 1.0 : 0.0, c2 = i == 2 ? 1.0 : 0.0, c3 = i == 3 ? 1.0 : 0.0;
+        // the load phase; NM = number of row moments accumulated beside it (0: none; the instances 3, 5, 8 cover
+        // NMOM <= 3, <= 5, <= 7 -- their accumulators live only in the instance that needs them)
+        auto load = [&](auto nm_tag) {
+            constexpr int NM = decltype(nm_tag)::value;
+            double mom[NM > 0 ? NM : 1];
 #pragma unroll
-            for (int m = 0; m < 8; m++)
-                if (m < NMOM)
+            for (int m = 0; m < (NM > 0 ? NM : 1); m++) mom[m] = 0.0;
+#pragma unroll
+            for (int Q = 0; Q < 4; Q++) {
+                const int slot = s % ROW_RING;
+                if (BULK) mbar_wait(&bar[slot], (unsigned)(s / ROW_RING) & 1u);
+#pragma unroll
+                for (int qq = 0; qq < 4; qq++) {
+                    const int q = 4 * Q + qq, x0 = 2 * (j + q * T);
+                    double a = 0.0, b = 0.0;
+                    if (BULK) {
+                        const double2 ab = *reinterpret_cast<const double2 *>(ring + (size_t)slot * C::FSLOT + r * (QP + 8) + 2 * j + 2 * T * qq);
+                        if (live && x0 < nx) { a = ab.x; b = ab.y; }
+                    } else if (live) {
+                        if (x0 < nx) a = img[rowoff + x0];
+                        if (x0 + 1 < nx) b = img[rowoff + x0 + 1];
+                    }
+                    if (MASK && live) {
+                        if (x0 < nx && !mask[rowoff + x0]) a = 0.0;
+                        if (x0 + 1 < nx && !mask[rowoff + x0 + 1]) b = 0.0;
+                    }
+                    const double xa = fma((double)q, xstep, xa0), xb = xa + xpix; // xt of pixels x0, x0 + 1
+                    if (NM > 0) {
+                        double pa = a, pb = b;
+#pragma unroll
+                        for (int m = 0; m < NM; m++) { mom[m] += pa + pb; pa *= xa; pb *= xb; }
+                    }
+                    v[q] = mk(a * fma(xa, fma(xa, fma(xa, c3, c2), c1), c0), b * fma(xb, fma(xb, fma(xb, c3, c2), c1), c0));
+                }
+                if (BULK) {
+                    group_sync(bar_id, GT); // every thread of the worker has read the slot
+                    if (t == 0 && s + ROW_RING < nsteps) issue(s + ROW_RING);
+                    s++;
+                }
+            }
+            if (NM > 0) {
+                // deterministic reduction over the T threads of each row: lanes of equal parity inside a warp, then warps
+                if (!BULK) group_sync(bar_id, GT); // (no ring barriers on this path: the previous item's reads of X must be done)
+                const int lane = threadIdx.x & 31, wrp = t >> 5;
+#pragma unroll
+                for (int m = 0; m < NM; m++) {
 #pragma unroll
                     for (int off = 16; off >= 2; off >>= 1) mom[m] += __shfl_xor_sync(0xffffffffu, mom[m], off);
-            const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-            if (lane < 2) {
-#pragma unroll
-                for (int m = 0; m < 8; m++) // static indices: a run-time bound here would push mom[] into local memory
-                    if (m < NMOM) wpart[wid][lane][m] = mom[m];
+                    if (lane < 2) wpart[wrp][lane][m] = mom[m];
+                }
             }
+        };
+        if (i == 0 && NMOM > 0) {
+            if (NMOM <= 3) load(std::integral_constant<int, 3>());
+            else if (NMOM <= 5) load(std::integral_constant<int, 5>());
+            else load(std::integral_constant<int, 8>());
             group_sync(bar_id, GT);
             if (j == 0 && live) {
-                const int w0 = (grp * GT) >> 5, nwarp = GT >> 5;
+                const int nwarp = GT >> 5;
                 for (int m = 0; m < NMOM; m++) {
                     double acc = 0.0;
-                    for (int k = 0; k < nwarp; k++) acc += wpart[w0 + k][r][m];
+                    for (int k = 0; k < nwarp; k++) acc += wpart[k][r][m];
                     mu[(size_t)m * ny + y] = acc;
                 }
             }
-        }
-        group_sync(bar_id, GT); // the previous transform's last-pass reads of X are done
+        } else load(std::integral_constant<int, 0>());
+        group_sync(bar_id, GT); // the previous transform's last-pass reads of X (and of wpart) are done
         {   // pass 1: radix 16, no twiddles
             dft16<-1>(v);
 #pragma unroll
@@ -150,6 +215,10 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
         load_canonical<4, 2>(v, X, r, j, T);
         group_sync(bar_id, GT);
         pass_store<C::R2, -1, 4, 2>(v, X, r, j, T, 4, tw, Nt);
+        // twiddles of the last pass and of the untangle: fetched here (not kept across the passes: 16 registers), their
+        // latency hides behind the barrier
+        const cplx wA = tw[(size_t)A * (Nt >> LOG2H)], wB = tw[(size_t)B * (Nt >> LOG2H)]; // exp(-2 pi i jb/Hx)
+        const cplx uA = tw[(size_t)(j == 0 ? T : A) * (Nt >> (LOG2H + 1))];               // exp(-2 pi i k/Mx), k = A (thread 0: T)
         group_sync(bar_id, GT);
         // last pass: radix 8, Ns = Hx/8, butterflies A and B
         cplx zA[8], zB[8];
@@ -181,7 +250,7 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
 #pragma unroll
             for (int m = 0; m < 4; m++) {
                 cplx Xk, Xnk;
-                untangle(zB[m], zB[7 - m], cmul(uT, w16(m)), Xk, Xnk);
+                untangle(zB[m], zB[7 - m], cmul(uA, w16(m)), Xk, Xnk);
                 if (live) { dst[(size_t)(T + m * TP) * My] = Xk; dst[(size_t)(T + (7 - m) * TP) * My] = Xnk; }
             }
         }
@@ -189,130 +258,236 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
 }
 
 // ------------------------------------------------------------------------------------------ inverse
-// inter (Hx columns x My, column-major) -> D = S - M - B (mode 0) or D = +M (mode 1: plain convolution, f2)
+__device__ __forceinline__ void tma_load2(void *dst, const CUtensorMap *tm, int c0, int c1, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void l2_prefetch(const void *gsrc, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
+}
+
+// inter (Hx columns x My, column-major; tensor map tmI: boxes {2 rows, Hx/8 kx} = the 32-byte sectors of one row
+// pair) -> D = S - M - B (mode 0) or D = +M (mode 1: plain convolution, f2).
+// grid: persistent, <= 2 CTAs per SM; block 256 = RP workers of 2 T threads; dynamic smem RowCfg::SMEM_I
 template <int LOG2H>
 __global__ void __launch_bounds__(ROW_THREADS, 2)
-row_inv_kernel(const cplx *__restrict__ inter, const double *__restrict__ S, const double *__restrict__ coef,
+row_inv_kernel(const __grid_constant__ CUtensorMap tmI, const double *__restrict__ S, const double *__restrict__ coef,
                double *__restrict__ D, Geom g, const cplx *__restrict__ tw, int mode) {
     using C = RowCfg<LOG2H>;
     constexpr int Hx = C::Hx, T = C::T, GT = C::GT, TP = 2 * T;
     extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ unsigned long long full[C::RP * ROW_RING];
     const int grp = threadIdx.x / GT, t = threadIdx.x - grp * GT, r = t & 1, j = t >> 1, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * 2 * Hx;
-    const int y = (blockIdx.x * C::RP + grp) * 2 + r, nx = g.nx, ny = g.ny, My = g.My, Nt = g.Nt;
-    const bool live = y < ny;
+    cplx *ring = reinterpret_cast<cplx *>(smem_raw + C::XBYTES) + (size_t)grp * ROW_RING * C::ISLOT;
+    unsigned long long *bar = full + grp * ROW_RING;
+    if (t == 0) {
+        for (int k = 0; k < ROW_RING; k++) mbar_init(&bar[k], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int nx = g.nx, ny = g.ny, My = g.My, Nt = g.Nt, npairs = (ny + 1) >> 1;
+    const int wid = blockIdx.x * C::RP + grp, nw = gridDim.x * C::RP;
+    const int nmine = wid < npairs ? (npairs - wid + nw - 1) / nw : 0;
+    const int nsteps = nmine * 4;
     const int A = j, B = j == 0 ? T : TP - j;
-    const cplx uA = tw[(size_t)A * (Nt >> (LOG2H + 1))], uT = tw[(size_t)T * (Nt >> (LOG2H + 1))];
-    const cplx *src = inter + y;
-    cplx zA[8], zB[8];
-    {
-        cplx xA[8], xB[8];
+    const bool vec = ((nx & 1) == 0) && (((size_t)S | (size_t)D) & 15) == 0;
+    auto issue = [&](int s) { // one thread: boxes m = 2Q, 2Q+1 of row pair n into slot s % RING
+        const int n = s >> 2, Q = s & 3, slot = s % ROW_RING;
+        const int y0 = 2 * (wid + n * nw);
+        mbar_expect(&bar[slot], (unsigned)(C::ISLOT * sizeof(cplx)));
+        tma_load2(ring + (size_t)slot * C::ISLOT, &tmI, 2 * y0, (2 * Q) * TP, &bar[slot]);
+        tma_load2(ring + (size_t)slot * C::ISLOT + 2 * TP, &tmI, 2 * y0, (2 * Q + 1) * TP, &bar[slot]);
+        if (Q == 0 && mode == 0 && vec) { // the science rows of this pair are wanted at the end of the item: start them towards L2 now
+            const int rows = y0 + 1 < ny ? 2 : 1;
+            l2_prefetch(S + (size_t)y0 * nx, (unsigned)(rows * nx * 8));
+        }
+    };
+    if (t == 0)
+        for (int s = 0; s < ROW_RING && s < nsteps; s++) issue(s);
+    const cplx uA = tw[(size_t)(j == 0 ? T : A) * (Nt >> (LOG2H + 1))]; // exp(-2 pi i k/Mx), k = A (thread 0: T)
+    const cplx wL = tw[(size_t)j * (Nt >> LOG2H)];                      // last pass: radix 16, Ns = T, one butterfly per thread
+    int s = 0;
+    const int j_outer_ = j; // (see the note at opaque_index)
+    for (int n = 0; n < nmine; n++) {
+        const int j = opaque_index(j_outer_);
+        const int y = 2 * (wid + n * nw) + r;
+        const bool live = y < ny;
+        cplx zA[8], zB[8];
+        {
+            cplx xA[8], xB[8];
+#pragma unroll
+            for (int Q = 0; Q < 4; Q++, s++) {
+                const int slot = s % ROW_RING;
+                mbar_wait(&bar[slot], (unsigned)(s / ROW_RING) & 1u);
+                const cplx *sl = ring + (size_t)slot * C::ISLOT;
+#pragma unroll
+                for (int bx = 0; bx < 2; bx++) {
+                    xA[2 * Q + bx] = live ? sl[(size_t)(bx * TP + A) * 2 + r] : mk(0.0, 0.0);
+                    xB[2 * Q + bx] = live ? sl[(size_t)(bx * TP + B) * 2 + r] : mk(0.0, 0.0);
+                }
+                group_sync(bar_id, GT); // every thread of the worker has read the slot
+                if (t == 0 && s + ROW_RING < nsteps) issue(s + ROW_RING);
+            }
+            if (j != 0) {
+#pragma unroll
+                for (int m = 0; m < 8; m++) tangle(xA[m], xB[7 - m], cmul(uA, w16(m)), zA[m], zB[7 - m]);
+            } else {
+                zA[0] = mk(0.5 * (xA[0].x + xA[0].y), 0.5 * (xA[0].x - xA[0].y)); // (DC, Nyquist), both real
+#pragma unroll
+                for (int m = 1; m <= 4; m++) {
+                    cplx Zk, Znk;
+                    tangle(xA[m], xA[8 - m], w16(m), Zk, Znk);
+                    zA[m] = Zk;
+                    if (m < 4) zA[8 - m] = Znk;
+                }
+#pragma unroll
+                for (int m = 0; m < 4; m++) tangle(xB[m], xB[7 - m], cmul(uA, w16(m)), zB[m], zB[7 - m]);
+            }
+        }
+        // pass 1: radix 8, no twiddles, butterflies A and B (the four ring barriers above order the previous pair's reads of X)
+        dft8<1>(zA);
+        dft8<1>(zB);
 #pragma unroll
         for (int m = 0; m < 8; m++) {
-            xA[m] = live ? src[(size_t)(A + m * TP) * My] : mk(0.0, 0.0);
-            xB[m] = live ? src[(size_t)(B + m * TP) * My] : mk(0.0, 0.0);
+            X[(size_t)out_pos<8, 3>(A, m, 0) * 2 + r] = zA[m];
+            X[(size_t)out_pos<8, 3>(B, m, 0) * 2 + r] = zB[m];
         }
-        if (j != 0) {
+        group_sync(bar_id, GT);
+        cplx v[16];
+        load_canonical<3, 2>(v, X, r, j, T);
+        group_sync(bar_id, GT);
+        pass_store<C::R2, 1, 3, 2>(v, X, r, j, T, 3, tw, Nt);
+        group_sync(bar_id, GT);
+        load_canonical<3, 2>(v, X, r, j, T);
+        bfly_w<16, 1>(v, wL);
+        if (!live) continue;
+        // background polynomial of this row: B(x) = sum_p cx[p] xt^p, cx[p] = sum_q b_(p,q) yt^q
+        double cx[MAX_DEG + 1];
 #pragma unroll
-            for (int m = 0; m < 8; m++) tangle(xA[m], xB[7 - m], cmul(uA, w16(m)), zA[m], zB[7 - m]);
-        } else {
-            zA[0] = mk(0.5 * (xA[0].x + xA[0].y), 0.5 * (xA[0].x - xA[0].y)); // (DC, Nyquist), both real
+        for (int p = 0; p <= MAX_DEG; p++) cx[p] = 0.0;
+        {
+            const double yt = (2.0 * y + 1.0 - ny) / (double)ny;
+            const double *b = coef + (size_t)g.NK * g.L * g.L;
+            for (int sI = 0; sI < g.NB; sI++) {
+                double yp = 1.0;
+                for (int k = 0; k < g.pj[sI]; k++) yp *= yt;
 #pragma unroll
-            for (int m = 1; m <= 4; m++) {
-                cplx Zk, Znk;
-                tangle(xA[m], xA[8 - m], w16(m), Zk, Znk);
-                zA[m] = Zk;
-                if (m < 4) zA[8 - m] = Znk;
+                for (int p = 0; p <= MAX_DEG; p++) if (g.pi[sI] == p) cx[p] = fma(b[sI], yp, cx[p]);
             }
-#pragma unroll
-            for (int m = 0; m < 4; m++) tangle(xB[m], xB[7 - m], cmul(uT, w16(m)), zB[m], zB[7 - m]);
         }
-    }
-    // pass 1: radix 8, no twiddles, butterflies A and B
-    dft8<1>(zA);
-    dft8<1>(zB);
-#pragma unroll
-    for (int m = 0; m < 8; m++) {
-        X[(size_t)out_pos<8, 3>(A, m, 0) * 2 + r] = zA[m];
-        X[(size_t)out_pos<8, 3>(B, m, 0) * 2 + r] = zB[m];
-    }
-    group_sync(bar_id, GT);
-    cplx v[16];
-    load_canonical<3, 2>(v, X, r, j, T);
-    group_sync(bar_id, GT);
-    pass_store<C::R2, 1, 3, 2>(v, X, r, j, T, 3, tw, Nt);
-    group_sync(bar_id, GT);
-    load_canonical<3, 2>(v, X, r, j, T);
-    pass_regs<16, 1>(v, j, T, LOG2H - 4, tw, Nt);
-    if (!live) return;
-    // background polynomial of this row: B(x) = sum_p cx[p] xt^p, cx[p] = sum_q b_(p,q) yt^q
-    double cx[MAX_DEG + 1];
-#pragma unroll
-    for (int p = 0; p <= MAX_DEG; p++) cx[p] = 0.0;
-    {
-        const double yt = (2.0 * y + 1.0 - ny) / (double)ny;
-        const double *b = coef + (size_t)g.NK * g.L * g.L;
-        for (int sI = 0; sI < g.NB; sI++) {
-            double yp = 1.0;
-            for (int k = 0; k < g.pj[sI]; k++) yp *= yt;
-#pragma unroll
-            for (int p = 0; p <= MAX_DEG; p++) if (g.pi[sI] == p) cx[p] = fma(b[sI], yp, cx[p]);
-        }
-    }
-    // mode 1 (plain convolution, f2): D = +M; the science image is not read and there is no background (NB = 0)
-    const double scale = (mode ? -1.0 : 1.0) / ((double)Hx * (double)My), inx = 1.0 / (double)nx;
-    const size_t ro = (size_t)y * nx;
-    const bool vec = ((nx & 1) == 0) && (((size_t)S | (size_t)D) & 15) == 0;
-#pragma unroll
-    for (int q = 0; q < 16; q++) {
-        const int x0 = 2 * (j + q * T);
-        if (x0 >= nx) continue;
-        const double xa = (2.0 * x0 + 1.0 - nx) * inx, xb = (2.0 * x0 + 3.0 - nx) * inx;
-        const double ba = fma(fma(fma(cx[3], xa, cx[2]), xa, cx[1]), xa, cx[0]);
-        const double bb = fma(fma(fma(cx[3], xb, cx[2]), xb, cx[1]), xb, cx[0]);
+        // mode 1 (plain convolution, f2): D = +M; the science image is not read and there is no background (NB = 0)
+        const double scale = (mode ? -1.0 : 1.0) / ((double)Hx * (double)My), inx = 1.0 / (double)nx;
+        const size_t ro = (size_t)y * nx;
         if (vec) {
-            const double2 sv = mode ? make_double2(0.0, 0.0) : *reinterpret_cast<const double2 *>(S + ro + x0);
-            double2 o; o.x = sv.x - scale * v[q].x - ba; o.y = sv.y - scale * v[q].y - bb;
-            *reinterpret_cast<double2 *>(D + ro + x0) = o;
+            // all loads of a batch first, then arithmetic and stores: one memory round trip per batch, not per pixel pair
+#pragma unroll
+            for (int h = 0; h < 4; h++) {
+                double2 sv[4];
+#pragma unroll
+                for (int qq = 0; qq < 4; qq++) {
+                    const int x0 = 2 * (j + (4 * h + qq) * T);
+                    sv[qq] = (mode == 0 && x0 < nx) ? __ldcs(reinterpret_cast<const double2 *>(S + ro + x0)) : make_double2(0.0, 0.0);
+                }
+#pragma unroll
+                for (int qq = 0; qq < 4; qq++) {
+                    const int q = 4 * h + qq, x0 = 2 * (j + q * T);
+                    const double xa = (2.0 * x0 + 1.0 - nx) * inx, xb = (2.0 * x0 + 3.0 - nx) * inx;
+                    const double ba = fma(fma(fma(cx[3], xa, cx[2]), xa, cx[1]), xa, cx[0]);
+                    const double bb = fma(fma(fma(cx[3], xb, cx[2]), xb, cx[1]), xb, cx[0]);
+                    double2 o; o.x = sv[qq].x - scale * v[q].x - ba; o.y = sv[qq].y - scale * v[q].y - bb;
+                    if (x0 < nx) __stcs(reinterpret_cast<double2 *>(D + ro + x0), o);
+                }
+            }
         } else {
-            D[ro + x0] = (mode ? 0.0 : S[ro + x0]) - scale * v[q].x - ba;
-            if (x0 + 1 < nx) D[ro + x0 + 1] = (mode ? 0.0 : S[ro + x0 + 1]) - scale * v[q].y - bb;
+#pragma unroll
+            for (int q = 0; q < 16; q++) {
+                const int x0 = 2 * (j + q * T);
+                if (x0 >= nx) continue;
+                const double xa = (2.0 * x0 + 1.0 - nx) * inx, xb = (2.0 * x0 + 3.0 - nx) * inx;
+                const double ba = fma(fma(fma(cx[3], xa, cx[2]), xa, cx[1]), xa, cx[0]);
+                const double bb = fma(fma(fma(cx[3], xb, cx[2]), xb, cx[1]), xb, cx[0]);
+                D[ro + x0] = (mode ? 0.0 : S[ro + x0]) - scale * v[q].x - ba;
+                if (x0 + 1 < nx) D[ro + x0 + 1] = (mode ? 0.0 : S[ro + x0 + 1]) - scale * v[q].y - bb;
+            }
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------ host side
 template <int LOG2H> static cudaError_t rows_attr() {
-    cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<LOG2H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM);
-    return e;
-}
-cudaError_t rows_init() { // per device, at plan creation
-    cudaError_t e = rows_attr<9>();
-    if (e == cudaSuccess) e = rows_attr<10>();
-    if (e == cudaSuccess) e = rows_attr<11>();
+    cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<LOG2H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_I);
     return e;
 }
 
-cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI, double *mu, int NMOM) {
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// per device and plan, at plan creation: kernel attributes and the tensor map of the a5 intermediate
+// (plane [Hx][My] complex = [Hx][2 My] doubles, box {4 doubles = rows y0, y0+1 of one kx; Hx/8 kx})
+cudaError_t rows_init(sfft_plan *p) {
     const Geom &g = p->g;
+    cudaError_t e = rows_attr<9>();
+    if (e == cudaSuccess) e = rows_attr<10>();
+    if (e == cudaSuccess) e = rows_attr<11>();
+    if (e != cudaSuccess) return e;
+    void *fn = nullptr; cudaDriverEntryPointQueryResult qr;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+    if (e != cudaSuccess) return e;
+    if (!fn || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    p->mapI = new (std::nothrow) CUtensorMap();
+    if (!p->mapI) return cudaErrorMemoryAllocation;
+    cuuint64_t dims[2] = {2 * (cuuint64_t)g.My, (cuuint64_t)g.Hx}, strides[1] = {(cuuint64_t)g.My * 16};
+    cuuint32_t box[2] = {4, (cuuint32_t)(g.Hx / 8)}, es[2] = {1, 1};
+    CUresult r = ((EncodeTiledFn)fn)(p->mapI, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void *)p->inter, dims, strides, box, es,
+                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+void rows_free(sfft_plan *p) { delete p->mapI; p->mapI = nullptr; }
+
+template <int LOG2H> static int row_grid(const sfft_plan *p) {
+    const int need = ((p->g.ny + 1) / 2 + RowCfg<LOG2H>::RP - 1) / RowCfg<LOG2H>::RP, cap = 2 * p->sms;
+    return need < cap ? need : cap;
+}
+
+template <int LOG2H>
+static void run_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI, double *mu, int NMOM) {
+    const Geom &g = p->g;
+    const bool bulk = ((g.nx & 1) == 0) && (((size_t)img & 15) == 0);
+    const int grid = row_grid<LOG2H>(p);
+    const size_t sm = RowCfg<LOG2H>::SMEM_F;
+    if (bulk && !mask) row_fwd_kernel<LOG2H, true, false><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+    else if (bulk) row_fwd_kernel<LOG2H, true, true><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+    else if (!mask) row_fwd_kernel<LOG2H, false, false><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+    else row_fwd_kernel<LOG2H, false, true><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+}
+
+cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI, double *mu, int NMOM) {
     KLaunch kl(p, NI > 1 ? "row_fwd_R" : "row_fwd_S");
-    switch (g.log2Hx) {
-    case 9: row_fwd_kernel<9><<<(g.ny + 2 * RowCfg<9>::RP - 1) / (2 * RowCfg<9>::RP), ROW_THREADS, RowCfg<9>::SMEM, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw); break;
-    case 10: row_fwd_kernel<10><<<(g.ny + 2 * RowCfg<10>::RP - 1) / (2 * RowCfg<10>::RP), ROW_THREADS, RowCfg<10>::SMEM, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw); break;
-    case 11: row_fwd_kernel<11><<<(g.ny + 2 * RowCfg<11>::RP - 1) / (2 * RowCfg<11>::RP), ROW_THREADS, RowCfg<11>::SMEM, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw); break;
+    switch (p->g.log2Hx) {
+    case 9: run_row_fwd<9>(p, img, mask, inter, NI, mu, NMOM); break;
+    case 10: run_row_fwd<10>(p, img, mask, inter, NI, mu, NMOM); break;
+    case 11: run_row_fwd<11>(p, img, mask, inter, NI, mu, NMOM); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
 }
 
+// inter must be the plan's intermediate buffer (the tensor map is built over it)
 cudaError_t launch_row_inv(sfft_plan *p, const cplx *inter, const double *S, const double *coef, double *D, int mode) {
     const Geom &g = p->g;
+    if (inter != p->inter) return cudaErrorInvalidValue;
     KLaunch kl(p, "row_inv");
     switch (g.log2Hx) {
-    case 9: row_inv_kernel<9><<<(g.ny + 2 * RowCfg<9>::RP - 1) / (2 * RowCfg<9>::RP), ROW_THREADS, RowCfg<9>::SMEM, p->stream>>>(inter, S, coef, D, g, p->tw, mode); break;
-    case 10: row_inv_kernel<10><<<(g.ny + 2 * RowCfg<10>::RP - 1) / (2 * RowCfg<10>::RP), ROW_THREADS, RowCfg<10>::SMEM, p->stream>>>(inter, S, coef, D, g, p->tw, mode); break;
-    case 11: row_inv_kernel<11><<<(g.ny + 2 * RowCfg<11>::RP - 1) / (2 * RowCfg<11>::RP), ROW_THREADS, RowCfg<11>::SMEM, p->stream>>>(inter, S, coef, D, g, p->tw, mode); break;
+    case 9: row_inv_kernel<9><<<row_grid<9>(p), ROW_THREADS, RowCfg<9>::SMEM_I, p->stream>>>(*p->mapI, S, coef, D, g, p->tw, mode); break;
+    case 10: row_inv_kernel<10><<<row_grid<10>(p), ROW_THREADS, RowCfg<10>::SMEM_I, p->stream>>>(*p->mapI, S, coef, D, g, p->tw, mode); break;
+    case 11: row_inv_kernel<11><<<row_grid<11>(p), ROW_THREADS, RowCfg<11>::SMEM_I, p->stream>>>(*p->mapI, S, coef, D, g, p->tw, mode); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
