@@ -134,52 +134,39 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------
 # the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference)
 # ------------------------------------------------------------------------------------------
-def oracle_step(S, R, crop, L, DK, DB):
-    """The oracle's whole path (direct-sum build_system, textbook Cholesky, real-space subtract) on
-    the top-left crop x crop corner of the pair.  Returns seconds of (build, solve, subtract)."""
+def oracle_step(S, R, L, DK, DB):
+    """The oracle's whole path (direct-sum build_system, textbook Cholesky, real-space subtract) on the full pair,
+    as it stands.  Returns seconds of (build, solve, subtract)."""
     import oracle
-    s = np.ascontiguousarray(S[:crop, :crop])
-    r = np.ascontiguousarray(R[:crop, :crop])
     t0 = time.perf_counter()
-    G, h = oracle.build_system(s, r, None, L, DK, DB)
+    G, h = oracle.build_system(S, R, None, L, DK, DB)
     t1 = time.perf_counter()
     c = oracle.solve(G, h)
     t2 = time.perf_counter()
-    oracle.subtract(s, r, L, DK, DB, c)
+    oracle.subtract(S, R, L, DK, DB, c)
     t3 = time.perf_counter()
     return t1 - t0, t2 - t1, t3 - t2
 
 
-def oracle_full_frame_seconds(tb, ts, tsub, crop, nx, ny):
-    """build and subtract are sums over pixels (linear in the pixel count), the solve is not."""
-    scale = (nx * ny) / float(crop * crop)
-    return (tb + tsub) * scale + ts
+def config_dict(cfg, world):
+    """The `config` object of the JSON line: identical for both arms (the driver compares them)."""
+    return dict(cfg, parallelism=f"replicas x{world}" if world > 1 else "single GPU",
+                l2="inputs larger than L2: S, R 134 MB each, ~5 GB streamed per step vs 126 MB L2; no flush")
 
 
-def pick_crop(S, R, L, DK, DB, budget_s, nsteps):
-    """Largest crop in {2044, 1022, 511} whose nsteps oracle passes fit budget_s (calibrated on 511)."""
-    tb, ts, tsub = oracle_step(S, R, 511, L, DK, DB)
-    per_pix = (tb + tsub) / (511.0 * 511.0)
-    for crop in (2044, 1022):
-        if nsteps * (per_pix * crop * crop + ts) <= budget_s:
-            return crop
-    return 511
-
-
-def cpu_baseline(S, R, cfg, budget_s=25.0):
+def cpu_baseline(S, R, cfg):
+    """One FULL oracle step on the same pair (about 15 s on 16 cores: the bounded sample is the whole workload)."""
     import oracle
-    crop = pick_crop(S, R, cfg["L"], cfg["DK"], cfg["DB"], budget_s, 1)
-    tb, ts, tsub = oracle_step(S, R, crop, cfg["L"], cfg["DK"], cfg["DB"])
-    full = oracle_full_frame_seconds(tb, ts, tsub, crop, cfg["nx"], cfg["ny"])
+    tb, ts, tsub = oracle_step(S, R, cfg["L"], cfg["DK"], cfg["DB"])
+    full = tb + ts + tsub
     return {"value": 1.0 / full, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"oracle build_system+solve+subtract on the top-left {crop}x{crop} crop of the same pair "
-                      f"({tb + ts + tsub:.2f} s); pixel-linear stages scaled by {cfg['nx'] * cfg['ny'] / crop / crop:.1f} "
-                      f"to 4088x4088, Cholesky (n={cfg['n']}) unscaled",
-            "seconds_sample": round(tb + ts + tsub, 3), "seconds_full_frame_est": round(full, 2)}
+            "sample": f"one full step (oracle build_system {tb:.2f} s + solve {ts:.2f} s + subtract {tsub:.2f} s) on the "
+                      f"same 4088x4088 pair; nothing scaled",
+            "seconds_full_frame": round(full, 3)}
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores, same config/metric; rank 0 only."""
+    """--impl reference: the oracle on the host cores, same config/metric, the full step every step; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return 0
     import oracle
@@ -187,22 +174,18 @@ def run_reference(args):
     cfg = dict(WORKLOAD)
     pair = starfield.make_pair(2)
     S, R = pair["S"], pair["R"]
-    crop = pick_crop(S, R, cfg["L"], cfg["DK"], cfg["DB"], 150.0, args.steps + args.warmup)
     for _ in range(args.warmup):
-        oracle_step(S, R, crop, cfg["L"], cfg["DK"], cfg["DB"])
-    tot, raw = 0.0, 0.0
+        oracle_step(S, R, cfg["L"], cfg["DK"], cfg["DB"])
+    t0 = time.perf_counter()
     for _ in range(args.steps):
-        tb, ts, tsub = oracle_step(S, R, crop, cfg["L"], cfg["DK"], cfg["DB"])
-        tot += oracle_full_frame_seconds(tb, ts, tsub, crop, cfg["nx"], cfg["ny"])
-        raw += tb + ts + tsub
-    sec = tot / args.steps
+        oracle_step(S, R, cfg["L"], cfg["DK"], cfg["DB"])
+    sec = (time.perf_counter() - t0) / args.steps
     val = 1.0 / sec
-    sample = (f"each step = oracle build_system+solve+subtract on the top-left {crop}x{crop} crop "
-              f"({raw / args.steps:.2f} s measured), pixel-linear stages scaled to 4088x4088")
+    sample = f"each step = the full oracle build_system+solve+subtract on the 4088x4088 pair ({sec:.2f} s measured); nothing scaled"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": dict(cfg, l2="n/a (CPU)"),
+            "config": config_dict(cfg, int(os.environ.get("WORLD_SIZE", str(args.gpus)))),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -229,10 +212,16 @@ def replica_throughput(world, ms_per_step):
 
 
 def ncu_traffic(kernel):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.json)."""
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.json).  The
+    capture is stamped with the hash of the kernel sources it was taken from; a different tree gets null, not a stale
+    number."""
     f = ROOT / "profiles" / "ncu_traffic.json"
     try:
-        return json.loads(f.read_text())["kernels"][kernel]["dram_bytes_per_launch"]
+        from paper_2509_18544_b200.build import source_hash
+        d = json.loads(f.read_text())
+        if d.get("csrc_sha256") != source_hash():
+            return None
+        return d["kernels"][kernel]["dram_bytes_per_launch"]
     except Exception:
         return None
 
@@ -318,8 +307,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": dict(cfg, parallelism=f"replicas x{world}" if world > 1 else "single GPU",
-                           l2="inputs larger than L2: S, R 134 MB each, ~5 GB streamed per step vs 126 MB L2; no flush"),
+            "config": config_dict(cfg, world),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(2 * nx * ny * 8),
                     "d2h_bytes_per_step": int(nx * ny * 8 + cfg["n"] * 8), "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": int(launches), "clocks": clk, "library": sfft.version(),
@@ -372,27 +360,48 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
            "kernels_ms": {k: round(v, 4) for k, v in sorted(kernels.items(), key=lambda kv: -kv[1])},
            "kernel_launches_per_step": kcnt}
 
-    # dominant kernel among those that stream images/spectra
+    # FP64 rates of this box (the ALU roofline of a2 and a4)
+    try:
+        out["fp64_probe_tflops"] = {"dfma": round(sfft.probe_fp64(0), 2), "dmma_m8n8k4": round(sfft.probe_fp64(1), 2)}
+    except Exception as e:  # pragma: no cover
+        out["fp64_probe_tflops"] = {"error": str(e)}
+    # dominant kernel among those that stream images/spectra.  The Omega lag pass is bound by FP64 instruction issue, not
+    # by HBM (21 pairs x (16 products + 16-point DFT + 21 folded lags) per 16 spectrum elements =
+    # 308/16 FP64 instructions per element and pair, counted as 2 flop each against the probed DFMA rate): if it is the
+    # dominant kernel the line says "alu"; the dominant HBM-bound kernel is reported beside it either way.
     hbm_kernels = {k: v for k, v in kernels.items() if k in kbytes}
     dom = max(hbm_kernels, key=hbm_kernels.get)
-    per_launch_ms = kernels[dom] / kcnt[dom]
-    ach = kbytes[dom] / (per_launch_ms * 1e-3) / 1e9
-    out["roofline"] = {"kernel": dom, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
-                       "frac": round(ach / peak, 4), "traffic": ncu_traffic(dom), "peak_source": peak_src,
-                       "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": round(per_launch_ms, 4),
-                       "share_of_step": round(kernels[dom] / sum(kernels.values()), 3)}
+
+    def hbm_line(kn):
+        per_launch_ms = kernels[kn] / kcnt[kn]
+        ach = kbytes[kn] / (per_launch_ms * 1e-3) / 1e9
+        return {"kernel": kn, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(ach / peak, 4), "traffic": ncu_traffic(kn), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": kbytes[kn], "ms_per_launch": round(per_launch_ms, 4),
+                "share_of_step": round(kernels[kn] / sum(kernels.values()), 3)}
+    if dom == "lagcol_omega" and "dfma" in out["fp64_probe_tflops"]:
+        npair = NK * (NK + 1) // 2
+        flop = npair * 4096.0 * 2049.0 * (64 + 160 + 84) / 16.0 * 2.0
+        ms_l = kernels[dom] / kcnt[dom]
+        pk = out["fp64_probe_tflops"]["dfma"]
+        out["roofline"] = {"kernel": dom, "bound": "alu", "achieved": round(flop / ms_l / 1e9, 2), "peak": pk, "unit": "TFLOP/s",
+                           "frac": round(flop / ms_l / 1e9 / pk, 4), "traffic": ncu_traffic(dom),
+                           "peak_source": "measured (sfft_probe_fp64: register-resident DFMA loop on every SM)",
+                           "algorithmic_flop_per_launch": flop, "ms_per_launch": round(ms_l, 4),
+                           "share_of_step": round(kernels[dom] / sum(kernels.values()), 3),
+                           "hbm_view": hbm_line(dom)}
+        rest = {k: v for k, v in hbm_kernels.items() if k != dom}
+        out["roofline_hbm_dominant"] = hbm_line(max(rest, key=rest.get))
+    else:
+        out["roofline"] = hbm_line(dom)
+    out["kernel_rooflines"] = {k: {"ms": round(kernels[k] / kcnt[k], 4), "frac_of_measured_hbm": round(kbytes[k] / (kernels[k] / kcnt[k]) / 1e6 / peak, 4)}
+                               for k in hbm_kernels}
     t_path = sum(stages[k] for k in ("a1_template", "a1_science", "a2_omega", "a2_theta", "a3_gather", "a5_subtract"))
     out["path_roofline"] = {"what": "a1+a2+a3+a5 (BASELINE.json target: >= 0.60)", "algorithmic_bytes": path_bytes,
                             "ms": round(t_path, 4), "achieved_gbs": round(path_bytes / t_path / 1e6, 1),
                             "frac_of_measured": round(path_bytes / t_path / 1e6 / peak, 4),
                             "frac_of_nominal_7.7TBs": round(path_bytes / t_path / 1e6 / NOMINAL_HBM_GBS, 4),
                             "a4_ms": round(stages["a4_factor"] + stages["a4_solve"], 4)}
-    # FP64 rates of this box (the ALU roofline of a2 and a4)
-    try:
-        out["fp64_probe_tflops"] = {"dfma": round(sfft.probe_fp64(0), 2), "dmma_m8n8k4": round(sfft.probe_fp64(1), 2)}
-    except Exception as e:  # pragma: no cover
-        out["fp64_probe_tflops"] = {"error": str(e)}
-
     # f2: cross-convolution S (*) psf_R, R (*) psf_S with L x L stamps on the same plan.
     # Algorithmic bytes per convolution: image 1 r + row intermediate 1 r written and read + spectrum 1 r written and
     # read + inverse intermediate 1 r written and read + output 1 r = 8 r.  The oracle is timed on a bounded crop.
@@ -596,32 +605,9 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
         D_arg = [D_list[b % len(D_list)] for b in range(B)]
         cb = torch.empty((B, cfg["n"]), dtype=torch.float64, device="cuda")
         stream = torch.cuda.current_stream()
-        for _ in range(2):
-            plan.set_template(dR)
-            plan.subtract_batch(S_list[:2], D_arg[:2], cb[:2].contiguous())
-        torch.cuda.synchronize()
         e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-        e[0].record(stream)
-        plan.set_template(dR)
-        e[1].record(stream)
-        plan.subtract_batch(S_list, D_arg, cb)
-        e[2].record(stream)
-        torch.cuda.synchronize()
-        plan.sync_status()
-        t_t, t_b = e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
-        r = nx * ny * 8.0
-        # per image: a1 of S 4 r, Theta (NK + 4)/4 r (four images share one pass over the NK template spectra), a5 (NK + 4) r
-        per_img_bytes = (4 + (NK + 4) / 4.0 + (NK + 4)) * r + (13 + NK) * r / B
-        out["batched"] = {"workload": f"BASELINE.json configs[3]: one template, B={B} science images "
-                                      f"({len(Ss)} distinct seeded images cycled)",
-                          "B": B, "template_ms": round(t_t, 3), "per_image_ms": round(t_b / B, 4),
-                          "images_per_s": round(B * 1e3 / (t_t + t_b), 1),
-                          "frac_of_measured_hbm": round(per_img_bytes / ((t_t + t_b) / B) / 1e6 / peak, 4)}
-        # the same batch in the constant-photometric-ratio plan mode (f4): auxiliary solves once per template
-        try:
-            plan.set_constant_ratio(True)
-            plan.set_template(dR); plan.subtract_batch(S_list[:2], D_arg[:2], cb[:2].contiguous())
-            torch.cuda.synchronize()
+
+        def batch_once():
             e[0].record(stream)
             plan.set_template(dR)
             e[1].record(stream)
@@ -629,12 +615,132 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
             e[2].record(stream)
             torch.cuda.synchronize()
             plan.sync_status()
-            t_t2, t_b2 = e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
+            return e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
+        batch_once()                                           # warm-up with the FULL batch (nothing is allocated after
+        reps = [batch_once() for _ in range(5)]                # plan creation, but clocks and caches settle)
+        t_t, t_b = float(np.median([a for a, _ in reps])), float(np.median([b for _, b in reps]))
+        r = nx * ny * 8.0
+        # per image: a1 of S 4 r, Theta (NK + 4)/4 r (four images share one pass over the NK template spectra), a5 (NK + 4) r
+        per_img_bytes = (4 + (NK + 4) / 4.0 + (NK + 4)) * r + (13 + NK) * r / B
+        out["batched"] = {"workload": f"BASELINE.json configs[3]: one template, B={B} science images "
+                                      f"({len(Ss)} distinct seeded images cycled)",
+                          "B": B, "repetitions": 5, "template_ms": round(t_t, 3), "per_image_ms": round(t_b / B, 4),
+                          "per_image_ms_all_reps": [round(b / B, 4) for _, b in reps],
+                          "images_per_s": round(B * 1e3 / (t_t + t_b), 1),
+                          "frac_of_measured_hbm": round(per_img_bytes / ((t_t + t_b) / B) / 1e6 / peak, 4)}
+        # the same batch in the constant-photometric-ratio plan mode (f4): auxiliary solves once per template
+        try:
+            plan.set_constant_ratio(True)
+            batch_once()
+            reps2 = [batch_once() for _ in range(5)]
+            t_t2, t_b2 = float(np.median([a for a, _ in reps2])), float(np.median([b for _, b in reps2]))
             out["batched"]["constant_ratio_mode"] = {"template_ms": round(t_t2, 3), "per_image_ms": round(t_b2 / B, 4),
                                                      "images_per_s": round(B * 1e3 / (t_t2 + t_b2), 1)}
         except Exception as ex:  # pragma: no cover
             out["batched"]["constant_ratio_mode"] = {"error": str(ex)}
         plan.set_constant_ratio(False)
+
+    # a4 on its own (BASELINE.json north_star: "FP64 tensor-pipe utilisation for the solve"): the factorisation of the
+    # n = 732 system as sfft_set_template runs it (alone on the machine, stage timer), n^3/3 flop against the probed DMMA rate
+    try:
+        dmma = out.get("fp64_probe_tflops", {}).get("dmma_m8n8k4")
+        fa = []
+        for _ in range(5):
+            plan.enable_timings(1)
+            plan.set_template(dR)
+            fa.append(plan.get_timings()["a4_factor"])
+        plan.enable_timings(0)
+        step()
+        n = cfg["n"]
+        ms_f = float(np.median(fa))
+        out["a4"] = {"n": n, "flops": n ** 3 / 3.0, "factor_ms_alone": round(ms_f, 4),
+                     "factor_ms_beside_science_side": out["stages_ms"]["a4_factor"], "solve_ms": out["stages_ms"]["a4_solve"],
+                     "achieved_tflops": round(n ** 3 / 3.0 / ms_f / 1e9, 3),
+                     "frac_of_dmma_probe": round(n ** 3 / 3.0 / ms_f / 1e9 / dmma, 4) if dmma else None,
+                     "bound": "latency (a 732-step dependent chain; 0.13 GFLOP)"}
+    except Exception as ex:  # pragma: no cover
+        out["a4"] = {"error": str(ex)}
+
+    # cuFFT beside the product's transforms (BASELINE.json north_star: "cuFFT timed only as a comparison, never on the product
+    # path"): torch.fft.rfft2 / irfft2 of one zero-padded 4096 x 4096 FP64 frame against row_fwd_S + col_fwd_S and col_inv + row_inv
+    try:
+        pad = torch.zeros((4096, 4096), dtype=torch.float64, device="cuda"); pad[:ny, :nx] = dS
+        for _ in range(3):
+            sp_ = torch.fft.rfft2(pad); back = torch.fft.irfft2(sp_, s=pad.shape)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        tf, ti = [], []
+        for _ in range(K):
+            ev[0].record(stream); sp_ = torch.fft.rfft2(pad); ev[1].record(stream); back = torch.fft.irfft2(sp_, s=pad.shape); ev[2].record(stream)
+            torch.cuda.synchronize()
+            tf.append(ev[0].elapsed_time(ev[1])); ti.append(ev[1].elapsed_time(ev[2]))
+        del pad, sp_, back
+        r = nx * ny * 8.0
+        ours_f = kernels.get("row_fwd_S", 0.0) + kernels.get("col_fwd_S", 0.0)
+        ours_i = kernels.get("col_inv", 0.0) + kernels.get("row_inv", 0.0)
+        out["cufft_compare"] = {"what": "comparison only, never on the product path: torch.fft (cuFFT) FP64 rfft2 / irfft2 of one 4096 x 4096 frame",
+                                "cufft_rfft2_ms": round(float(np.median(tf)), 4), "cufft_irfft2_ms": round(float(np.median(ti)), 4),
+                                "cufft_rfft2_frac_of_measured_hbm_4r": round(4 * r / float(np.median(tf)) / 1e6 / peak, 4),
+                                "ours_row_fwd_S_plus_col_fwd_S_ms": round(ours_f, 4),
+                                "ours_fwd_frac_of_measured_hbm_4r": round(4 * r / ours_f / 1e6 / peak, 4) if ours_f else None,
+                                "ours_col_inv_plus_row_inv_ms": round(ours_i, 4),
+                                "note": "ours inverse = NK = 6 spectra combined with the synthesised kernel spectra + the fused subtraction (10 r), cuFFT inverse = one plain transform (4 r)"}
+    except Exception as ex:  # pragma: no cover
+        out["cufft_compare"] = {"error": str(ex)}
+
+    # BASELINE.json configs[4] (large kernel: L = 21, DK = 3, n = 4416): one more plan, the seeded pair of the config
+    if args.large:
+        try:
+            from paper_2509_18544_b200 import SfftPlan as _Plan
+            c4 = starfield.make_pair(4)
+            d4S, d4R = torch.from_numpy(c4["S"]).cuda(), torch.from_numpy(c4["R"]).cuda()
+            p4 = _Plan(nx, ny, c4["L"], c4["DK"], c4["DB"])
+            o4 = torch.empty_like(d4S)
+
+            def step4():
+                p4.build_system(d4S, d4R); p4.solve(); p4.subtract(o4)
+            for _ in range(2):
+                step4()
+            p4.sync_status()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(5):
+                step4()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms4 = e0.elapsed_time(e1) / 5
+            st4 = {}
+            for _ in range(3):
+                p4.enable_timings(1); step4()
+                for k_, v_ in p4.get_timings().items():
+                    st4.setdefault(k_, []).append(v_)
+            st4 = {k_: round(float(np.median(v_)), 4) for k_, v_ in st4.items()}
+            p4.enable_timings(2); step4()
+            k4 = {}
+            for name, ms in p4.kernel_timings():
+                k4[name] = k4.get(name, 0.0) + ms
+            p4.enable_timings(0)
+            n4 = p4.n
+            NK4, W4 = 10, 20
+            dfma = out.get("fp64_probe_tflops", {}).get("dfma"); dmma = out.get("fp64_probe_tflops", {}).get("dmma_m8n8k4")
+            # Omega pass: 55 pairs x 4096 x 2049 elements, two lag halves; per 16 elements and half: 16 products (64) +
+            # 16-point DFT (160) + 21 lags folded (84) FP64 instructions, 2 flop each
+            om_flop = 55 * 4096.0 * 2049 * 2 * (64 + 160 + 84) / 16.0 * 2
+            om_ms = k4.get("lagcol_omega", 0.0)
+            fac_ms = st4.get("a4_factor", 0.0)
+            out["large_kernel"] = {"workload": "BASELINE.json configs[4]: 4088x4088 pair, L=21, DK=3, DB=2 (n=4416)", "n": n4,
+                                   "ms_per_step": round(ms4, 4), "images_per_s": round(1e3 / ms4, 2), "stages_ms": st4,
+                                   "kernels_ms": {k_: round(v_, 4) for k_, v_ in sorted(k4.items(), key=lambda kv: -kv[1])[:10]},
+                                   "a2_omega_lagcol": {"ms": round(om_ms, 4), "fp64_flop": om_flop,
+                                                       "frac_of_dfma_probe": round(om_flop / om_ms / 1e9 / dfma, 4) if dfma and om_ms else None},
+                                   "a4_factor": {"ms": fac_ms, "flops": n4 ** 3 / 3.0,
+                                                 "achieved_tflops": round(n4 ** 3 / 3.0 / fac_ms / 1e9, 3) if fac_ms else None,
+                                                 "frac_of_dmma_probe": round(n4 ** 3 / 3.0 / fac_ms / 1e9 / dmma, 4) if dmma and fac_ms else None},
+                                   "workspace_gb": round(p4.workspace_bytes / 1e9, 3)}
+            p4.destroy()
+            del d4S, d4R, o4
+        except Exception as ex:  # pragma: no cover
+            out["large_kernel"] = {"error": str(ex)}
     return out
 
 
@@ -645,6 +751,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=32, help="science images of the batched (configs[3]) extra; 0 = skip")
+    ap.add_argument("--large", type=int, default=1, help="1: also run BASELINE.json configs[4] (n = 4416) as the `large_kernel` extra")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -89,6 +89,14 @@ enum {
  * Errors: INVALID_ARG, ALLOC, CUDA (no usable device). */
 sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int DB);
 
+/* The same with option flags.  SFFT_PLAN_FP32_SPECTRA: the reduced-memory mode (PAPER.md:105, 113 name GPU memory as
+ * the barrier) -- the spectra (the plan's largest buffers: NK + 4 planes) are STORED as complex64,
+ * all arithmetic and every other buffer stay FP64.  Halves the spectrum memory and the bytes the lag passes and the
+ * subtraction read; the loosened tolerances this costs are stated as numbers in DESIGN.md (reduced-memory mode) and
+ * asserted by tests/test_gpu_fp32_spectra.py.  Unknown flag bits: INVALID_ARG. */
+#define SFFT_PLAN_FP32_SPECTRA 1u
+sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, int DB, unsigned flags);
+
 /* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream). */
 sfft_status sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
 
@@ -228,6 +236,17 @@ sfft_status sfft_decorrelation_stamp(sfft_plan *plan, const double *K, int Lk, c
  * SYNCHRONISES.  Returns NOT_SPD if the pivot test failed. */
 sfft_status sfft_difference_host(sfft_plan *plan, const double *S_host, const double *R_host,
                                  const uint8_t *mask_host, double *D_host, double *coeffs_host);
+
+/* The batched path (BASELINE.json configs[3]; every template against many science images; PAPER.md:101:
+ * "holds all data in-memory to minimize time spent on file I/O") from HOST buffers: R_host (and mask_host, may be NULL)
+ * go up once and sfft_set_template runs; then the B science images S_host[b] (HOST array of B host pointers, ny*nx
+ * doubles each) stream through a three-deep pipeline -- upload of image b+1 | a1, Theta, solve, a5 of image b |
+ * download of D of image b-1 -- on two plan-owned copy streams beside the plan's stream, one cudaMemcpyAsync per
+ * buffer.  D_host[b]: B host pointers (ny*nx doubles each); coeffs_host: B*n doubles or NULL.  Pinned host memory is
+ * needed for the copies to overlap.  Allocates seven frame-sized staging buffers on first use; SYNCHRONISES.
+ * Errors: INVALID_ARG, ALLOC, CUDA, NOT_SPD. */
+sfft_status sfft_difference_host_batch(sfft_plan *plan, const double *R_host, const uint8_t *mask_host,
+                                       const double *const *S_host, int B, double *const *D_host, double *coeffs_host);
 
 /* ---- introspection for tests and bench ------------------------------------------------ */
 

@@ -29,6 +29,15 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def source_hash() -> str:
+    """sha256 over the kernel sources and headers (name + content, sorted): stamps profiles taken from this tree."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + [HERE.parent / "include" / "sfft.h"]):
+        h.update(f.name.encode()); h.update(f.read_bytes())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
     if not LIB.exists():
         return True

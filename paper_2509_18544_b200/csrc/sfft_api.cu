@@ -94,6 +94,11 @@ static void free_plan(sfft_plan *p) {
     if (p->fstream) cudaStreamDestroy(p->fstream);
     if (p->ev_ffork) cudaEventDestroy(p->ev_ffork);
     if (p->cstream) cudaStreamDestroy(p->cstream);
+    if (p->ostream) cudaStreamDestroy(p->ostream);
+    for (int k = 0; k < 3; k++) {
+        if (p->hbS[k]) cudaFree(p->hbS[k]); if (p->hbD[k]) cudaFree(p->hbD[k]); if (p->hbC[k]) cudaFree(p->hbC[k]);
+        if (p->ev_hin[k]) cudaEventDestroy(p->ev_hin[k]); if (p->ev_hcomp[k]) cudaEventDestroy(p->ev_hcomp[k]); if (p->ev_hout[k]) cudaEventDestroy(p->ev_hout[k]);
+    }
     if (p->ev_copy) cudaEventDestroy(p->ev_copy);
     if (p->ev_fjoin) cudaEventDestroy(p->ev_fjoin);
     if (p->fstream2) cudaStreamDestroy(p->fstream2);
@@ -111,7 +116,12 @@ extern "C" {
 const char *sfft_version(void) { return "sfft-b200 0.1 (sm_100a)"; }
 
 sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int DB) {
+    return sfft_plan_create_ex(out, nx, ny, L, DK, DB, 0u);
+}
+
+sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, int DB, unsigned flags) {
     if (!out) return SFFT_ERR_INVALID_ARG;
+    if (flags & ~(unsigned)SFFT_PLAN_FP32_SPECTRA) return SFFT_ERR_INVALID_ARG;
     *out = nullptr;
     if (L < 1 || L > MAX_L || !(L & 1) || DK < 0 || DK > MAX_DEG || DB < 0 || DB > MAX_DEG) return SFFT_ERR_INVALID_ARG;
     if (nx < 2 * L - 1 || ny < 2 * L - 1 || nx > SFFT_MAX_SIDE || ny > SFFT_MAX_SIDE) return SFFT_ERR_INVALID_ARG;
@@ -120,6 +130,7 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
     sfft_plan *p = new (std::nothrow) sfft_plan();
     if (!p) return SFFT_ERR_ALLOC;
     memset(p, 0, sizeof(*p));
+    p->spec32 = (flags & SFFT_PLAN_FP32_SPECTRA) != 0; p->spec_esz = p->spec32 ? 8 : 16;
     Geom &g = p->g;
     g.nx = nx; g.ny = ny; g.L = L; g.w = (L - 1) / 2; g.DK = DK; g.DB = DB;
     g.NK = (DK + 1) * (DK + 2) / 2; g.NB = (DB + 1) * (DB + 2) / 2; g.n = L * L * g.NK + g.NB;
@@ -152,18 +163,20 @@ sfft_status sfft_plan_create(sfft_plan **out, int nx, int ny, int L, int DK, int
         if (cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || p->sms <= 0) p->sms = 148;
     }
     // lag-pass launch shapes first: they size Q
-    lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &p->cfgO);
-    for (int k = 1; k <= NSCI; k++) lagcol_config(g, k * g.NK, g.NK + k, g.w, &p->cfgT[k - 1]);
+    lagcol_config(g, p->plO.np, g.NK, 2 * g.w, &p->cfgO, p->spec_esz);
+    for (int k = 1; k <= NSCI; k++) lagcol_config(g, k * g.NK, g.NK + k, g.w, &p->cfgT[k - 1], p->spec_esz);
     size_t bO = (size_t)border_chunks() * p->plO.np * W2 * W2;
     { const size_t bT2 = (size_t)border_chunks() * NSCI * g.NK * L * L; if (bT2 > bO) bO = bT2; }
     cudaError_t e = cudaSuccess;
 #define AL(ptr, cnt) if (e == cudaSuccess) e = dalloc(p, &ptr, (size_t)(cnt))
     AL(p->tw, g.Nt);
     AL(p->inter, (size_t)(DK + 1) * iplane);
-    AL(p->specT, g.NK * splane);
-    AL(p->specS, splane);
+#define ALB(ptr_, nb_) if (e == cudaSuccess) { e = cudaMalloc(&ptr_, (size_t)(nb_)); if (e == cudaSuccess) p->bytes += (size_t)(nb_); }
+    ALB(p->specT, g.NK * splane * p->spec_esz);
+    ALB(p->specS, splane * p->spec_esz);
     p->specSx[0] = p->specS;
-    for (int i = 1; i < NSCI; i++) AL(p->specSx[i], splane); // batched path: up to NSCI science spectra per Theta pass
+    for (int i = 1; i < NSCI; i++) ALB(p->specSx[i], splane * p->spec_esz); // batched path: up to NSCI science spectra per Theta pass
+#undef ALB
     AL(p->muR, (size_t)(DK + DB + 1) * ny);
     AL(p->muS, (size_t)(DB + 1) * ny);
     for (int i = 1; i < NSCI; i++) AL(p->muSx[i], (size_t)(DB + 1) * ny);
@@ -309,7 +322,9 @@ static sfft_status template_side(sfft_plan *p) {
     {
         StageTimer tm(p, SFFT_STAGE_A1_TEMPLATE);
         if (p->mask && p->specTo == p->specT) { // the subtraction needs spectra of the UNMASKED template (C7): allocated with the first mask
-            CK(dalloc(p, &p->specTo, (size_t)g.NK * g.My * (g.Hx + 1)), "alloc unmasked spectra");
+            const size_t nb = (size_t)g.NK * g.My * (g.Hx + 1) * p->spec_esz;
+            CK(cudaMalloc(&p->specTo, nb), "alloc unmasked spectra");
+            p->bytes += nb;
         }
         if (p->mask) {
             CK(launch_row_fwd(p, p->R, nullptr, p->inter, g.DK + 1, nullptr, 0), "row_fwd(R unmasked)");
@@ -694,6 +709,58 @@ sfft_status sfft_difference_host(sfft_plan *p, const double *S_host, const doubl
     return sfft_sync_status(p);
 }
 
+
+// e2e for configs[3]: one template, B science images, all in HOST memory.  The template goes up once; the images run
+// through a three-deep pipeline  H2D(S_{i+1}) | compute(i) | D2H(D_{i-1})  on two plan-owned copy streams beside the
+// caller's stream, one plain cudaMemcpyAsync per buffer (PCIe is full duplex: the upload of the next image and the
+// download of the previous result overlap each other and the ~0.6 ms of device work).
+sfft_status sfft_difference_host_batch(sfft_plan *p, const double *R_host, const uint8_t *mask_host, const double *const *S_host,
+                                       int B, double *const *D_host, double *coeffs_host) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    if (!R_host || !S_host || !D_host || B < 1) return fail(p, SFFT_ERR_INVALID_ARG, "difference_host_batch: bad arguments");
+    for (int b = 0; b < B; b++) if (!S_host[b] || !D_host[b]) return fail(p, SFFT_ERR_INVALID_ARG, "difference_host_batch: NULL image");
+    const size_t npix = (size_t)p->g.nx * p->g.ny, n = p->g.n;
+    constexpr int NSLOT = 3;
+    if (!p->hbS[0]) { // first use: staging buffers, the download stream, events
+        if (!p->stR) CK(dalloc(p, &p->stR, npix), "alloc staging");
+        for (int k = 0; k < NSLOT; k++) {
+            CK(dalloc(p, &p->hbS[k], npix), "alloc staging"); CK(dalloc(p, &p->hbD[k], npix), "alloc staging");
+            CK(dalloc(p, &p->hbC[k], n), "alloc staging");
+            CK(cudaEventCreateWithFlags(&p->ev_hin[k], cudaEventDisableTiming), "event");
+            CK(cudaEventCreateWithFlags(&p->ev_hcomp[k], cudaEventDisableTiming), "event");
+            CK(cudaEventCreateWithFlags(&p->ev_hout[k], cudaEventDisableTiming), "event");
+        }
+        CK(cudaStreamCreateWithFlags(&p->ostream, cudaStreamNonBlocking), "stream");
+    }
+    if (mask_host && !p->stM) CK(dalloc(p, &p->stM, npix), "alloc staging");
+    // the first science image starts up beside the template
+    CK(cudaEventRecord(p->ev_copy, p->stream), "event");       // everything enqueued before this call is done with the buffers
+    CK(cudaStreamWaitEvent(p->cstream, p->ev_copy, 0), "wait");
+    CK(cudaStreamWaitEvent(p->ostream, p->ev_copy, 0), "wait");
+    if (mask_host) CK(cudaMemcpyAsync(p->stM, mask_host, npix, cudaMemcpyHostToDevice, p->stream), "H2D mask");
+    CK(cudaMemcpyAsync(p->stR, R_host, npix * sizeof(double), cudaMemcpyHostToDevice, p->stream), "H2D R");
+    sfft_status st = sfft_set_template(p, p->stR, mask_host ? p->stM : nullptr);
+    if (st != SFFT_OK) return st;
+    for (int b = 0; b < B; b++) {
+        const int k = b % NSLOT;
+        if (b >= NSLOT) CK(cudaStreamWaitEvent(p->cstream, p->ev_hcomp[k], 0), "wait"); // image b-3 no longer reads hbS[k]
+        CK(cudaMemcpyAsync(p->hbS[k], S_host[b], npix * sizeof(double), cudaMemcpyHostToDevice, p->cstream), "H2D S");
+        CK(cudaEventRecord(p->ev_hin[k], p->cstream), "event");
+        CK(cudaStreamWaitEvent(p->stream, p->ev_hin[k], 0), "wait");
+        if (b >= NSLOT) CK(cudaStreamWaitEvent(p->stream, p->ev_hout[k], 0), "wait");   // D of image b-3 has left hbD[k], hbC[k]
+        const double *Sd = p->hbS[k]; double *Dd = p->hbD[k];
+        st = sfft_subtract_batch(p, &Sd, 1, &Dd, p->hbC[k]);
+        if (st != SFFT_OK) return st;
+        CK(cudaEventRecord(p->ev_hcomp[k], p->stream), "event");
+        CK(cudaStreamWaitEvent(p->ostream, p->ev_hcomp[k], 0), "wait");
+        CK(cudaMemcpyAsync(D_host[b], p->hbD[k], npix * sizeof(double), cudaMemcpyDeviceToHost, p->ostream), "D2H D");
+        if (coeffs_host) CK(cudaMemcpyAsync(coeffs_host + (size_t)b * n, p->hbC[k], n * sizeof(double), cudaMemcpyDeviceToHost, p->ostream), "D2H coeffs");
+        CK(cudaEventRecord(p->ev_hout[k], p->ostream), "event");
+    }
+    CK(cudaStreamSynchronize(p->ostream), "sync downloads");
+    return sfft_sync_status(p);
+}
+
 } // extern "C"
 
 // ------------------------------------------------------------------------------------------
@@ -749,12 +816,12 @@ sfft_status sfft_get_timings(sfft_plan *p, float *ms, int n_stages) {
 sfft_status sfft_debug_read(sfft_plan *p, int which, int idx, void *host_dst, size_t nbytes) {
     if (!p || !host_dst) return SFFT_ERR_INVALID_ARG;
     const Geom &g = p->g;
-    const size_t plane = (size_t)g.My * (g.Hx + 1) * sizeof(cplx);
+    const size_t plane = (size_t)g.My * (g.Hx + 1) * sizeof(cplx), dplane = (size_t)g.My * (g.Hx + 1) * p->spec_esz;
     const int W2 = 4 * g.w + 1, LL = g.L * g.L;
     const void *src = nullptr; size_t sz = 0;
     double dims[2] = {(double)g.Mx, (double)g.My};
     switch (which) {
-    case 0: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->specT + (size_t)idx * g.My * (g.Hx + 1); sz = plane; break;
+    case 0: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = (const char *)p->specT + (size_t)idx * dplane; sz = plane; break;
     case 1: src = p->specS; sz = plane; break;
     case 2: if (idx < 0 || idx >= p->npairsO) return SFFT_ERR_INVALID_ARG; src = p->lagO + (size_t)idx * W2 * W2; sz = sizeof(double) * W2 * W2; break;
     case 3: if (idx < 0 || idx >= g.NK) return SFFT_ERR_INVALID_ARG; src = p->lagT + (size_t)idx * LL; sz = sizeof(double) * LL; break;
@@ -762,17 +829,21 @@ sfft_status sfft_debug_read(sfft_plan *p, int which, int idx, void *host_dst, si
     case 5: src = p->phi; sz = sizeof(double) * g.NB * g.NB; break;
     case 6: src = p->delta; sz = sizeof(double) * g.NB; break;
     case 7: if (nbytes != sizeof(dims)) return SFFT_ERR_INVALID_ARG; memcpy(host_dst, dims, sizeof(dims)); return SFFT_OK;
+    case 8: src = p->inter; sz = (size_t)g.My * g.Hx * sizeof(cplx); break; // plane 0 of the intermediates, raw [Hx][My]
     default: return SFFT_ERR_INVALID_ARG;
     }
     if (nbytes != sz) return fail(p, SFFT_ERR_INVALID_ARG, "debug_read: size mismatch");
     CK(cudaStreamSynchronize(p->stream), "sync");
-    if (which <= 1) { // spectra are column-major on the device (plane_idx): hand them out as [My][Hx+1]
-        cplx *tmp = (cplx *)malloc(sz);
+    if (which <= 1) { // spectra are column-major on the device (plane_idx), complex128 or complex64: hand them out as [My][Hx+1] complex128
+        void *tmp = malloc(dplane);
         if (!tmp) return fail(p, SFFT_ERR_ALLOC, "debug_read: host allocation failed");
-        cudaError_t e = cudaMemcpy(tmp, src, sz, cudaMemcpyDeviceToHost);
+        cudaError_t e = cudaMemcpy(tmp, src, dplane, cudaMemcpyDeviceToHost);
         if (e == cudaSuccess)
             for (int ky = 0; ky < g.My; ky++)
-                for (int kx = 0; kx <= g.Hx; kx++) ((cplx *)host_dst)[(size_t)ky * (g.Hx + 1) + kx] = tmp[plane_idx(ky, kx, g.My)];
+                for (int kx = 0; kx <= g.Hx; kx++) {
+                    const size_t i = plane_idx(ky, kx, g.My);
+                    ((cplx *)host_dst)[(size_t)ky * (g.Hx + 1) + kx] = p->spec32 ? ld_c(((const float2 *)tmp)[i]) : ((const cplx *)tmp)[i];
+                }
         free(tmp);
         CK(e, "debug copy");
         return SFFT_OK;

@@ -75,20 +75,20 @@ __device__ __forceinline__ void col_fft(cplx (&v)[16], cplx *X, int j, int bar_i
 // ------------------------------------------------------------------------------------------ forward
 // grid: persistent, <= 2 CTAs per SM; block 256 = G workers of T threads; dynamic smem ColCfg::SMEM.
 // jobs packed 4 bits each, (ii << 2) | jj: output k = FFT_y(yt^jj * inter[ii]).
-template <int LOG2N>
+template <int LOG2N, typename ST>
 __global__ void __launch_bounds__(COL_THREADS, 2)
-col_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, unsigned long long jpack, int njobs, Geom g,
+col_fwd_kernel(const cplx *__restrict__ inter, ST *__restrict__ spec, unsigned long long jpack, int njobs, Geom g,
                const cplx *__restrict__ tw) {
     using C = ColCfg<LOG2N>;
     constexpr int N = C::N, T = C::T, G = C::G, QE = C::QE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ unsigned long long full[G * COL_RING];
+    __shared__ unsigned long long full[G * COL_RING], done[G * COL_RING];
     const int grp = threadIdx.x / T, j = threadIdx.x - grp * T, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * N;
     cplx *ring = reinterpret_cast<cplx *>(smem_raw) + (size_t)G * N + (size_t)grp * COL_RING * QE;
-    unsigned long long *bar = full + grp * COL_RING;
+    unsigned long long *bar = full + grp * COL_RING, *rel = done + grp * COL_RING;
     if (j == 0) {
-        for (int s = 0; s < COL_RING; s++) mbar_init(&bar[s], 1);
+        for (int s = 0; s < COL_RING; s++) { mbar_init(&bar[s], 1); mbar_init(&rel[s], T); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -129,14 +129,18 @@ col_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, unsigned
                 else if (jp > 0) a = cscale(a, ipw3((2.0 * row + 1.0 - ny) * inv_ny, jp));
                 v[4 * Q + qq] = a;
             }
-            group_sync(bar_id, T); // every thread of the worker has read the slot
-            if (j == 0 && s + COL_RING < nsteps) issue(s + COL_RING);
+            // release the slot: every thread arrives (release semantics: its loads of the slot are done) and the issuing
+            // thread refills it once all have.  (A bar.sync is not enough here: the copy engine is not ordered behind
+            // it -- a refill could overtake a slow warp's reads.)
+            slot_release(&rel[slot]);
+            if (j == 0 && s + COL_RING < nsteps) { mbar_wait(&rel[slot], (unsigned)(s / COL_RING) & 1u); issue(s + COL_RING); }
         }
+        group_sync(bar_id, T); // the previous item's reads of X are done
         col_fft<LOG2N, -1>(v, X, j, bar_id, tw, Nt, w2, w3);
-        cplx *dst = spec + (size_t)k * splane;
+        ST *dst = spec + (size_t)k * splane;
         if (col != 0) {
 #pragma unroll
-            for (int q = 0; q < 16; q++) dst[(size_t)col * N + j + q * T] = v[q];
+            for (int q = 0; q < 16; q++) st_c(&dst[(size_t)col * N + j + q * T], v[q]);
         } else {
             // packed column: separate F = F0 + i FH through the exchange buffer (natural order, mirror read)
             group_sync(bar_id, T);
@@ -147,11 +151,10 @@ col_fwd_kernel(const cplx *__restrict__ inter, cplx *__restrict__ spec, unsigned
             for (int q = 0; q < 16; q++) {
                 const int row = j + q * T;
                 const cplx m = X[swz<4>((N - row) & (N - 1))];
-                dst[row] = mk(0.5 * (v[q].x + m.x), 0.5 * (v[q].y - m.y));
-                dst[(size_t)Hx * N + row] = mk(0.5 * (v[q].y + m.y), -0.5 * (v[q].x - m.x));
+                st_c(&dst[row], mk(0.5 * (v[q].x + m.x), 0.5 * (v[q].y - m.y)));
+                st_c(&dst[(size_t)Hx * N + row], mk(0.5 * (v[q].y + m.y), -0.5 * (v[q].x - m.x)));
             }
         }
-        // (the four ring-step barriers of the next item order these reads of X before its first pass writes X)
     }
 }
 
@@ -178,20 +181,20 @@ __device__ __forceinline__ void khat4(cplx (&kh)[4], const cplx *e, int w, cplx 
 
 // grid / block / smem as the forward kernel.  spec: NK planes of (Hx+1) columns; Ep: taps [NK][L][Hx+1];
 // inter: one plane of Hx columns (rows < ny written).
-template <int LOG2N>
+template <int LOG2N, typename ST>
 __global__ void __launch_bounds__(COL_THREADS, 2)
-col_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, cplx *__restrict__ inter, Geom g,
+col_inv_kernel(const ST *__restrict__ spec, const cplx *__restrict__ Ep, cplx *__restrict__ inter, Geom g,
                const cplx *__restrict__ tw) {
     using C = ColCfg<LOG2N>;
     constexpr int N = C::N, T = C::T, G = C::G, QE = C::QE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ unsigned long long full[G * COL_RING];
+    __shared__ unsigned long long full[G * COL_RING], done[G * COL_RING];
     const int grp = threadIdx.x / T, j = threadIdx.x - grp * T, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * N;
     cplx *ring = reinterpret_cast<cplx *>(smem_raw) + (size_t)G * N + (size_t)grp * COL_RING * QE;
-    unsigned long long *bar = full + grp * COL_RING;
+    unsigned long long *bar = full + grp * COL_RING, *rel = done + grp * COL_RING;
     if (j == 0) {
-        for (int s = 0; s < COL_RING; s++) mbar_init(&bar[s], 1);
+        for (int s = 0; s < COL_RING; s++) { mbar_init(&bar[s], 1); mbar_init(&rel[s], T); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -205,10 +208,10 @@ col_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, cplx 
     auto issue = [&]() {   // one thread: row set pq (rows T pq + 4T q1 + [0,T)) of virtual spectrum pv of column pn
         const int col = wid + pn * nw, nv = col == 0 ? 2 * NK : NK;
         const int t = pv % NK, sc = pv < NK ? col : Hx, slot = ps % COL_RING;
-        const cplx *src = spec + (size_t)t * splane + (size_t)sc * N + T * pq;
-        mbar_expect(&bar[slot], (unsigned)(N * 4));
+        const ST *src = spec + (size_t)t * splane + (size_t)sc * N + T * pq;
+        mbar_expect(&bar[slot], (unsigned)(QE * sizeof(ST)));
 #pragma unroll
-        for (int q1 = 0; q1 < 4; q1++) bulk_g2s(ring + (size_t)slot * QE + q1 * T, src + q1 * QE, (unsigned)(T * 16), &bar[slot]);
+        for (int q1 = 0; q1 < 4; q1++) bulk_g2s(reinterpret_cast<ST *>(ring + (size_t)slot * QE) + q1 * T, src + q1 * QE, (unsigned)(T * sizeof(ST)), &bar[slot]);
         ps++;
         if (++pq == 4) { pq = 0; if (++pv == nv) { pv = 0; pn++; } }
     };
@@ -244,15 +247,16 @@ col_inv_kernel(const cplx *__restrict__ spec, const cplx *__restrict__ Ep, cplx 
                 mbar_wait(&bar[slot], (unsigned)(s / COL_RING) & 1u);
 #pragma unroll
                 for (int q1 = 0; q1 < 4; q1++) {
-                    const cplx z = ring[(size_t)slot * QE + q1 * T + j];
+                    const cplx z = ld_c(reinterpret_cast<const ST *>(ring + (size_t)slot * QE)[q1 * T + j]);
                     cplx &a = acc[q0 + 4 * q1];
                     a.x = fma(z.x, kh[q1].x, fma(-z.y, kh[q1].y, a.x));
                     a.y = fma(z.x, kh[q1].y, fma(z.y, kh[q1].x, a.y));
                 }
-                group_sync(bar_id, T);
-                if (j == 0 && s + COL_RING < nsteps) issue();
+                slot_release(&rel[slot]); // release the slot (see col_fwd_kernel)
+                if (j == 0 && s + COL_RING < nsteps) { mbar_wait(&rel[slot], (unsigned)(s / COL_RING) & 1u); issue(); }
             }
         }
+        group_sync(bar_id, T); // every thread has read its taps from X
         col_fft<LOG2N, 1>(acc, X, j, bar_id, tw, Nt, w2, w3);
         cplx *dst = inter + (size_t)col * N;
 #pragma unroll
@@ -281,8 +285,10 @@ __global__ void __launch_bounds__(128) ktab_plain_kernel(const double *__restric
 
 // ------------------------------------------------------------------------------------------ host side
 template <int LOG2N> static cudaError_t cols_attr() {
-    cudaError_t e = cudaFuncSetAttribute(col_fwd_kernel<LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ColCfg<LOG2N>::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(col_inv_kernel<LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ColCfg<LOG2N>::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(col_fwd_kernel<LOG2N, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ColCfg<LOG2N>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(col_fwd_kernel<LOG2N, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ColCfg<LOG2N>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(col_inv_kernel<LOG2N, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ColCfg<LOG2N>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(col_inv_kernel<LOG2N, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ColCfg<LOG2N>::SMEM);
     return e;
 }
 cudaError_t cols_init() { // per device, at plan creation
@@ -299,12 +305,24 @@ static int col_grid(const sfft_plan *p, int reserve) {
     int grid = 2 * p->sms;
     // while a factorisation runs beside us, leave a few SMs to it: a persistent CTA would otherwise block its chain
     // of small launches for the whole kernel
-    if (reserve > 0 && grid > 8 * reserve) grid -= 2 * reserve;
+    if (reserve > 0 && grid > 2 * reserve) grid -= 2 * reserve;
     const int need = (g.Hx + G - 1) / G;
     return grid < need ? grid : need;
 }
 
-cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj) {
+template <int LOG2N>
+static void run_col_fwd(sfft_plan *p, int grid, const cplx *inter, void *spec, unsigned long long jpack, int ns) {
+    if (p->spec32) col_fwd_kernel<LOG2N, float2><<<grid, COL_THREADS, ColCfg<LOG2N>::SMEM, p->stream>>>(inter, (float2 *)spec, jpack, ns, p->g, p->tw);
+    else col_fwd_kernel<LOG2N, cplx><<<grid, COL_THREADS, ColCfg<LOG2N>::SMEM, p->stream>>>(inter, (cplx *)spec, jpack, ns, p->g, p->tw);
+}
+template <int LOG2N>
+static void run_col_inv(sfft_plan *p, int grid, const void *spec, cplx *inter) {
+    if (p->spec32) col_inv_kernel<LOG2N, float2><<<grid, COL_THREADS, ColCfg<LOG2N>::SMEM, p->stream>>>((const float2 *)spec, p->E, inter, p->g, p->tw);
+    else col_inv_kernel<LOG2N, cplx><<<grid, COL_THREADS, ColCfg<LOG2N>::SMEM, p->stream>>>((const cplx *)spec, p->E, inter, p->g, p->tw);
+}
+
+// spec: ns planes of (Hx+1) x My spectrum elements (cplx, or float2 in the FP32-spectra plan mode)
+cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, void *spec, int ns, const int *ii, const int *jj) {
     const Geom &g = p->g;
     unsigned long long jpack = 0; // job k: (ii << 2) | jj, both <= 3 (DK <= 3)
     if (ns > 16) return cudaErrorInvalidValue;
@@ -315,25 +333,25 @@ cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, 
     KLaunch kl(p, ns > 1 ? "col_fwd_R" : "col_fwd_S");
     const int grid = col_grid(p, p->factor_pending ? p->knob.factor_sms : 0);
     switch (g.log2My) {
-    case 9: col_fwd_kernel<9><<<grid, COL_THREADS, ColCfg<9>::SMEM, p->stream>>>(inter, spec, jpack, ns, g, p->tw); break;
-    case 10: col_fwd_kernel<10><<<grid, COL_THREADS, ColCfg<10>::SMEM, p->stream>>>(inter, spec, jpack, ns, g, p->tw); break;
-    case 11: col_fwd_kernel<11><<<grid, COL_THREADS, ColCfg<11>::SMEM, p->stream>>>(inter, spec, jpack, ns, g, p->tw); break;
-    case 12: col_fwd_kernel<12><<<grid, COL_THREADS, ColCfg<12>::SMEM, p->stream>>>(inter, spec, jpack, ns, g, p->tw); break;
+    case 9: run_col_fwd<9>(p, grid, inter, spec, jpack, ns); break;
+    case 10: run_col_fwd<10>(p, grid, inter, spec, jpack, ns); break;
+    case 11: run_col_fwd<11>(p, grid, inter, spec, jpack, ns); break;
+    case 12: run_col_fwd<12>(p, grid, inter, spec, jpack, ns); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
 }
 
-cudaError_t launch_col_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter) {
+cudaError_t launch_col_inv(sfft_plan *p, const void *spec, const double *coef, cplx *inter) {
     const Geom &g = p->g;
     { KLaunch kl(p, "ktab"); ktab_plain_kernel<<<dim3((g.Hx + 1 + 127) / 128, g.L, g.NK), 128, 0, p->stream>>>(coef, p->E, g, p->tw); }
     KLaunch kl(p, "col_inv");
     const int grid = col_grid(p, 0);
     switch (g.log2My) {
-    case 9: col_inv_kernel<9><<<grid, COL_THREADS, ColCfg<9>::SMEM, p->stream>>>(spec, p->E, inter, g, p->tw); break;
-    case 10: col_inv_kernel<10><<<grid, COL_THREADS, ColCfg<10>::SMEM, p->stream>>>(spec, p->E, inter, g, p->tw); break;
-    case 11: col_inv_kernel<11><<<grid, COL_THREADS, ColCfg<11>::SMEM, p->stream>>>(spec, p->E, inter, g, p->tw); break;
-    case 12: col_inv_kernel<12><<<grid, COL_THREADS, ColCfg<12>::SMEM, p->stream>>>(spec, p->E, inter, g, p->tw); break;
+    case 9: run_col_inv<9>(p, grid, spec, inter); break;
+    case 10: run_col_inv<10>(p, grid, spec, inter); break;
+    case 11: run_col_inv<11>(p, grid, spec, inter); break;
+    case 12: run_col_inv<12>(p, grid, spec, inter); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

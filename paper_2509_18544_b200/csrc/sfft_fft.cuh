@@ -41,6 +41,13 @@ template <int DIR> SFFT_HD cplx mul_w4(cplx a) { return DIR > 0 ? mk(-a.y, a.x) 
 // kx = 0..Hx (the forward column pass separates the packed column once, sfft_cols.cu).
 SFFT_HD size_t plane_idx(int ky, int kx, int My) { return (size_t)kx * My + ky; }
 
+// Storage of spectra: complex128 (cplx) or, in the reduced-memory plan mode (sfft_plan_create_ex, SFFT_PLAN_FP32_SPECTRA),
+// complex64 (float2); arithmetic is FP64 either way.
+SFFT_HD cplx ld_c(const double2 &a) { return a; }
+SFFT_HD cplx ld_c(const float2 &a) { return mk((double)a.x, (double)a.y); }
+SFFT_HD void st_c(double2 *p, cplx v) { *p = v; }
+SFFT_HD void st_c(float2 *p, cplx v) { float2 f; f.x = (float)v.x; f.y = (float)v.y; *p = f; }
+
 template <int LR0> SFFT_HD int swz(int i) { return i ^ ((i >> LR0) & ((1 << LR0) - 1)); }
 
 template <int DIR> SFFT_HD void dft2(cplx &a0, cplx &a1) {
@@ -226,6 +233,16 @@ __device__ __forceinline__ void mbar_expect(unsigned long long *b, unsigned byte
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(unsigned long long *b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+// A consumer thread hands a staging-ring slot back for refilling: the slot was read through the generic proxy and will be
+// WRITTEN by the copy engine (async proxy), and nothing orders the two unless the reader says so -- a refill from L2
+// takes ~150 ns, a shared-memory load queued behind another CTA's exchange phase can take longer.  The proxy fence
+// makes this thread's earlier shared-memory accesses complete before anything the async proxy does after the arrival.
+// (Without it: a handful of wrong spectrum elements per 4088 x 4088 frame, run-to-run different; bar.sync does not
+// order the copy engine either.  tests/test_gpu_fullsize.py::test_run_to_run_reproducibility_at_full_size.)
+__device__ __forceinline__ void slot_release(unsigned long long *b) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity) {

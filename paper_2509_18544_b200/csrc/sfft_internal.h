@@ -76,11 +76,13 @@ struct sfft_plan {
     sfft::cplx *tw;          // [Nt]
     // planes are column-major (sfft_fft.cuh: plane_idx): intermediates [Hx][My] (column 0 packed), spectra [Hx+1][My]
     sfft::cplx *inter;       // [(DK+1)][Hx][My] row-transformed intermediates (a1) / a5 intermediate
-    sfft::cplx *specT;       // [NK][Hx+1][My] spectra of the fit (masked) template images
-    sfft::cplx *specTo;      // [NK][Hx+1][My] spectra of the unmasked template images (allocated with the first mask)
-    sfft::cplx *specS;       // [Hx+1][My]
+    // spectrum elements are complex128, or complex64 in the reduced-memory plan mode (spec32; arithmetic stays FP64)
+    bool spec32; size_t spec_esz; // element size in bytes: 16 or 8
+    void *specT;             // [NK][Hx+1][My] spectra of the fit (masked) template images
+    void *specTo;            // [NK][Hx+1][My] spectra of the unmasked template images (allocated with the first mask)
+    void *specS;             // [Hx+1][My]
     // batched path: up to NSCI science images share one Theta pass; groups of images are pipelined two deep
-    sfft::cplx *specSx[sfft::NSCI]; // [Hx+1][My] each; [0] aliases specS
+    void *specSx[sfft::NSCI]; // [Hx+1][My] each; [0] aliases specS
     double *muSx[sfft::NSCI], *deltax[sfft::NSCI]; // row moments / Delta per image; [0] alias muS, delta
     double *hq[2 * sfft::NSCI], *cq[2 * sfft::NSCI]; // right-hand sides / solutions: group parity x image; [0] alias h, coef
     const double *Sx[sfft::NSCI];   // the science images of the current group
@@ -115,6 +117,8 @@ struct sfft_plan {
     int *flag_host;          // pinned mirror
     // host staging for sfft_difference_host
     double *stS, *stR, *stD; uint8_t *stM;
+    // sfft_difference_host_batch: three-deep upload | compute | download pipeline (allocated on first use)
+    double *hbS[3], *hbD[3], *hbC[3]; cudaStream_t ostream; cudaEvent_t ev_hin[3], ev_hcomp[3], ev_hout[3];
     size_t bytes;
     // state
     const double *S, *R; const uint8_t *mask;
@@ -144,9 +148,9 @@ cudaError_t cols_init();
 cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI,
                            double *mu, int NMOM);
 // columns: FFT_y(yt^jj[k] * inter[ii[k]]) -> spec[k] ([Hx+1][My]), k = 0..ns-1
-cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, cplx *spec, int ns, const int *ii, const int *jj);
+cudaError_t launch_col_fwd(sfft_plan *p, const cplx *inter, void *spec, int ns, const int *ii, const int *jj);
 // inter = IFFT_y(sum_t spec_t K^_t(coef))
-cudaError_t launch_col_inv(sfft_plan *p, const cplx *spec, const double *coef, cplx *inter);
+cudaError_t launch_col_inv(sfft_plan *p, const void *spec, const double *coef, cplx *inter);
 // mode 0: D = S - M - B; mode 1: D = +M
 cudaError_t launch_row_inv(sfft_plan *p, const cplx *inter, const double *S, const double *coef, double *D, int mode);
 
@@ -156,7 +160,7 @@ size_t border_lp_doubles(const Geom &g, int W, int EB);
 size_t border_strip_doubles(const Geom &g, int W);
 cudaError_t launch_border(sfft_plan *p, const PairList &pl, int W, bool science, double *bpart);
 // ---- a2, a3 (sfft_lags.cu, sfft_assemble.cu) ---------------------------------------------------------
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c);
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, size_t esz); // esz: bytes per spectrum element
 cudaError_t lags_init(sfft_plan *p);   // launch shapes, tensor maps, phase tables (plan creation, after the spectra exist)
 void lags_free(sfft_plan *p);
 size_t lag_q_elems(const sfft_plan *p);
@@ -176,7 +180,7 @@ cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream
 // spec: the NK spectra to convolve (default: the plan's unmasked template spectra); mode 0: D = S - M - B,
 // mode 1 (f2, sfft_convolve_stamp): D = +M, S unused
 cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D,
-                            const cplx *spec = nullptr, int mode = 0);
+                            const void *spec = nullptr, int mode = 0);
 
 // ---- f1 (sfft_decorr.cu) -----------------------------------------------------------------
 cudaError_t launch_local_kernel(sfft_plan *p, const double *coef, double xt, double yt, double *K);

@@ -71,14 +71,14 @@ struct LagArgs {
     int phW;             // lag bound of the phase table PH[b/8][d-1][b%8], d = 1..phW
 };
 
-template <int DLO, int DHI>
+template <int DLO, int DHI, typename ST>
 __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int zsplit,
                                             const cplx *__restrict__ PH, cplx *__restrict__ Q, const Geom &g,
-                                            cplx *tile, unsigned long long *full, unsigned long long *done) {
+                                            unsigned char *tile, unsigned long long *full, unsigned long long *done) {
     const int Hx = g.Hx, Tb = g.My / LC_NA, KXC = la.KXC, W = la.W, NK = g.NK;
-    const int col_elems = LC_NA * LC_NB;                       // one (spectrum, kx) of a stage: 2 KB
-    const int stage_elems = la.ns * KXC * col_elems + la.phW * LC_NB;
-    const unsigned stage_bytes = (unsigned)stage_elems * 16u;
+    const int col_elems = LC_NA * LC_NB;                       // one (spectrum, kx) of a stage: 128 elements of ST
+    // a stage: the spectra part in ST elements, then the phase factors (cplx); sized in bytes
+    const unsigned spec_bytes = (unsigned)(la.ns * KXC * col_elems * sizeof(ST)), stage_bytes = spec_bytes + (unsigned)(la.phW * LC_NB * sizeof(cplx));
     const int kx0 = blockIdx.x * KXC;
     const int b0 = zsplit * la.nbs, b1 = min(Tb, b0 + la.nbs);
     const int nIt = max(0, (b1 - b0) / LC_NB);
@@ -98,13 +98,13 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
     }
     __syncthreads();
     auto issue = [&](int it) { // thread 0
-        cplx *st = tile + (size_t)(it % la.nst) * stage_elems;
+        unsigned char *st = tile + (size_t)(it % la.nst) * stage_bytes;
         unsigned long long *bar = &full[it % la.nst];
         const int b = b0 + it * LC_NB;
         mbar_expect(bar, stage_bytes);
         tma_load4(st, &maps.t, 2 * b, 0, kx0, 0, bar);
-        for (int i = 0; i < la.nsci; i++) tma_load3(st + (size_t)(NK + i) * KXC * col_elems, &maps.s[i], 2 * b, 0, kx0, bar);
-        if (la.phW > 0) bulk_g2s(st + (size_t)la.ns * KXC * col_elems, PH + (size_t)(b / LC_NB) * la.phW * LC_NB, (unsigned)(la.phW * LC_NB * 16), bar);
+        for (int i = 0; i < la.nsci; i++) tma_load3(reinterpret_cast<ST *>(st) + (size_t)(NK + i) * KXC * col_elems, &maps.s[i], 2 * b, 0, kx0, bar);
+        if (la.phW > 0) bulk_g2s(st + spec_bytes, PH + (size_t)(b / LC_NB) * la.phW * LC_NB, (unsigned)(la.phW * LC_NB * 16), bar);
     };
     if (threadIdx.x == 0)
         for (int it = 0; it < LC_PRE && it < nIt; it++) issue(it);
@@ -117,15 +117,16 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
         }
         mbar_wait(&full[st_i], (unsigned)(it / la.nst) & 1u);
         if (active) {
-            const cplx *st = tile + (size_t)st_i * stage_elems;
-            const cplx *pa = st + (size_t)(sa * KXC + kxl) * col_elems + bl, *pb = st + (size_t)(sb * KXC + kxl) * col_elems + bl;
+            const unsigned char *st = tile + (size_t)st_i * stage_bytes;
+            const ST *pa = reinterpret_cast<const ST *>(st) + (size_t)(sa * KXC + kxl) * col_elems + bl;
+            const ST *pb = reinterpret_cast<const ST *>(st) + (size_t)(sb * KXC + kxl) * col_elems + bl;
             cplx x[LC_NA];
 #pragma unroll
-            for (int a = 0; a < LC_NA; a++) x[a] = cmulc(pa[a * LC_NB], pb[a * LC_NB]);
+            for (int a = 0; a < LC_NA; a++) x[a] = cmulc(ld_c(pa[a * LC_NB]), ld_c(pb[a * LC_NB]));
             dft16<1>(x);
-            lag_fold<DLO, DHI>(x, st + (size_t)la.ns * KXC * col_elems + bl, acc);
+            lag_fold<DLO, DHI>(x, reinterpret_cast<const cplx *>(st + spec_bytes) + bl, acc);
         }
-        mbar_arrive(&done[st_i]);
+        slot_release(&done[st_i]);
     }
     // sum over the 8 b-lanes, then lane 0 of each (pair, kx) writes its lags
 #pragma unroll
@@ -147,18 +148,18 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
 
 // WB <= 10: one thread folds all 2 WB + 1 lags.  WB = 20: the lag range is split in two halves
 // (blockIdx.z parity) to keep the accumulators in registers; both halves write disjoint rows of Q.
-template <int WB>
+template <int WB, typename ST>
 __global__ void __launch_bounds__(192, 2)
 lagcol_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, const cplx *__restrict__ PH, cplx *__restrict__ Q, Geom g) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long full[4], done[4];
-    cplx *tile = reinterpret_cast<cplx *>(smem_raw);
+    unsigned char *tile = smem_raw;
     if (WB > 10) {
         const int half = blockIdx.z & 1, zs = blockIdx.z >> 1;
-        if (half == 0) lagcol_body<0, WB>(maps, la, pl, zs, PH, Q, g, tile, full, done);
-        else lagcol_body<-WB, -1>(maps, la, pl, zs, PH, Q, g, tile, full, done);
+        if (half == 0) lagcol_body<0, WB, ST>(maps, la, pl, zs, PH, Q, g, tile, full, done);
+        else lagcol_body<-WB, -1, ST>(maps, la, pl, zs, PH, Q, g, tile, full, done);
     } else {
-        lagcol_body<-WB, WB>(maps, la, pl, blockIdx.z, PH, Q, g, tile, full, done);
+        lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.z, PH, Q, g, tile, full, done);
     }
 }
 
@@ -231,14 +232,14 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
 // Launch shape of stage 1, fixed at plan creation (it sizes Q and the TMA boxes): 8 b-lanes per (pair, kx),
 // KXC kx per CTA, pairs in even groups, CTAs of <= 192 threads so that two fit an SM with the accumulators in
 // registers; the ring takes what two CTAs per SM leave of shared memory.
-void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c) {
+void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, size_t esz) {
     const int WB = W <= 3 ? 3 : W <= 5 ? 5 : W <= 6 ? 6 : W <= 10 ? 10 : 20;
     const int Tb = g.My / LC_NA;
     const int KXC = ns <= 7 ? 2 : 1;
     int npg = 192 / (LC_NB * KXC); if (npg > np) npg = np;
     int ngr = (np + npg - 1) / npg; npg = (np + ngr - 1) / ngr;   // even groups (21 pairs: 11 + 10)
     while ((npg * KXC) & 3) npg++;                                 // whole warps (inactive pair slots idle)
-    const size_t stage = ((size_t)ns * KXC * LC_NA * LC_NB + (size_t)WB * LC_NB) * sizeof(cplx); // the kernel folds WB lags (>= W)
+    const size_t stage = (size_t)ns * KXC * LC_NA * LC_NB * esz + (size_t)WB * LC_NB * sizeof(cplx); // the kernel folds WB lags (>= W)
     int nst = 4;
     while (nst > 2 && nst * stage > (size_t)110 * 1024) nst--;
     c->WB = WB; c->KXC = KXC; c->npg = npg; c->ngr = ngr; c->nkb = (g.Hx + 1 + KXC - 1) / KXC;
@@ -254,23 +255,26 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 // tensor map over spectra planes [plane][kx 0..Hx][a 0..15][b 0..Tb-1] (a complex = 2 doubles):
 // box {8 b, 16 a, KXC kx, all planes}; rank 4 for the template set (NK planes, contiguous), rank 3 for one science spectrum
-static cudaError_t make_lag_map(CUtensorMap *tm, const cplx *base, int nplanes, int rank, int KXC, const Geom &g) {
+static cudaError_t make_lag_map(CUtensorMap *tm, const void *base, bool f32, int nplanes, int rank, int KXC, const Geom &g) {
     void *fn = nullptr; cudaDriverEntryPointQueryResult qr;
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
     if (e != cudaSuccess) return e;
     if (!fn || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
     const cuuint64_t Tb = (cuuint64_t)g.My / LC_NA;
     cuuint64_t dims[4] = {2 * Tb, LC_NA, (cuuint64_t)g.Hx + 1, (cuuint64_t)nplanes};
-    cuuint64_t strides[3] = {Tb * 16, (cuuint64_t)g.My * 16, ((cuuint64_t)g.Hx + 1) * g.My * 16};
+    const cuuint64_t eb = f32 ? 8 : 16; // bytes per complex element
+    cuuint64_t strides[3] = {Tb * eb, (cuuint64_t)g.My * eb, ((cuuint64_t)g.Hx + 1) * g.My * eb};
     cuuint32_t box[4] = {2 * LC_NB, LC_NA, (cuuint32_t)KXC, (cuuint32_t)nplanes}, es[4] = {1, 1, 1, 1};
-    CUresult r = ((EncodeTiledFn)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, (void *)base, dims, strides, box, es,
+    CUresult r = ((EncodeTiledFn)fn)(tm, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, (void *)base, dims, strides, box, es,
                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
 template <int WB> static cudaError_t lag_attr() {
-    return cudaFuncSetAttribute(lagcol_kernel<WB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(lagcol_kernel<WB, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(lagcol_kernel<WB, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    return e;
 }
 
 // plan creation (after the spectra are allocated): launch shapes, tensor maps, phase tables, kernel attributes
@@ -278,10 +282,10 @@ cudaError_t lags_init(sfft_plan *p) {
     const Geom &g = p->g;
     p->mapsO = new (std::nothrow) LagMaps(); p->mapsT = new (std::nothrow) LagMaps[NSCI]();
     if (!p->mapsO || !p->mapsT) return cudaErrorMemoryAllocation;
-    cudaError_t e = make_lag_map(&p->mapsO->t, p->specT, g.NK, 4, p->cfgO.KXC, g);
+    cudaError_t e = make_lag_map(&p->mapsO->t, p->specT, p->spec32, g.NK, 4, p->cfgO.KXC, g);
     for (int n = 1; n <= NSCI && e == cudaSuccess; n++) {
-        e = make_lag_map(&p->mapsT[n - 1].t, p->specT, g.NK, 4, p->cfgT[n - 1].KXC, g);
-        for (int i = 0; i < n && e == cudaSuccess; i++) e = make_lag_map(&p->mapsT[n - 1].s[i], p->specSx[i], 1, 3, p->cfgT[n - 1].KXC, g);
+        e = make_lag_map(&p->mapsT[n - 1].t, p->specT, p->spec32, g.NK, 4, p->cfgT[n - 1].KXC, g);
+        for (int i = 0; i < n && e == cudaSuccess; i++) e = make_lag_map(&p->mapsT[n - 1].s[i], p->specSx[i], p->spec32, 1, 3, p->cfgT[n - 1].KXC, g);
     }
     if (e != cudaSuccess) return e;
     const int Tb = g.My / LC_NA;
@@ -311,7 +315,8 @@ static cudaError_t run_lagcol(sfft_plan *p, const LagMaps &maps, int ns, int nsc
     la.ns = ns; la.nsci = nsci; la.npg = c.npg; la.KXC = c.KXC; la.W = W; la.nbs = c.rows_per_split; la.nst = c.nst; la.phW = c.WB;
     dim3 grid(c.nkb, c.ngr, c.nsplit * c.halves);
     KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega");
-    lagcol_kernel<WB><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
+    if (p->spec32) lagcol_kernel<WB, float2><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
+    else lagcol_kernel<WB, cplx><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
     return cudaGetLastError();
 }
 

@@ -34,10 +34,8 @@ template <int LOG2H> struct RowCfg {
     static constexpr int QP = 8 * T;                          // pixels of a quarter row (Mx / 4)
     static constexpr int FSLOT = 2 * QP + 16;                 // forward ring slot in doubles: two quarter rows, the second
                                                               // skewed by 64 B (+ pad to 128 B) against bank conflicts
-    static constexpr int ISLOT = 2 * (Hx / 8) * 2;            // inverse ring slot in cplx: two TMA boxes {2 rows x Hx/8 kx}
     static constexpr size_t XBYTES = (size_t)RP * 2 * Hx * sizeof(cplx);
     static constexpr size_t SMEM_F = XBYTES + (size_t)RP * ROW_RING * FSLOT * sizeof(double);
-    static constexpr size_t SMEM_I = XBYTES + (size_t)RP * ROW_RING * ISLOT * sizeof(cplx);
 };
 
 __device__ __forceinline__ double ipow_small(double b, int e) {
@@ -91,16 +89,16 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
     using C = RowCfg<LOG2H>;
     constexpr int Hx = C::Hx, T = C::T, GT = C::GT, TP = 2 * T, QP = C::QP; // TP = Hx/8: butterflies of the last pass
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ unsigned long long full[C::RP * ROW_RING];
+    __shared__ unsigned long long full[C::RP * ROW_RING], done[C::RP * ROW_RING];
     const int grp = threadIdx.x / GT, t = threadIdx.x - grp * GT, r = t & 1, j = t >> 1, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * 2 * Hx;
     // warp partials of the row moments [warp of the worker][row][m]: they live in the exchange buffer, which is idle
     // during the load phase (two CTAs per SM leave no room for another static array)
     double (*wpart)[2][8] = reinterpret_cast<double (*)[2][8]>(X);
     double *ring = reinterpret_cast<double *>(smem_raw + C::XBYTES) + (size_t)grp * ROW_RING * C::FSLOT;
-    unsigned long long *bar = full + grp * ROW_RING;
+    unsigned long long *bar = full + grp * ROW_RING, *rel = done + grp * ROW_RING;
     if (BULK && t == 0) {
-        for (int k = 0; k < ROW_RING; k++) mbar_init(&bar[k], 1);
+        for (int k = 0; k < ROW_RING; k++) { mbar_init(&bar[k], 1); mbar_init(&rel[k], GT); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -174,14 +172,17 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
                     v[q] = mk(a * fma(xa, fma(xa, fma(xa, c3, c2), c1), c0), b * fma(xb, fma(xb, fma(xb, c3, c2), c1), c0));
                 }
                 if (BULK) {
-                    group_sync(bar_id, GT); // every thread of the worker has read the slot
-                    if (t == 0 && s + ROW_RING < nsteps) issue(s + ROW_RING);
+                    // release the slot: every thread arrives (release semantics: its loads of the slot are done) and the
+                    // issuing thread refills it once all have.  (A bar.sync is not enough here: the copy engine is not
+                    // ordered behind it -- a refill could overtake a slow warp's reads.)
+                    slot_release(&rel[slot]);
+                    if (t == 0 && s + ROW_RING < nsteps) { mbar_wait(&rel[slot], (unsigned)(s / ROW_RING) & 1u); issue(s + ROW_RING); }
                     s++;
                 }
             }
             if (NM > 0) {
                 // deterministic reduction over the T threads of each row: lanes of equal parity inside a warp, then warps
-                if (!BULK) group_sync(bar_id, GT); // (no ring barriers on this path: the previous item's reads of X must be done)
+                group_sync(bar_id, GT); // the previous item's last-pass reads of X are done (wpart lives in X)
                 const int lane = threadIdx.x & 31, wrp = t >> 5;
 #pragma unroll
                 for (int m = 0; m < NM; m++) {
@@ -258,56 +259,44 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
 }
 
 // ------------------------------------------------------------------------------------------ inverse
-__device__ __forceinline__ void tma_load2(void *dst, const CUtensorMap *tm, int c0, int c1, unsigned long long *bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ void l2_prefetch(const void *gsrc, unsigned bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
 }
 
+__device__ __forceinline__ void tma_prefetch2(const CUtensorMap *tm, int c0, int c1) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(tm), "r"(c0), "r"(c1) : "memory");
+}
+
 // inter (Hx columns x My, column-major; tensor map tmI: boxes {2 rows, Hx/8 kx} = the 32-byte sectors of one row
 // pair) -> D = S - M - B (mode 0) or D = +M (mode 1: plain convolution, f2).
-// grid: persistent, <= 2 CTAs per SM; block 256 = RP workers of 2 T threads; dynamic smem RowCfg::SMEM_I
+// A thread needs exactly 16 elements of the intermediate (its two butterflies) and nobody else needs them, so they
+// go straight to registers: 16 independent 16-byte loads, lane pairs covering whole 32-byte sectors.  What hides
+// their latency is a TMA PREFETCH: while a pair is transformed, one thread asks the copy engine to bring the next
+// pair's boxes (and its two science rows) into L2 -- no shared-memory ring, no barriers, nothing to release.
+// grid: persistent, <= 2 CTAs per SM; block 256 = RP workers of 2 T threads; dynamic smem RowCfg::XBYTES
 template <int LOG2H>
 __global__ void __launch_bounds__(ROW_THREADS, 2)
-row_inv_kernel(const __grid_constant__ CUtensorMap tmI, const double *__restrict__ S, const double *__restrict__ coef,
-               double *__restrict__ D, Geom g, const cplx *__restrict__ tw, int mode) {
+row_inv_kernel(const __grid_constant__ CUtensorMap tmI, const cplx *__restrict__ inter, const double *__restrict__ S,
+               const double *__restrict__ coef, double *__restrict__ D, Geom g, const cplx *__restrict__ tw, int mode) {
     using C = RowCfg<LOG2H>;
     constexpr int Hx = C::Hx, T = C::T, GT = C::GT, TP = 2 * T;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ unsigned long long full[C::RP * ROW_RING];
     const int grp = threadIdx.x / GT, t = threadIdx.x - grp * GT, r = t & 1, j = t >> 1, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * 2 * Hx;
-    cplx *ring = reinterpret_cast<cplx *>(smem_raw + C::XBYTES) + (size_t)grp * ROW_RING * C::ISLOT;
-    unsigned long long *bar = full + grp * ROW_RING;
-    if (t == 0) {
-        for (int k = 0; k < ROW_RING; k++) mbar_init(&bar[k], 1);
-        mbar_fence_init();
-    }
-    __syncthreads();
     const int nx = g.nx, ny = g.ny, My = g.My, Nt = g.Nt, npairs = (ny + 1) >> 1;
     const int wid = blockIdx.x * C::RP + grp, nw = gridDim.x * C::RP;
     const int nmine = wid < npairs ? (npairs - wid + nw - 1) / nw : 0;
-    const int nsteps = nmine * 4;
     const int A = j, B = j == 0 ? T : TP - j;
     const bool vec = ((nx & 1) == 0) && (((size_t)S | (size_t)D) & 15) == 0;
-    auto issue = [&](int s) { // one thread: boxes m = 2Q, 2Q+1 of row pair n into slot s % RING
-        const int n = s >> 2, Q = s & 3, slot = s % ROW_RING;
+    auto prefetch = [&](int n) { // one thread: the boxes and the science rows of row pair n towards L2
         const int y0 = 2 * (wid + n * nw);
-        mbar_expect(&bar[slot], (unsigned)(C::ISLOT * sizeof(cplx)));
-        tma_load2(ring + (size_t)slot * C::ISLOT, &tmI, 2 * y0, (2 * Q) * TP, &bar[slot]);
-        tma_load2(ring + (size_t)slot * C::ISLOT + 2 * TP, &tmI, 2 * y0, (2 * Q + 1) * TP, &bar[slot]);
-        if (Q == 0 && mode == 0 && vec) { // the science rows of this pair are wanted at the end of the item: start them towards L2 now
-            const int rows = y0 + 1 < ny ? 2 : 1;
-            l2_prefetch(S + (size_t)y0 * nx, (unsigned)(rows * nx * 8));
-        }
+#pragma unroll
+        for (int m = 0; m < 8; m++) tma_prefetch2(&tmI, 2 * y0, m * TP);
+        if (mode == 0 && vec) l2_prefetch(S + (size_t)y0 * nx, (unsigned)((y0 + 1 < ny ? 2 : 1) * nx * 8));
     };
-    if (t == 0)
-        for (int s = 0; s < ROW_RING && s < nsteps; s++) issue(s);
+    if (t == 0 && nmine > 0) prefetch(0);
     const cplx uA = tw[(size_t)(j == 0 ? T : A) * (Nt >> (LOG2H + 1))]; // exp(-2 pi i k/Mx), k = A (thread 0: T)
     const cplx wL = tw[(size_t)j * (Nt >> LOG2H)];                      // last pass: radix 16, Ns = T, one butterfly per thread
-    int s = 0;
     const int j_outer_ = j; // (see the note at opaque_index)
     for (int n = 0; n < nmine; n++) {
         const int j = opaque_index(j_outer_);
@@ -316,19 +305,13 @@ row_inv_kernel(const __grid_constant__ CUtensorMap tmI, const double *__restrict
         cplx zA[8], zB[8];
         {
             cplx xA[8], xB[8];
+            const cplx *src = inter + y;
 #pragma unroll
-            for (int Q = 0; Q < 4; Q++, s++) {
-                const int slot = s % ROW_RING;
-                mbar_wait(&bar[slot], (unsigned)(s / ROW_RING) & 1u);
-                const cplx *sl = ring + (size_t)slot * C::ISLOT;
-#pragma unroll
-                for (int bx = 0; bx < 2; bx++) {
-                    xA[2 * Q + bx] = live ? sl[(size_t)(bx * TP + A) * 2 + r] : mk(0.0, 0.0);
-                    xB[2 * Q + bx] = live ? sl[(size_t)(bx * TP + B) * 2 + r] : mk(0.0, 0.0);
-                }
-                group_sync(bar_id, GT); // every thread of the worker has read the slot
-                if (t == 0 && s + ROW_RING < nsteps) issue(s + ROW_RING);
+            for (int m = 0; m < 8; m++) {
+                xA[m] = live ? src[(size_t)(A + m * TP) * My] : mk(0.0, 0.0);
+                xB[m] = live ? src[(size_t)(B + m * TP) * My] : mk(0.0, 0.0);
             }
+            if (t == 0 && n + 1 < nmine) prefetch(n + 1);
             if (j != 0) {
 #pragma unroll
                 for (int m = 0; m < 8; m++) tangle(xA[m], xB[7 - m], cmul(uA, w16(m)), zA[m], zB[7 - m]);
@@ -345,9 +328,10 @@ row_inv_kernel(const __grid_constant__ CUtensorMap tmI, const double *__restrict
                 for (int m = 0; m < 4; m++) tangle(xB[m], xB[7 - m], cmul(uA, w16(m)), zB[m], zB[7 - m]);
             }
         }
-        // pass 1: radix 8, no twiddles, butterflies A and B (the four ring barriers above order the previous pair's reads of X)
+        // pass 1: radix 8, no twiddles, butterflies A and B
         dft8<1>(zA);
         dft8<1>(zB);
+        group_sync(bar_id, GT); // the previous pair's last reads of X are done
 #pragma unroll
         for (int m = 0; m < 8; m++) {
             X[(size_t)out_pos<8, 3>(A, m, 0) * 2 + r] = zA[m];
@@ -420,7 +404,7 @@ template <int LOG2H> static cudaError_t rows_attr() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(row_fwd_kernel<LOG2H, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_F);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<LOG2H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::SMEM_I);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(row_inv_kernel<LOG2H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RowCfg<LOG2H>::XBYTES);
     return e;
 }
 
@@ -452,7 +436,11 @@ cudaError_t rows_init(sfft_plan *p) {
 void rows_free(sfft_plan *p) { delete p->mapI; p->mapI = nullptr; }
 
 template <int LOG2H> static int row_grid(const sfft_plan *p) {
-    const int need = ((p->g.ny + 1) / 2 + RowCfg<LOG2H>::RP - 1) / RowCfg<LOG2H>::RP, cap = 2 * p->sms;
+    const int need = ((p->g.ny + 1) / 2 + RowCfg<LOG2H>::RP - 1) / RowCfg<LOG2H>::RP;
+    int cap = 2 * p->sms;
+    // while a factorisation runs beside us, leave a few SMs to it: persistent CTAs would otherwise block its chain of
+    // small launches for the whole kernel
+    if (p->factor_pending && cap > 2 * p->knob.factor_sms) cap -= 2 * p->knob.factor_sms;
     return need < cap ? need : cap;
 }
 
@@ -485,9 +473,9 @@ cudaError_t launch_row_inv(sfft_plan *p, const cplx *inter, const double *S, con
     if (inter != p->inter) return cudaErrorInvalidValue;
     KLaunch kl(p, "row_inv");
     switch (g.log2Hx) {
-    case 9: row_inv_kernel<9><<<row_grid<9>(p), ROW_THREADS, RowCfg<9>::SMEM_I, p->stream>>>(*p->mapI, S, coef, D, g, p->tw, mode); break;
-    case 10: row_inv_kernel<10><<<row_grid<10>(p), ROW_THREADS, RowCfg<10>::SMEM_I, p->stream>>>(*p->mapI, S, coef, D, g, p->tw, mode); break;
-    case 11: row_inv_kernel<11><<<row_grid<11>(p), ROW_THREADS, RowCfg<11>::SMEM_I, p->stream>>>(*p->mapI, S, coef, D, g, p->tw, mode); break;
+    case 9: row_inv_kernel<9><<<row_grid<9>(p), ROW_THREADS, RowCfg<9>::XBYTES, p->stream>>>(*p->mapI, inter, S, coef, D, g, p->tw, mode); break;
+    case 10: row_inv_kernel<10><<<row_grid<10>(p), ROW_THREADS, RowCfg<10>::XBYTES, p->stream>>>(*p->mapI, inter, S, coef, D, g, p->tw, mode); break;
+    case 11: row_inv_kernel<11><<<row_grid<11>(p), ROW_THREADS, RowCfg<11>::XBYTES, p->stream>>>(*p->mapI, inter, S, coef, D, g, p->tw, mode); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -156,7 +156,7 @@ __device__ __forceinline__ void tile_abt(const double (*As)[CLD], const double (
 // with DMMA and subtracts them from the tiles it has just loaded.  The trailing-update kernel then only covers
 // block columns >= k0 + 64 and runs beside this kernel (launch_factor).
 // dynamic smem: 2 * 64 * CLD doubles (X_b, X_d).
-__global__ void __launch_bounds__(256) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
+__global__ void __launch_bounds__(256, 2) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
                                                          int bs, int *flag) {
     extern __shared__ __align__(16) double psm[];
     __shared__ double l[CPAD][CB + 1];

@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
 }
 
 cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D,
-                            const cplx *spec, int mode) {
+                            const void *spec, int mode) {
     const Geom &g = p->g;
     if (!spec) spec = p->mask ? p->specTo : p->specT; // a mask keeps a second, unmasked set (C7); without one the fit spectra are it
     cudaError_t e = launch_col_inv(p, spec, coef, p->inter);

@@ -21,10 +21,10 @@ _STATUS = {0: "OK", -1: "INVALID_ARG", -2: "ALLOC", -3: "CUDA", -4: "STATE", -5:
 
 # every symbol include/sfft.h declares (tests check the library exports all of them)
 SYMBOLS = (
-    "sfft_plan_create", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
+    "sfft_plan_create", "sfft_plan_create_ex", "sfft_plan_set_stream", "sfft_plan_destroy", "sfft_num_unknowns",
     "sfft_workspace_bytes", "sfft_build_system", "sfft_solve", "sfft_solve_constant_ratio", "sfft_set_constant_ratio", "sfft_subtract", "sfft_subtract_with",
     "sfft_set_template", "sfft_subtract_batch", "sfft_convolve_stamp", "sfft_resample_affine", "sfft_resample_affine_mask", "sfft_local_kernel",
-    "sfft_decorrelation_stamp", "sfft_difference_host", "sfft_sync_status",
+    "sfft_decorrelation_stamp", "sfft_difference_host", "sfft_difference_host_batch", "sfft_sync_status",
     "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
     "sfft_kernel_timing_get", "sfft_launch_count",
     "sfft_last_error", "sfft_version", "sfft_debug_read", "sfft_probe_fp64",
@@ -51,6 +51,7 @@ def load_library():
     lib = ctypes.CDLL(str(LIB_PATH))
     vp, ci, dp = ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p
     lib.sfft_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci]
+    lib.sfft_plan_create_ex.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ctypes.c_uint]
     lib.sfft_plan_set_stream.argtypes = [vp, vp]
     lib.sfft_plan_destroy.argtypes = [vp]
     lib.sfft_num_unknowns.argtypes = [vp]
@@ -71,6 +72,7 @@ def load_library():
     lib.sfft_set_template.argtypes = [vp, dp, dp]
     lib.sfft_subtract_batch.argtypes = [vp, ctypes.POINTER(vp), ci, ctypes.POINTER(vp), dp]
     lib.sfft_difference_host.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.sfft_difference_host_batch.argtypes = [vp, dp, dp, ctypes.POINTER(vp), ci, ctypes.POINTER(vp), dp]
     lib.sfft_sync_status.argtypes = [vp]
     lib.sfft_get_system.argtypes = [vp, dp, dp]
     lib.sfft_enable_timings.argtypes = [vp, ci]
@@ -122,15 +124,18 @@ def _dev_mask(m, shape):
 class SfftPlan:
     """sfft_plan_create(nx, ny, L, DK, DB) and the calls on it; same names as the C ABI."""
 
-    def __init__(self, nx, ny, L, DK, DB, stream=None):
+    FP32_SPECTRA = 1   # SFFT_PLAN_FP32_SPECTRA: the reduced-memory mode (spectra stored as complex64)
+
+    def __init__(self, nx, ny, L, DK, DB, stream=None, flags=0):
         if not torch.cuda.is_available():
             raise RuntimeError("libsfft needs a CUDA device (sm_100a); there is no CPU fallback")
         self._lib = load_library()
         self._h = ctypes.c_void_p()
-        rc = self._lib.sfft_plan_create(ctypes.byref(self._h), nx, ny, L, DK, DB)
+        rc = self._lib.sfft_plan_create_ex(ctypes.byref(self._h), nx, ny, L, DK, DB, int(flags))
         if rc:
             self._h = None
-            raise SfftError(rc, "sfft_plan_create")
+            raise SfftError(rc, "sfft_plan_create_ex" if flags else "sfft_plan_create")
+        self.flags = int(flags)
         self.nx, self.ny, self.L, self.DK, self.DB = nx, ny, L, DK, DB
         self.shape = (ny, nx)
         self.n = self._lib.sfft_num_unknowns(self._h)
@@ -286,6 +291,23 @@ class SfftPlan:
                                                 D_host.data_ptr(), coeffs_host.data_ptr()), "sfft_difference_host")
         return D_host, coeffs_host
 
+    def difference_host_batch(self, R_host, S_hosts, mask_host=None, D_hosts=None, coeffs_host=None):
+        """One template, B science images, all CPU float64 tensors (pinned for the copies to overlap).  Synchronises."""
+        B = len(S_hosts)
+        for t, nm in [(R_host, "R_host")] + [(s, "S_hosts[b]") for s in S_hosts]:
+            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != self.shape:
+                raise TypeError(f"{nm}: need a contiguous CPU float64 tensor of shape {self.shape}")
+        if D_hosts is None:
+            D_hosts = [torch.empty(self.shape, dtype=torch.float64).pin_memory() for _ in range(B)]
+        if coeffs_host is None:
+            coeffs_host = torch.empty((B, self.n), dtype=torch.float64)
+        Sp = (ctypes.c_void_p * B)(*[s.data_ptr() for s in S_hosts])
+        Dp = (ctypes.c_void_p * B)(*[d.data_ptr() for d in D_hosts])
+        mp = mask_host.data_ptr() if mask_host is not None else None
+        self._ck(self._lib.sfft_difference_host_batch(self._h, R_host.data_ptr(), mp, Sp, B, Dp, coeffs_host.data_ptr()),
+                 "sfft_difference_host_batch")
+        return D_hosts, coeffs_host
+
     # -- introspection ---------------------------------------------------------------------
     def sync_status(self):
         self._ck(self._lib.sfft_sync_status(self._h), "sfft_sync_status")
@@ -326,7 +348,8 @@ class SfftPlan:
         NK, NB = (self.DK + 1) * (self.DK + 2) // 2, (self.DB + 1) * (self.DB + 2) // 2
         shapes = {0: ((My, Mx // 2 + 1), np.complex128), 1: ((My, Mx // 2 + 1), np.complex128),
                   2: ((4 * w + 1, 4 * w + 1), np.float64), 3: ((L, L), np.float64),
-                  4: ((NK, NB, L, L), np.float64), 5: ((NB, NB), np.float64), 6: ((NB,), np.float64)}
+                  4: ((NK, NB, L, L), np.float64), 5: ((NB, NB), np.float64), 6: ((NB,), np.float64),
+                  8: ((Mx // 2, My), np.complex128)}
         shp, dt = shapes[which]
         out = np.zeros(shp, dtype=dt)
         self._ck(self._lib.sfft_debug_read(self._h, which, idx, out.ctypes.data_as(ctypes.c_void_p), out.nbytes),

@@ -300,6 +300,31 @@ def test_difference_host_matches_device_path():
     assert np.array_equal(Dh.numpy(), D) and np.array_equal(ch.numpy(), cd)
 
 
+def test_difference_host_batch_matches_device_batch():
+    """The PCIe-pipelined host call (three staging slots, two copy streams): B = 7 images (two full turns of the slots and
+    a ragged one) must reproduce the device-resident batched call bit for bit, with and without a mask."""
+    nx, ny, L, DK, DB, B = 100, 72, 5, 1, 1, 7
+    _, R = starfield.random_pair(nx, ny, seed=300)
+    Ss = [starfield.random_pair(nx, ny, seed=301 + b)[0] for b in range(B)]
+    rng = np.random.default_rng(4)
+    for mask in (None, (rng.random((ny, nx)) > 0.05).astype(np.uint8)):
+        p = SfftPlan(nx, ny, L, DK, DB)
+        p.set_template(dev(R), dev(mask) if mask is not None else None)
+        Ds, cs = p.subtract_batch([dev(s) for s in Ss])
+        p.sync_status()
+        hm = torch.from_numpy(mask).pin_memory() if mask is not None else None
+        Dh, ch = p.difference_host_batch(torch.from_numpy(R).pin_memory(), [torch.from_numpy(s).pin_memory() for s in Ss], hm)
+        for b in range(B):
+            # (the device call runs the images in groups of four through one Theta pass, the host call one by one: the
+            #  same sums in another split order -- rounding level, as in test_batched_groups_of_images_masked)
+            assert np.max(np.abs(ch[b].numpy() - cs[b].cpu().numpy())) <= 1e-10 * np.max(np.abs(ch[b].numpy())), b
+            assert np.max(np.abs(Dh[b].numpy() - Ds[b].cpu().numpy())) <= 1e-8 * 20.0, b
+        Dh2, ch2 = p.difference_host_batch(torch.from_numpy(R).pin_memory(), [torch.from_numpy(s).pin_memory() for s in Ss], hm)
+        for b in range(B):
+            assert torch.equal(Dh[b], Dh2[b]) and torch.equal(ch[b], ch2[b])
+        p.destroy()
+
+
 # ---------------------------------------------------------------- f2: cross-convolution with a PSF stamp (PAPER.md:86)
 # Bar: |out_gpu - out_oracle| <= 1e-11 * max|img| * sum|stamp| everywhere.  The FFT route's rounding error is
 # ~ log2(Mx My) * 2^-53 * max|img| * sum|stamp| ~ 3e-15 of that product (DESIGN.md section 11), so the bar has three
