@@ -332,6 +332,7 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
     peak, peak_src = measured_peaks()
     kbytes, path_bytes = algorithmic_bytes(nx, ny, DK, NK)
     K = max(3, min(args.steps, 10))
+    ws_fp64 = plan.workspace_bytes          # before the host-batch call adds its staging buffers
 
     # per stage
     stages = {}
@@ -639,6 +640,75 @@ def detail_rank0(plan, step, args, cfg, NK, dS, dR, pair, torch):
         except Exception as ex:  # pragma: no cover
             out["batched"]["constant_ratio_mode"] = {"error": str(ex)}
         plan.set_constant_ratio(False)
+
+        # the same batch from HOST memory (sfft_difference_host_batch): template up once, three-deep upload | compute |
+        # download pipeline; 4 pinned science buffers and 4 pinned outputs cycled
+        try:
+            hR = torch.from_numpy(pair["R"]).pin_memory()
+            hS = [t_.cpu().pin_memory() for t_ in Ss]
+            hD = [torch.empty((ny, nx), dtype=torch.float64).pin_memory() for _ in range(len(Ss))]
+            hc = torch.empty((B, cfg["n"]), dtype=torch.float64).pin_memory()
+            S_h = [hS[b % len(hS)] for b in range(B)]; D_h = [hD[b % len(hD)] for b in range(B)]
+            plan.difference_host_batch(hR, S_h, None, D_h, hc)
+            th = []
+            for _ in range(3):
+                t0 = time.perf_counter()
+                plan.difference_host_batch(hR, S_h, None, D_h, hc)
+                th.append((time.perf_counter() - t0) * 1e3)
+            ms_h = float(np.median(th))
+            out["batched"]["e2e"] = {"what": "sfft_difference_host_batch: R up once, per image 134 MB up and 134 MB down over PCIe inside the timed region (host clock, the call synchronises)",
+                                     "ms_per_image": round(ms_h / B, 4), "images_per_s": round(B * 1e3 / ms_h, 1),
+                                     "h2d_bytes_per_image": int(nx * ny * 8), "d2h_bytes_per_image": int(nx * ny * 8 + cfg["n"] * 8),
+                                     "pcie_gbs_each_way": round(nx * ny * 8 / (ms_h / B) / 1e6, 1)}
+            del hS, hD
+        except Exception as ex:  # pragma: no cover
+            out["batched"]["e2e"] = {"error": str(ex)}
+
+    # f4, reduced-memory mode (SFFT_PLAN_FP32_SPECTRA): spectra stored as complex64 -- workspace and speed beside the FP64 plan
+    try:
+        from paper_2509_18544_b200 import SfftPlan as _Plan
+        p32 = _Plan(nx, ny, cfg["L"], cfg["DK"], cfg["DB"], flags=_Plan.FP32_SPECTRA)
+        o32 = torch.empty_like(dS)
+
+        def step32():
+            p32.build_system(dS, dR); p32.solve(); p32.subtract(o32)
+        for _ in range(3):
+            step32()
+        p32.sync_status()
+        stream = torch.cuda.current_stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            step32()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms32 = e0.elapsed_time(e1) / K
+        p32.enable_timings(2); step32()
+        k32 = {}
+        for name, ms in p32.kernel_timings():
+            k32[name] = k32.get(name, 0.0) + ms
+        p32.enable_timings(0)
+        rm = {"workload": "the headline step on a plan created with SFFT_PLAN_FP32_SPECTRA (complex64 spectra, FP64 arithmetic)",
+              "ms_per_step": round(ms32, 4), "images_per_s": round(1e3 / ms32, 1), "workspace_gb": round(p32.workspace_bytes / 1e9, 3),
+              "fp64_plan_workspace_gb": round(ws_fp64 / 1e9, 3),
+              "kernels_ms": {k_: round(v_, 4) for k_, v_ in sorted(k32.items(), key=lambda kv: -kv[1])[:8]},
+              "tolerances": "G, h 2e-7; kernel coefficients 1e-4; background 5e-3; D 3e-3 sigma (tests/test_gpu_fp32_spectra.py; measured 8e-8, 5e-8, 1e-5, 6e-4, 5e-4)"}
+        if B > 0:
+            cb32 = torch.empty((B, cfg["n"]), dtype=torch.float64, device="cuda")
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            tt = []
+            for _ in range(4):
+                ev[0].record(stream); p32.set_template(dR); ev[1].record(stream); p32.subtract_batch(S_list, D_arg, cb32); ev[2].record(stream)
+                torch.cuda.synchronize()
+                tt.append((ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])))
+            tt = tt[1:]
+            a_, b_ = float(np.median([x for x, _ in tt])), float(np.median([y for _, y in tt]))
+            rm["batched"] = {"B": B, "template_ms": round(a_, 3), "per_image_ms": round(b_ / B, 4), "images_per_s": round(B * 1e3 / (a_ + b_), 1)}
+        out["reduced_memory"] = rm
+        p32.destroy()
+        del o32
+    except Exception as ex:  # pragma: no cover
+        out["reduced_memory"] = {"error": str(ex)}
 
     # a4 on its own (BASELINE.json north_star: "FP64 tensor-pipe utilisation for the solve"): the factorisation of the
     # n = 732 system as sfft_set_template runs it (alone on the machine, stage timer), n^3/3 flop against the probed DMMA rate
