@@ -173,9 +173,12 @@ sfft_status sfft_subtract_batch(sfft_plan *plan, const double *const *S, int B,
  * doubles, same tap layout as the kernel coefficients; L, w = (L-1)/2 are the plan's), circular at the
  * native nx x ny like the subtraction (reading C6).  out: device, ny*nx doubles, must not alias img.
  * Runs the a1 transforms of img, the a5 K^ synthesis / inverse transforms and the border wrap
- * correction; uses the plan's science-spectrum and intermediate buffers as scratch: call it BEFORE
- * sfft_build_system / sfft_set_template or after sfft_subtract, not between them (no state check is
- * made).  The plan's DK, DB are irrelevant.  Asynchronous on the plan's stream.
+ * correction; uses the plan's science-spectrum and intermediate buffers as scratch.  Both are dead between the
+ * plan's calls (the intermediates live inside sfft_build_system / sfft_subtract, the science spectrum is consumed by
+ * sfft_build_system and rebuilt per image by sfft_subtract_batch), and everything is ordered on the plan's stream, so
+ * the call is allowed ANYWHERE in the call sequence, also between sfft_build_system and sfft_subtract
+ * (tests/test_gpu_parity.py::test_scratch_users_between_build_and_subtract).  The plan's DK, DB are irrelevant.
+ * Asynchronous on the plan's stream.
  * Errors: INVALID_ARG (NULL or aliased pointers), CUDA. */
 sfft_status sfft_convolve_stamp(sfft_plan *plan, const double *img, const double *stamp, double *out);
 
@@ -219,8 +222,8 @@ sfft_status sfft_local_kernel(sfft_plan *plan, const double *coeffs, double x, d
  * K: device, Lk*Lk doubles (e.g. from sfft_local_kernel); psf_S, psf_R: device, Lp*Lp doubles each; all stamps in
  * the tap layout stamp[(v + w) * P + (u + w)], P odd.  stamp_out: device, L*L doubles.
  * N: any integer with max(Lk + Lp - 1, L) <= N <= 1024 (no power-of-two restriction: the transforms are pruned direct
- * sums over the stamp taps); (N*N + 1) doubles of the plan's intermediate buffer serve as scratch, so the call-order
- * rule of sfft_convolve_stamp applies (not between sfft_build_system and sfft_subtract).
+ * sums over the stamp taps); (N*N + 1) doubles of the plan's intermediate buffer serve as scratch (dead between the
+ * plan's calls: allowed anywhere in the call sequence, like sfft_convolve_stamp).
  * SYNCHRONISES the plan's stream (a per-frame set-up call) and returns INVALID_ARG if F is zero, negative or not finite
  * at any grid frequency (the kernel is undefined there; stamp_out is then unspecified).
  * Errors: INVALID_ARG (NULL pointers, even or non-positive stamp sizes, N out of range or larger than the scratch,

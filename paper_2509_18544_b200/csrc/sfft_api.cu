@@ -74,7 +74,7 @@ static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
                     p->Q, p->phO, p->phT, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
-                    p->ywork, p->zwork, p->coef, p->ratioEZ, p->ratioW, p->E, p->flag, p->stS, p->stR, p->stD, p->stM};
+                    p->ywork, p->zwork, p->coef, p->ratioEZ, p->ratioW, p->E, p->wcorr, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
@@ -206,6 +206,7 @@ sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, 
     AL(p->coef, n);
     for (int i = 1; i < 2 * NSCI; i++) { AL(p->hq[i], n); AL(p->cq[i], n); }
     AL(p->E, (size_t)g.NK * L * (g.Hx + 1));
+    AL(p->wcorr, (size_t)(2LL * g.w * nx + 2LL * g.w * (ny - 2 * g.w)) + 1);
     AL(p->flag, 2);   // [0] pivot test failed (factorisation), [1] triangular-solve error
 #undef AL
     p->specTo = p->specT;

@@ -113,6 +113,7 @@ struct sfft_plan {
     double *coef;            // [n]   solved coefficients
     double *ratioEZ;         // [2][NK-1][n] indicator right-hand sides and their solves (sfft_solve_constant_ratio; allocated on first use)
     sfft::cplx *E;           // [NK][L][Hx+1] kernel row tables for a5
+    double *wcorr;           // [border pixels] native-grid wrap corrections of a5 (sfft_subtract.cu)
     int *flag;               // device: 1 = pivot test failed
     int *flag_host;          // pinned mirror
     // host staging for sfft_difference_host

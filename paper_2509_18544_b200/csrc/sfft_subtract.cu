@@ -15,8 +15,10 @@ namespace sfft {
 // One thread per border pixel (within w of an edge).  For every tap (u,v) whose source pixel
 // (x-u, y-v) leaves the frame, the padded-grid FFT used Rpad((x-u) mod Mx, (y-v) mod My) (zero in
 // the padding) where the method wants R((x-u) mod nx, (y-v) mod ny): subtract the difference.
-__global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__ R, const double *__restrict__ coef,
-                                                     double *__restrict__ D, Geom g, int mode) {
+// Two kernels: wrapcorr computes the corrections (they depend on R and the coefficients only, so it runs on a side stream
+// BESIDE the inverse transforms) into corr[border pixel id]; wrapapply subtracts them from D afterwards.
+__global__ void __launch_bounds__(128) wrapcorr_kernel(const double *__restrict__ R, const double *__restrict__ coef,
+                                                      double *__restrict__ cbuf, Geom g) {
     const int nx = g.nx, ny = g.ny, w = g.w, L = g.L, LL = L * L;
     const long long nA = 2LL * w * nx, nB = 2LL * w * (ny - 2 * w);
     // 4 adjacent lanes share a pixel (tap rows v = -w + part, step 4): the per-thread chain of dependent R loads is 4x shorter
@@ -62,20 +64,40 @@ __global__ void __launch_bounds__(128) wrapfix_kernel(const double *__restrict__
     }
     corr += __shfl_xor_sync(0xffffffffu, corr, 1);
     corr += __shfl_xor_sync(0xffffffffu, corr, 2);
-    if (live && part == 0) D[(size_t)y * nx + x] -= mode ? -corr : corr;
+    if (live && part == 0) cbuf[id] = corr;
+}
+
+__global__ void __launch_bounds__(256) wrapapply_kernel(const double *__restrict__ cbuf, double *__restrict__ D, Geom g, int mode) {
+    const int nx = g.nx, ny = g.ny, w = g.w;
+    const long long nA = 2LL * w * nx, nB = 2LL * w * (ny - 2 * w);
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= nA + nB) return;
+    int x, y;
+    if (id < nA) { const int r = (int)(id / nx); x = (int)(id - (long long)r * nx); y = r < w ? r : ny - 2 * w + r; }
+    else { const long long k = id - nA; const int r = (int)(k / (2 * w)), cidx = (int)(k - (long long)r * 2 * w); y = w + r; x = cidx < w ? cidx : nx - 2 * w + cidx; }
+    const double c = cbuf[id];
+    D[(size_t)y * nx + x] -= mode ? -c : c;
 }
 
 cudaError_t launch_subtract(sfft_plan *p, const double *S, const double *R, const double *coef, double *D,
                             const void *spec, int mode) {
     const Geom &g = p->g;
     if (!spec) spec = p->mask ? p->specTo : p->specT; // a mask keeps a second, unmasked set (C7); without one the fit spectra are it
+    const bool fix = (g.Mx != g.nx || g.My != g.ny) && g.w > 0;
+    const long long nb = 2LL * g.w * g.nx + 2LL * g.w * (g.ny - 2 * g.w);
+    if (fix) {   // the corrections on a side stream beside the transforms (needs R and the coefficients only)
+        fork_side(p);
+        use_side(p, 0);
+        { KLaunch kl(p, "wrapcorr"); wrapcorr_kernel<<<(unsigned)((4 * nb + 127) / 128), 128, 0, p->cur>>>(R, coef, p->wcorr, g); }
+        back_to_main(p);
+    }
     cudaError_t e = launch_col_inv(p, spec, coef, p->inter);
     if (e == cudaSuccess) e = launch_row_inv(p, p->inter, S, coef, D, mode);
     if (e != cudaSuccess) return e;
-    if ((g.Mx != g.nx || g.My != g.ny) && g.w > 0) {
-        const long long nb = 2LL * g.w * g.nx + 2LL * g.w * (g.ny - 2 * g.w);
-        KLaunch kl(p, "wrapfix");
-        wrapfix_kernel<<<(unsigned)((4 * nb + 127) / 128), 128, 0, p->stream>>>(R, coef, D, g, mode);
+    if (fix) {
+        join_side(p);
+        KLaunch kl(p, "wrapapply");
+        wrapapply_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, p->stream>>>(p->wcorr, D, g, mode);
     }
     return cudaGetLastError();
 }

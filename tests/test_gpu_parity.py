@@ -39,6 +39,9 @@ def assert_system(G, h, G0, h0, Sf):
     assert np.all(np.abs(G - G0) <= TOL_G * np.outer(d, d)), np.max(np.abs(G - G0) / np.outer(d, d))
     assert np.all(np.abs(h - h0) <= TOL_H * d * np.linalg.norm(Sf)), np.max(np.abs(h - h0) / (d * np.linalg.norm(Sf)))
     assert np.array_equal(G, G.T)
+    # the plain element-wise relative error, for every entry that is not a cancellation: floor 1e-6 of the scale
+    big = np.abs(G0) >= 1e-6 * np.outer(d, d)
+    assert np.max(np.abs(G - G0)[big] / np.abs(G0)[big]) <= 1e-8
 
 
 def assert_coeffs(c, c0, nker):
@@ -381,6 +384,26 @@ def test_cross_convolve_then_subtract_on_one_plan():
     assert_coeffs(c.cpu().numpy(), c0, L * L * 3)
     D0 = oracle.subtract(Sc0, Rc0, L, 1, 1, c0)
     assert np.max(np.abs(D.cpu().numpy() - D0)) <= TOL_D * 20.0
+    p.destroy()
+
+
+def test_scratch_users_between_build_and_subtract():
+    """sfft_convolve_stamp and sfft_decorrelation_stamp use the science-spectrum and intermediate buffers as scratch; both
+    are dead between the plan's calls, so calling them between build_system, solve and subtract must change nothing."""
+    nx, ny, L = 100, 72, 5
+    S, R = starfield.random_pair(nx, ny, seed=21)
+    p = SfftPlan(nx, ny, L, 1, 1)
+    p.build_system(dev(S), dev(R)); p.solve(); D0, c0 = p.subtract(); p.sync_status()
+    D0, c0 = D0.clone(), c0.clone()
+    st = dev(_psf_stamp(L, 3, 1.0))
+    p.build_system(dev(S), dev(R))
+    junk = p.convolve_stamp(dev(R), st)
+    p.solve()
+    W = p.decorrelation_stamp(st, st, st, 4.0, 1.0, 32)
+    junk2 = p.convolve_stamp(dev(S), W)
+    D1, c1 = p.subtract()
+    p.sync_status()
+    assert torch.equal(c0, c1) and torch.equal(D0, D1)
     p.destroy()
 
 
