@@ -48,7 +48,7 @@ __device__ __forceinline__ void tma_load3(void *dst, const CUtensorMap *tm, int 
 // Spectra are column-major, so the 8 consecutive b of one (spectrum, kx, a) are one 128-byte line: a stage is the
 // TMA box {8 b, 16 a, KXC kx, all template spectra} (+ one box per science spectrum) + the 8 W phase factors,
 // landing as [spectrum][kx][a][b]; stages form a ring with full/done mbarriers, thread 0 issues.
-// grid = (kx blocks, pair groups, b splits * halves); block = npg * KXC * 8 threads.
+// grid = (pair groups * lag halves, kx blocks, b splits); block = npg * KXC * 8 threads.
 template <int DLO, int DHI>
 __device__ __forceinline__ void lag_fold(const cplx *x, const cplx *ph, cplx *acc) {
 #pragma unroll
@@ -72,19 +72,20 @@ struct LagArgs {
 };
 
 template <int DLO, int DHI, typename ST>
-__device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int zsplit,
+__device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int group, int zsplit,
                                             const cplx *__restrict__ PH, cplx *__restrict__ Q, const Geom &g,
                                             unsigned char *tile, unsigned long long *full, unsigned long long *done) {
     const int Hx = g.Hx, Tb = g.My / LC_NA, KXC = la.KXC, W = la.W, NK = g.NK;
     const int col_elems = LC_NA * LC_NB;                       // one (spectrum, kx) of a stage: 128 elements of ST
     // a stage: the spectra part in ST elements, then the phase factors (cplx); sized in bytes
     const unsigned spec_bytes = (unsigned)(la.ns * KXC * col_elems * sizeof(ST)), stage_bytes = spec_bytes + (unsigned)(la.phW * LC_NB * sizeof(cplx));
-    const int kx0 = blockIdx.x * KXC;
+    const int kx0 = blockIdx.y * KXC;   // (the pair group is the FASTEST grid index: the groups of one kx chunk run side by
+                                        //  side and the second reads the chunk's spectra from L2, not from DRAM again)
     const int b0 = zsplit * la.nbs, b1 = min(Tb, b0 + la.nbs);
     const int nIt = max(0, (b1 - b0) / LC_NB);
     const int bl = threadIdx.x & (LC_NB - 1), u = threadIdx.x >> 3;
     const int lp = u / KXC, kxl = u - lp * KXC;
-    const int p = blockIdx.y * la.npg + lp;
+    const int p = group * la.npg + lp;
     const bool active = (p < pl.np) && (lp < la.npg);
     const int sa = active ? pl.a[p] : 0, sb = active ? pl.b[p] : 0;
     constexpr int NACC = DHI - DLO + 1;
@@ -147,7 +148,7 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
 }
 
 // WB <= 10: one thread folds all 2 WB + 1 lags.  WB = 20: the lag range is split in two halves
-// (blockIdx.z parity) to keep the accumulators in registers; both halves write disjoint rows of Q.
+// (blockIdx.x parity) to keep the accumulators in registers; both halves write disjoint rows of Q.
 template <int WB, typename ST>
 __global__ void __launch_bounds__(192, 2)
 lagcol_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, const cplx *__restrict__ PH, cplx *__restrict__ Q, Geom g) {
@@ -155,11 +156,11 @@ lagcol_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, con
     __shared__ unsigned long long full[4], done[4];
     unsigned char *tile = smem_raw;
     if (WB > 10) {
-        const int half = blockIdx.z & 1, zs = blockIdx.z >> 1;
-        if (half == 0) lagcol_body<0, WB, ST>(maps, la, pl, zs, PH, Q, g, tile, full, done);
-        else lagcol_body<-WB, -1, ST>(maps, la, pl, zs, PH, Q, g, tile, full, done);
+        const int half = blockIdx.x & 1, grp = blockIdx.x >> 1;   // (the lag halves too: fastest index, shared L2 reads)
+        if (half == 0) lagcol_body<0, WB, ST>(maps, la, pl, grp, blockIdx.z, PH, Q, g, tile, full, done);
+        else lagcol_body<-WB, -1, ST>(maps, la, pl, grp, blockIdx.z, PH, Q, g, tile, full, done);
     } else {
-        lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.z, PH, Q, g, tile, full, done);
+        lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, blockIdx.z, PH, Q, g, tile, full, done);
     }
 }
 
@@ -313,7 +314,7 @@ template <int WB>
 static cudaError_t run_lagcol(sfft_plan *p, const LagMaps &maps, int ns, int nsci, const PairList &pl, int W, const LagCfg &c, bool science) {
     LagArgs la;
     la.ns = ns; la.nsci = nsci; la.npg = c.npg; la.KXC = c.KXC; la.W = W; la.nbs = c.rows_per_split; la.nst = c.nst; la.phW = c.WB;
-    dim3 grid(c.nkb, c.ngr, c.nsplit * c.halves);
+    dim3 grid(c.ngr * c.halves, c.nkb, c.nsplit);
     KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega");
     if (p->spec32) lagcol_kernel<WB, float2><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
     else lagcol_kernel<WB, cplx><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
