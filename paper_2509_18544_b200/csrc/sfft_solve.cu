@@ -28,103 +28,39 @@ __global__ void equil_scale_kernel(const double *__restrict__ G, const double *_
     Lf[id] = c <= r ? dscale[r] * G[id] * dscale[c] : 0.0;
 }
 
-// Fused panel step: every CTA factors the diagonal block k0..k0+bs redundantly (thread (r, cq) keeps
-// a[r][c], c = cq mod 4, in 16 registers; one barrier per column, through which the current column is
-// shared), CTA 0 writes L_kk back, and CTA b then solves its own 64 rows below the block,
-// X L_kk^T = A, by a register-resident right-looking substitution (4 lanes per row, shuffles only).
-// No FP64 division or sqrt on the dependent chain: inv = rsqrt(pivot), L_jj = pivot * inv.
-// The chain is INSTRUCTION-bound (ncu: 40 % issue utilisation on the one busy SM, ~135 instructions per
-// column and thread), so the loops below are written for instruction count:
-//   * the 16 column groups run as 4 chunks of 4 with a compile-time register window WIN = 16, 12, 8, 4
-//     (rolled inside a chunk, the window shifts down one group per iteration);
-//   * the rank-1 updates are UNCONDITIONAL: entries right of the diagonal (c > r), rows already finished
-//     (r <= j) and window slots past the last column only ever receive values that are never read
-//     (every read of areg / xr is guarded by c <= r or c < bs), so no predicates are computed for them;
-//     shared arrays are padded so that those dead reads stay in bounds.
-// grid = max(1, row tiles below); block 256; static smem.
-constexpr int CPAD = CB + 16; // dead-slot reads reach index 63 + 4 * 3
-
-template <int WIN>
-__device__ __forceinline__ void potrf_chunk(double (&areg)[16], double (*col)[CPAD], double *rd, double (*l)[CB + 1],
-                                            double *__restrict__ Ldiag, int j4_0, int r, int cq, int tid, int *flag) {
-#pragma unroll 1
-    for (int j4 = j4_0; j4 < j4_0 + 4; j4++) {
-#pragma unroll
-        for (int jj = 0; jj < 4; jj++) {
-            const int j = 4 * j4 + jj;
-            double *cj = col[jj & 1];
-            if (cq == jj && r >= j) cj[r] = areg[0];
-            __syncthreads();
-            // all shared-memory reads of this step are issued before the rsqrt chain, so their latency hides behind it
-            const double *cjc = cj + 4 * j4 + cq;
-            double piv = cj[j];
-            const double cr = cj[r];
-            double cv[WIN];
-#pragma unroll
-            for (int qq = 0; qq < WIN; qq++) cv[qq] = cjc[4 * qq];
-            if (!(piv > PIVOT_MIN)) { if (tid == 0 && blockIdx.x == 0) *flag = 1; piv = 1.0; }
-            const double inv = rsqrt(piv);
-            const double lr = (r == j) ? piv * inv : cr * inv;
-            if (tid == 0) rd[j] = inv;
-            if (cq == jj && r >= j) areg[0] = lr;
-            const double lri = -lr * inv;
-            if (cq > jj) areg[0] = fma(lri, cv[0], areg[0]);
-#pragma unroll
-            for (int qq = 1; qq < WIN; qq++) areg[qq] = fma(lri, cv[qq], areg[qq]);
-        }
-        {
-            const int c = 4 * j4 + cq;
-            l[r][c] = c <= r ? areg[0] : 0.0;
-            // the factored block goes to Ldiag, NOT back into Lf: the other CTAs of this launch read the
-            // unfactored block from Lf whenever they get scheduled
-            if (blockIdx.x == 0) Ldiag[r * CB + c] = c <= r ? areg[0] : 0.0;
-        }
-#pragma unroll
-        for (int qq = 0; qq < WIN - 1; qq++) areg[qq] = areg[qq + 1];
-        areg[WIN - 1] = 0.0;
-    }
-}
-
-// panel rows: x_j = x_j / l_jj, then x_c -= x_j l_cj for c > j; lanes 4g..4g+3 hold row r; same window shift
-template <int WIN>
-__device__ __forceinline__ void panel_chunk(double (&xr)[16], const double *rd, double (*l)[CB + 1], double *__restrict__ Lf,
-                                            int j4_0, int r, int cq, int lane, int r0, int n, int k0, int bs) {
-#pragma unroll 1
-    for (int j4 = j4_0; j4 < j4_0 + 4; j4++) {
-#pragma unroll
-        for (int jj = 0; jj < 4; jj++) {
-            const int j = 4 * j4 + jj;
-            const double *lc = &l[4 * j4 + cq][j];
-            double lv[WIN];
-#pragma unroll
-            for (int qq = 0; qq < WIN; qq++) lv[qq] = lc[(size_t)4 * qq * (CB + 1)];
-            double xj = xr[0] * rd[j];
-            xj = __shfl_sync(0xffffffffu, xj, (lane & ~3) | jj);
-            if (cq == jj) xr[0] = xj;
-            const double nxj = -xj;
-            if (cq > jj) xr[0] = fma(nxj, lv[0], xr[0]);
-#pragma unroll
-            for (int qq = 1; qq < WIN; qq++) xr[qq] = fma(nxj, lv[qq], xr[qq]);
-        }
-        {
-            const int c = 4 * j4 + cq;
-            if (r0 + r < n && c < bs) Lf[(size_t)(r0 + r) * n + k0 + c] = xr[0];
-        }
-#pragma unroll
-        for (int qq = 0; qq < WIN - 1; qq++) xr[qq] = xr[qq + 1];
-        xr[WIN - 1] = 0.0;
-    }
-}
+constexpr int MP = 8;       // micro-panel width = the DMMA tile
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b);
 
-// U = A B^T for two 64 x 64 shared-memory tiles (leading dimension CLD) on the FP64 tensor pipe, written to
-// out[r][c]; 8 warps, warp tile 16 x 32 (the same fragment layout as syrk_kernel).
-__device__ __forceinline__ void tile_abt(const double (*As)[CLD], const double (*Bs)[CLD], double (*out)[CB + 1], int tid) {
-    const int warp = tid >> 5, lane = tid & 31;
-    const int rw = (warp >> 1) * 16, cw = (warp & 1) * 32;
-    const int fr = lane >> 2, fk = lane & 3;
-    double acc[2][4][2];
+// ---- panel step of the blocked Cholesky ------------------------------------------------------------------------
+// One launch per 64-column panel; CTA b owns the 64 rows r0.. below the diagonal block and (redundantly, like every
+// CTA of the launch) the diagonal block itself: a 128 x 64 matrix M = [A_kk; A_bk] in shared memory.  The panel is
+// factored LEFT-LOOKING in micro-panels of 8 columns, the shape of the FP64 tensor instruction (mma.sync m8n8k4):
+//   P/U(q) every 8-row tile t >= q of M:  M[t, Cq] -= M[t, C<q] M[q, C<q]^T           (DMMA, 2q k-steps)
+//   D(q)   the warp that owns tile q factors the 8 x 8 diagonal tile IN REGISTERS (accumulator layout, columns
+//          shared by shuffles: no barrier on the 8-pivot chain, rsqrt instead of sqrt and divide) and carries the
+//          row operations along on an identity, which yields W = L_qq^-1 for free (micro_potrf)
+//   S(q)   every tile t > q:  M[t, Cq] = M[t, Cq] W^T                                  (DMMA, 2 k-steps)
+// so the rows below the diagonal -- of the diagonal block and of the panel alike -- never see a substitution chain,
+// and the only serial work is D: the next owner solves and updates its own diagonal tile straight after barrier A
+// and starts D(q + 1) while the other warps still work on step q (named barriers, bar.arrive for the owner).
+// Measured on B200 (clock64 stamps, CTA 0 of panel 1, nothing else on the SM): D 1.35 k cycles, a step 1.8-2.0 k,
+// the 8 steps 14-16 k, the whole panel 32 k cycles against 51 k for the round-1 kernel (one barrier per column
+// across 256 threads, 445 cycles per column, then a 64-step shuffle substitution for the panel rows, bound by its
+// shared-memory reads); with a science-side CTA on the same SM every phase takes 1.5-2 x longer.
+// FUSED look-ahead (k0 > 0): the update of block column k0 by the previous panel (columns k0-64..k0-1) is applied on
+// the way in: U_dd = X_d X_d^T and U_bd = X_b X_d^T (X_d, X_b: the previous panel's rows of the diagonal block and
+// of this CTA's rows) by DMMA, subtracted from the tiles (which are loaded one phase ahead of their use) as they
+// are written to M.  The trailing-update kernel then only covers block columns >= k0 + 64 and runs beside this
+// kernel (launch_factor).
+// CTA 0 writes L_kk to Ldiag, NOT back into Lf: the other CTAs of the launch read the unfactored block from Lf
+// whenever they get scheduled.  grid = max(1, row tiles below); block 256; dynamic smem 2 * 64 * CLD doubles
+// (X_d, X_b, then M) -- 70 KB, so a panel CTA fits beside a science-side CTA.
+
+// acc = A B^T for two 64 x 64 shared-memory tiles (leading dimension CLD); 8 warps, warp tile 16 x 32: lane (fr, fk)
+// holds rows rw + 8a + fr, columns cw + 8b + 2fk, +1 (the same fragment layout as syrk_kernel)
+__device__ __forceinline__ void tile_abt(const double (*As)[CLD], const double (*Bs)[CLD], double (&acc)[2][4][2], int rw, int cw,
+                                         int fr, int fk) {
 #pragma unroll
     for (int a = 0; a < 2; a++)
 #pragma unroll
@@ -141,88 +77,223 @@ __device__ __forceinline__ void tile_abt(const double (*As)[CLD], const double (
 #pragma unroll
             for (int b = 0; b < 4; b++) dmma884(acc[a][b][0], acc[a][b][1], af[a], bf[b]);
     }
+}
+
+// D(q): Cholesky of the 8 x 8 diagonal tile and its inverse, by one warp, in the DMMA accumulator layout: lane
+// (fr, fk) holds a[fr][2fk], a[fr][2fk+1] (lower triangle valid) and the same two entries of the row-reduced identity.
+// Right-looking, all in registers: per column j four shuffles fetch the pivot, this row's a_rj and the two a_cj of
+// this lane's columns (the tile is symmetric, so a_cj stands for a_jc), then a_rc -= a_rj a_cj / piv and
+// L_rj = a_rj / sqrt(piv); the same row operations on an identity, u_r -= (l_rj / l_jj) u_j, give row j of
+// W = L^-1 as u_j / l_jj at step j.  Column j of L and row j of W go to shared memory the moment they are final, so
+// the updates run UNCONDITIONALLY afterwards (finished entries turn into finite garbage nobody reads): ~40
+// instructions per column on a 119-cycle dependent chain (shuffle, rsqrt, two multiplies, fma).
+__device__ __forceinline__ void micro_potrf(double a0, double a1, double (*M)[CLD], double (*Ws)[MP + 2], int q, int lane, int *flag,
+                                            bool report) {
+    const int fr = lane >> 2, fk = lane & 3;
+    double w0 = (fr == 2 * fk) ? 1.0 : 0.0, w1 = (fr == 2 * fk + 1) ? 1.0 : 0.0;
+    double *lrow = &M[MP * q + fr][MP * q];
+    bool bad = false;
+#pragma unroll
+    for (int j = 0; j < MP; j++) {
+        const int jh = j >> 1;
+        const double aj = (j & 1) ? a1 : a0;                       // this lane's entry of column j if fk == jh
+        double piv = __shfl_sync(0xffffffffu, aj, 4 * j + jh);
+        const double arj = __shfl_sync(0xffffffffu, aj, (lane & ~3) | jh);
+        const double ac0 = __shfl_sync(0xffffffffu, aj, 8 * fk + jh);
+        const double ac1 = __shfl_sync(0xffffffffu, aj, 8 * fk + 4 + jh);
+        const double uj0 = __shfl_sync(0xffffffffu, w0, 4 * j + fk);
+        const double uj1 = __shfl_sync(0xffffffffu, w1, 4 * j + fk);
+        if (!(piv > PIVOT_MIN)) { bad = true; piv = 1.0; }
+        const double inv = rsqrt(piv);
+        const double lrj = arj * inv;                              // row j: a_jj / sqrt(a_jj) = l_jj
+        const double s = -lrj * inv;
+        if (fk == jh) lrow[j] = lrj;                               // (rows above j store garbage right of the diagonal)
+        if (fr == j) *reinterpret_cast<double2 *>(&Ws[j][2 * fk]) = make_double2(w0 * inv, w1 * inv);
+        a0 = fma(s, ac0, a0); a1 = fma(s, ac1, a1);
+        w0 = fma(s, uj0, w0); w1 = fma(s, uj1, w1);
+    }
+    if (bad && report && lane == 0) *flag = 1;
+}
+
+__global__ void __launch_bounds__(256, 2) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
+                                                             int bs, int *flag) {
+    extern __shared__ __align__(16) double psm[];
+    __shared__ __align__(16) double Ws[2][MP][MP + 2];
+    double (*M)[CLD] = reinterpret_cast<double (*)[CLD]>(psm);   // rows 0..63: diagonal block, 64..127: this CTA's rows
+    const int tid = threadIdx.x, lane = tid & 31, fr = lane >> 2, fk = lane & 3;
+    // the warp index through a shuffle: the compiler then knows it is warp-uniform, and the shuffles and DMMA inside
+    // the per-warp branches below compile without divergence guards (3 x fewer instructions in micro_potrf)
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    const int rw = (warp >> 1) * 16, cw = (warp & 1) * 32;
+    const int r0 = k0 + bs + blockIdx.x * CB;
+    const bool have_rows = r0 < n;
+    // the two tiles in the fragment layout of the products; every global load is issued one phase before its use:
+    // the diagonal tile with the previous panel's rows, this CTA's tile before the second product
+    double cur[2][4][2], acc[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int b = 0; b < 4; b++)
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int r = rw + 8 * a + fr, c = cw + 8 * b + 2 * fk + h;
+                double d = (r == c) ? 1.0 : 0.0;                   // identity padding for a short last block
+                if (r < bs && c < bs) d = (c <= r) ? Lf[(size_t)(k0 + r) * n + k0 + c] : 0.0;
+                cur[a][b][h] = d;
+            }
+    if (k0 > 0) {
+        double (*Xd)[CLD] = reinterpret_cast<double (*)[CLD]>(psm);
+        double (*Xb)[CLD] = reinterpret_cast<double (*)[CLD]>(psm + CB * CLD);
+        const int kp = k0 - CB; // the previous panel is always a full block
+        {
+            double td[16], tb[16]; // all loads in flight before the first store (one global round trip, not sixteen)
+#pragma unroll
+            for (int i = 0; i < 16; i++) {
+                const int e = tid + 256 * i, rr = e >> 6, cc = e & 63;
+                td[i] = (k0 + rr < n) ? Lf[(size_t)(k0 + rr) * n + kp + cc] : 0.0;
+                tb[i] = (have_rows && r0 + rr < n) ? Lf[(size_t)(r0 + rr) * n + kp + cc] : 0.0;
+            }
+#pragma unroll
+            for (int i = 0; i < 16; i++) {
+                const int e = tid + 256 * i, rr = e >> 6, cc = e & 63;
+                Xd[rr][cc] = td[i]; Xb[rr][cc] = tb[i];
+            }
+        }
+        __syncthreads();
+        tile_abt(Xd, Xd, acc, rw, cw, fr, fk);
+#pragma unroll
+        for (int a = 0; a < 2; a++)
+#pragma unroll
+            for (int b = 0; b < 4; b++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const int r = rw + 8 * a + fr, c = cw + 8 * b + 2 * fk + h;
+                    if (r < bs && c < bs && c <= r) cur[a][b][h] -= acc[a][b][h];
+                }
+    }
+    double curb[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int b = 0; b < 4; b++)
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int r = rw + 8 * a + fr, c = cw + 8 * b + 2 * fk + h;
+                curb[a][b][h] = (have_rows && r0 + r < n && c < bs) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
+            }
+    if (k0 > 0) {
+        double (*Xd)[CLD] = reinterpret_cast<double (*)[CLD]>(psm);
+        double (*Xb)[CLD] = reinterpret_cast<double (*)[CLD]>(psm + CB * CLD);
+        if (have_rows) {
+            tile_abt(Xb, Xd, acc, rw, cw, fr, fk);
+#pragma unroll
+            for (int a = 0; a < 2; a++)
+#pragma unroll
+                for (int b = 0; b < 4; b++)
+#pragma unroll
+                    for (int h = 0; h < 2; h++) {
+                        const int r = rw + 8 * a + fr, c = cw + 8 * b + 2 * fk + h;
+                        if (r0 + r < n && c < bs) curb[a][b][h] -= acc[a][b][h];
+                    }
+        }
+        __syncthreads();                                           // X_d, X_b are dead: M takes their place
+    }
 #pragma unroll
     for (int a = 0; a < 2; a++)
 #pragma unroll
         for (int b = 0; b < 4; b++) {
-            out[rw + 8 * a + fr][cw + 8 * b + 2 * fk] = acc[a][b][0];
-            out[rw + 8 * a + fr][cw + 8 * b + 2 * fk + 1] = acc[a][b][1];
+            const int r = rw + 8 * a + fr, c = cw + 8 * b + 2 * fk;
+            *reinterpret_cast<double2 *>(&M[r][c]) = make_double2(cur[a][b][0], cur[a][b][1]);
+            *reinterpret_cast<double2 *>(&M[CB + r][c]) = make_double2(curb[a][b][0], curb[a][b][1]);
         }
-}
-
-// FUSED look-ahead (k0 > 0): the update of block column k0 by the previous panel (columns k0-64..k0-1) is applied here,
-// in registers, instead of by a separate trailing-update launch on the critical path: every CTA forms
-// U_dd = X_d X_d^T (X_d: the previous panel's rows of this diagonal block) and U_bd = X_b X_d^T for its own rows
-// with DMMA and subtracts them from the tiles it has just loaded.  The trailing-update kernel then only covers
-// block columns >= k0 + 64 and runs beside this kernel (launch_factor).
-// dynamic smem: 2 * 64 * CLD doubles (X_b, X_d).
-__global__ void __launch_bounds__(256, 2) potrf_panel_kernel(double *__restrict__ Lf, double *__restrict__ Ldiag, int n, int k0,
-                                                         int bs, int *flag) {
-    extern __shared__ __align__(16) double psm[];
-    __shared__ double l[CPAD][CB + 1];
-    __shared__ double col[2][CPAD];
-    __shared__ double rd[CB];
-    const int tid = threadIdx.x, r = tid >> 2, cq = tid & 3, lane = tid & 31;
-    const int r0 = k0 + bs + blockIdx.x * CB;
-    const bool have_rows = r0 < n;
-    double areg[16], xr[16];
-#pragma unroll
-    for (int q = 0; q < 16; q++) {
-        const int c = 4 * q + cq;
-        double v = (r == c) ? 1.0 : 0.0;                         // identity padding for a short last block
-        if (r < bs && c < bs) v = (c <= r) ? Lf[(size_t)(k0 + r) * n + k0 + c] : 0.0;
-        areg[q] = v;
-        xr[q] = (have_rows && r0 + r < n && c < bs) ? Lf[(size_t)(r0 + r) * n + k0 + c] : 0.0;
-    }
-    if (k0 > 0) {
-        double (*Xb)[CLD] = reinterpret_cast<double (*)[CLD]>(psm);
-        double (*Xd)[CLD] = reinterpret_cast<double (*)[CLD]>(psm + CB * CLD);
-        const int kp = k0 - CB; // the previous panel is always a full block
-        double td[16], tb[16]; // all 32 loads in flight before the first store (one global round trip, not sixteen)
-#pragma unroll
-        for (int i = 0; i < 16; i++) {
-            const int e = tid + 256 * i, rr = e >> 6, cc = e & 63;
-            td[i] = (k0 + rr < n) ? Lf[(size_t)(k0 + rr) * n + kp + cc] : 0.0;
-            tb[i] = (have_rows && r0 + rr < n) ? Lf[(size_t)(r0 + rr) * n + kp + cc] : 0.0;
+    __syncthreads();
+    // ---- the micro-panel pipeline -----------------------------------------------------------------------------
+    // Warp w owns diagonal tile w and panel tile 8 + w (rows 64 + 8w..).  Step q:
+    //   phase 1  warp q factors tile q (D); in its shadow the others apply the k-blocks < q to column block q + 1 (P)
+    //   barrier A (everyone)
+    //   phase 2  S(q): X = M[t, Cq] W^T.  Warp q + 1 does its diagonal tile only, ARRIVES at barrier B without
+    //            waiting, applies the last k-block to that tile in registers and goes straight on to D(q + 1)
+    //   barrier B (the others wait), phase 3: the last k-block q of column block q + 1 for all other tiles
+    // so a step costs the chain D + A + four DMMA latencies.  The panel tile of a warp that is on the chain is handled
+    // by the previous owner (which has no diagonal tile left).
+    const bool rows = have_rows;
+    constexpr int NQ = CB / MP;
+    // M[t, cb] -= sum over k-blocks [p0, p1) of M[t, p] M[cb, p]^T; two accumulation chains
+    auto upd = [&](int t, int cb, int p0, int p1) -> double2 {
+        const double *ar = &M[MP * t + fr][fk], *br = &M[MP * cb + fr][fk];
+        double2 c = *reinterpret_cast<const double2 *>(&M[MP * t + fr][MP * cb + 2 * fk]), e = make_double2(0.0, 0.0);
+#pragma unroll 2
+        for (int kk = MP * p0; kk < MP * p1; kk += 8) {
+            dmma884(c.x, c.y, -ar[kk], br[kk]);
+            dmma884(e.x, e.y, -ar[kk + 4], br[kk + 4]);
         }
-#pragma unroll
-        for (int i = 0; i < 16; i++) {
-            const int e = tid + 256 * i, rr = e >> 6, cc = e & 63;
-            Xd[rr][cc] = td[i]; Xb[rr][cc] = tb[i];
-        }
-        __syncthreads();
-        tile_abt(Xd, Xd, l, tid);
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < 16; q++) {
-            const int c = 4 * q + cq;
-            if (r < bs && c < bs && c <= r) areg[q] -= l[r][c];
-        }
-        __syncthreads();
-        if (have_rows) {
-            tile_abt(Xb, Xd, l, tid);
-            __syncthreads();
-#pragma unroll
-            for (int q = 0; q < 16; q++) {
-                const int c = 4 * q + cq;
-                if (r0 + r < n && c < bs) xr[q] -= l[r][c];
+        return make_double2(c.x + e.x, c.y + e.y);
+    };
+    auto put = [&](int t, int cb, double2 v) { *reinterpret_cast<double2 *>(&M[MP * t + fr][MP * cb + 2 * fk]) = v; };
+    // X = M[t, Cq] W^T
+    auto solve = [&](int t, int q, const double (*W)[MP + 2]) {
+        const double w0 = W[fr][fk], w1 = W[fr][4 + fk];
+        const double f0 = M[MP * t + fr][MP * q + fk], f1 = M[MP * t + fr][MP * q + 4 + fk];
+        double2 x = make_double2(0.0, 0.0), y = x;
+        dmma884(x.x, x.y, f0, w0);
+        dmma884(y.x, y.y, f1, w1);
+        __syncwarp();
+        put(t, q, make_double2(x.x + y.x, x.y + y.y));
+    };
+    double2 dt = *reinterpret_cast<const double2 *>(&M[MP * warp + fr][MP * warp + 2 * fk]);   // used by warp 0 first
+#pragma unroll 1
+    for (int q = 0; q < NQ; q++) {
+        const double (*W)[MP + 2] = Ws[q & 1];
+        if (warp == q) micro_potrf(dt.x, dt.y, M, Ws[q & 1], q, lane, flag, blockIdx.x == 0);
+        else if (q >= 1 && q + 1 < NQ) {
+            if (warp > q) put(warp, q + 1, upd(warp, q + 1, 0, q));
+            if (rows) {
+                put(8 + warp, q + 1, upd(8 + warp, q + 1, 0, q));
+                if (warp == q - 1) put(8 + q, q + 1, upd(8 + q, q + 1, 0, q));
             }
         }
-        __syncthreads();
+        asm volatile("bar.sync 1, 256;" ::: "memory");             // A: W_q, L_qq and every P are in place
+        if (warp == q + 1) {
+            solve(warp, q, W);
+            __syncwarp();
+            asm volatile("bar.arrive 2, 256;" ::: "memory");       // B: X[q + 1, q] is out; do not wait for the others
+            dt = upd(warp, q + 1, q, q + 1);
+        } else {
+            if (warp > q + 1) solve(warp, q, W);
+            if (rows) {
+                solve(8 + warp, q, W);
+                if (warp == q && q + 1 < NQ) solve(8 + q + 1, q, W);
+            }
+            asm volatile("bar.sync 2, 256;" ::: "memory");         // B: every X[., q] is visible
+            if (q + 1 < NQ) {
+                if (warp > q + 1) put(warp, q + 1, upd(warp, q + 1, q, q + 1));
+                if (rows) {
+                    put(8 + warp, q + 1, upd(8 + warp, q + 1, q, q + 1));
+                    if (warp == q) put(8 + q + 1, q + 1, upd(8 + q + 1, q + 1, q, q + 1));
+                }
+            }
+        }
     }
-    if (tid < 2 * CPAD) col[tid / CPAD][tid % CPAD] = 0.0;       // dead-slot reads must see numbers (0 * NaN would not matter, but keep it clean)
-    for (int e = tid; e < (CPAD - CB) * (CB + 1); e += 256) l[CB + e / (CB + 1)][e % (CB + 1)] = 0.0;
     __syncthreads();
-    potrf_chunk<16>(areg, col, rd, l, Ldiag, 0, r, cq, tid, flag);
-    potrf_chunk<12>(areg, col, rd, l, Ldiag, 4, r, cq, tid, flag);
-    potrf_chunk<8>(areg, col, rd, l, Ldiag, 8, r, cq, tid, flag);
-    potrf_chunk<4>(areg, col, rd, l, Ldiag, 12, r, cq, tid, flag);
-    __syncthreads();
-    if (!have_rows) return;
-    panel_chunk<16>(xr, rd, l, Lf, 0, r, cq, lane, r0, n, k0, bs);
-    panel_chunk<12>(xr, rd, l, Lf, 4, r, cq, lane, r0, n, k0, bs);
-    panel_chunk<8>(xr, rd, l, Lf, 8, r, cq, lane, r0, n, k0, bs);
-    panel_chunk<4>(xr, rd, l, Lf, 12, r, cq, lane, r0, n, k0, bs);
+    // write-out, all shared-memory reads of a thread before its first store
+    {
+        const int c = tid & 63, rb = tid >> 6;
+        if (blockIdx.x == 0) {
+            double v[16];
+#pragma unroll
+            for (int i = 0; i < 16; i++) v[i] = M[rb + 4 * i][c];
+#pragma unroll
+            for (int i = 0; i < 16; i++) Ldiag[(rb + 4 * i) * CB + c] = c <= rb + 4 * i ? v[i] : 0.0;
+        }
+        if (have_rows) {
+            double v[16];
+#pragma unroll
+            for (int i = 0; i < 16; i++) v[i] = M[CB + rb + 4 * i][c];
+#pragma unroll
+            for (int i = 0; i < 16; i++)
+                if (r0 + rb + 4 * i < n && c < bs) Lf[(size_t)(r0 + rb + 4 * i) * n + k0 + c] = v[i];
+        }
+    }
 }
 
 // Inverses of the 64 x 64 diagonal blocks of the factor (identity-padded), for the triangular solves.
