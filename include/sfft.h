@@ -293,6 +293,27 @@ const char *sfft_version(void);
  * Returns INVALID_ARG if nbytes is not the array's size. */
 sfft_status sfft_debug_read(sfft_plan *plan, int which, int idx, void *host_dst, size_t nbytes);
 
+/* Allocation-free variant of step a4 (north_star (c), reading C9): solves G c = h by the
+ * same kernels as sfft_solve (Jacobi equilibration, blocked Cholesky, the two triangular solves) WITHOUT a plan and
+ * without allocating anything: no cudaMalloc / cudaFree, no stream or event creation, no allocating library call.
+ * For callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ *   G  DEVICE, n x n doubles, row-major, symmetric positive definite; only the lower triangle (c <= r) is read
+ *   h  DEVICE, n doubles          c  DEVICE, n doubles, written          (caller-owned; G and h are not modified)
+ *   n  1 <= n <= SFFT_SOLVE_STATIC_MAX_N; larger n (or n < 1, or a NULL pointer) returns SFFT_ERR_INVALID_ARG and
+ *      sfft_solve_static_last_error() names the limit
+ *   cuda_stream  the cudaStream_t the work is ordered on (NULL = the default stream)
+ * Scratch (the factor, the inverted diagonal blocks, the scaling, the exchange words of the triangular solves, the
+ * flags: 8.6 MiB) lives in ONE file-scope `static __device__` array: every GPU that loads the library holds it until
+ * the process exits.  Every call on a device shares it and it keeps the previous call's contents (the call clears
+ * what must start at zero), so calls that overlap on the GPU -- two streams, two host threads -- RACE: serialise them.
+ * The call BLOCKS until the solve has finished (it reads the pivot flag back) and returns SFFT_ERR_NOT_SPD if a pivot
+ * of the equilibrated matrix was <= 1e-12 (c is then meaningless), SFFT_ERR_CUDA on a CUDA error or a lost exchange
+ * block (c is then NaN-poisoned). */
+#define SFFT_SOLVE_STATIC_MAX_N 1024
+sfft_status sfft_solve_static(const double *G, const double *h, double *c, int n, void *cuda_stream);
+/* Thread-local, NUL-terminated description of the calling thread's most recent sfft_solve_static error ("" if none). */
+const char *sfft_solve_static_last_error(void);
+
 /* FP64 rate probes used by bench.py to state the ALU roofline it divides by
  * (DESIGN.md "peaks"): runs a register-resident DFMA (kind=0) or DMMA m8n8k4 (kind=1)
  * loop on every SM for `iters` iterations and returns the achieved TFLOP/s in *tflops. */

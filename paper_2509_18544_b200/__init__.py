@@ -4,4 +4,4 @@ The product is libsfft.so (C ABI in include/sfft.h, CUDA kernels in csrc/); `sff
 ctypes binding and `starfield` the seeded synthetic input generators.
 """
 from . import starfield  # noqa: F401
-from .sfft import SfftError, SfftPlan, load_library, probe_fp64, version  # noqa: F401
+from .sfft import SfftError, SfftPlan, load_library, probe_fp64, solve_static, version  # noqa: F401

@@ -4,7 +4,10 @@
 // solve, trailing update C -= X X^T on the FP64 tensor pipe (mma.sync m8n8k4 f64 -- the one
 // dense contraction of the path).  A pivot L_kk^2 <= 1e-12 raises the device flag
 // (SFFT_ERR_NOT_SPD).  c = D^-1/2 L^-T L^-1 D^-1/2 h by two blocked triangular solves.
+#include <cstdarg>
+#include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -620,4 +623,101 @@ cudaError_t launch_trisolve(sfft_plan *p, const double *h, double *c, cudaStream
     return cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, st ? st : p->stream);
 }
 
+// ---- sfft_solve_static: the same solve with its scratch in a file-scope device array (include/sfft.h) -----------
+// Layout of the array, in doubles (every part starts on a 256-byte boundary):
+//   Lf [MAX_N * MAX_N] (used with leading dimension n) | Linv [MAX_N / 64 blocks of 64 x 64] | dscale [MAX_N]
+//   | y, z exchange words [2 * MAX_N each] | flags (2 ints: pivot test, solve error)
+constexpr int SS_MAXN = SFFT_SOLVE_STATIC_MAX_N;
+static_assert(SS_MAXN % CB == 0, "the scratch layout assumes whole blocks");
+constexpr size_t SS_LF = 0, SS_LINV = SS_LF + (size_t)SS_MAXN * SS_MAXN, SS_DSC = SS_LINV + (size_t)SS_MAXN * CB,
+                 SS_Y = SS_DSC + SS_MAXN, SS_Z = SS_Y + 2 * SS_MAXN, SS_FLAG = SS_Z + 2 * SS_MAXN, SS_TOTAL = SS_FLAG + 32;
+static __device__ __align__(256) double g_solve_scratch[SS_TOTAL];
+
+constexpr int SS_MAXDEV = 64;
+struct StaticSolveDev { double *base; int epoch; };
+static StaticSolveDev g_ss_dev[SS_MAXDEV];          // per device: the array's DEVICE address and the solve epoch
+static std::mutex g_ss_mutex;
+static thread_local char g_ss_err[256];
+
+static sfft_status ss_fail(sfft_status st, const char *fmt, ...) {
+    va_list ap; va_start(ap, fmt); vsnprintf(g_ss_err, sizeof g_ss_err, fmt, ap); va_end(ap);
+    return st;
+}
+
+// Once per device, with that device current.  In host code the name g_solve_scratch is a host-side stand-in, not a
+// device address: the kernels get the address cudaGetSymbolAddress returns for THIS device.
+static cudaError_t ss_setup(int dev, cudaStream_t st, StaticSolveDev **out) {
+    std::lock_guard<std::mutex> lock(g_ss_mutex);
+    StaticSolveDev &d = g_ss_dev[dev];
+    if (!d.base) {
+        double *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_solve_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        // epoch 0 never matches a solve: the exchange words start cleared
+        e = cudaMemsetAsync(ptr + SS_Y, 0, sizeof(double) * 4 * SS_MAXN, st);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * CB * CLD * sizeof(double)));
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(potrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * CB * CLD * sizeof(double)));
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * CB * (CB + 1) * sizeof(double)));
+        if (e != cudaSuccess) return e;
+        d.base = ptr; d.epoch = 0;
+    }
+    if (d.epoch == 0x7fffffff) {                   // the epoch is about to repeat: start over from cleared words
+        const cudaError_t e = cudaMemsetAsync(d.base + SS_Y, 0, sizeof(double) * 4 * SS_MAXN, st);
+        if (e != cudaSuccess) return e;
+        d.epoch = 0;
+    }
+    d.epoch++;
+    *out = &d;
+    return cudaSuccess;
+}
+
 } // namespace sfft
+
+extern "C" const char *sfft_solve_static_last_error(void) { return sfft::g_ss_err; }
+
+extern "C" sfft_status sfft_solve_static(const double *G, const double *h, double *c, int n, void *cuda_stream) {
+    using namespace sfft;
+    g_ss_err[0] = 0;
+    if (!G || !h || !c) return ss_fail(SFFT_ERR_INVALID_ARG, "sfft_solve_static: NULL pointer");
+    if (n < 1 || n > SS_MAXN)
+        return ss_fail(SFFT_ERR_INVALID_ARG, "sfft_solve_static: n = %d is outside 1..%d (SFFT_SOLVE_STATIC_MAX_N, the size of the static scratch array)", n, SS_MAXN);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return ss_fail(SFFT_ERR_CUDA, "sfft_solve_static: cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= SS_MAXDEV) return ss_fail(SFFT_ERR_INVALID_ARG, "sfft_solve_static: device %d not supported (< %d)", dev, SS_MAXDEV);
+    StaticSolveDev *d = nullptr;
+    e = ss_setup(dev, st, &d);
+    if (e != cudaSuccess) return ss_fail(SFFT_ERR_CUDA, "sfft_solve_static: set-up: %s", cudaGetErrorString(e));
+    double *Lf = d->base + SS_LF, *Linv = d->base + SS_LINV, *dscale = d->base + SS_DSC;
+    unsigned long long *y = reinterpret_cast<unsigned long long *>(d->base + SS_Y), *z = reinterpret_cast<unsigned long long *>(d->base + SS_Z);
+    int *flag = reinterpret_cast<int *>(d->base + SS_FLAG);
+    const int nblk = (n + CB - 1) / CB;
+    const size_t sm_mm = 2 * CB * CLD * sizeof(double);
+    cudaMemsetAsync(flag, 0, 2 * sizeof(int), st);  // the flags must start at zero; everything else is overwritten
+    equil_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(G, dscale, n, flag);
+    equil_scale_kernel<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, st>>>(G, dscale, Lf, n);
+    for (int kb = 0; kb < nblk; kb++) {             // launch_factor's sequence on ONE stream (no look-ahead stream or events)
+        const int k0 = kb * CB, bs = n - k0 < CB ? n - k0 : CB;
+        const int rem = n - k0 - bs, nt = (rem + CB - 1) / CB;
+        potrf_panel_kernel<<<nt > 0 ? nt : 1, 256, sm_mm, st>>>(Lf, Linv + (size_t)kb * CB * CB, n, k0, bs, flag);
+        if (nt >= 2) syrk_kernel<<<(nt - 1) * nt / 2, 256, sm_mm, st>>>(Lf, n, k0, bs, k0 + bs, 2);
+    }
+    trinv_kernel<<<nblk, 256, 3 * CB * (CB + 1) * sizeof(double), st>>>(Linv, n, 0);
+    {
+        const double *cLf = Lf, *cLi = Linv, *cds = dscale;
+        int *err = flag + 1, epoch = d->epoch, nn = n;
+        void *args[] = {(void *)&cLf, (void *)&cLi, (void *)&cds, (void *)&h, (void *)&y, (void *)&z, (void *)&c, (void *)&nn, (void *)&err, (void *)&epoch};
+        e = cudaLaunchCooperativeKernel((const void *)trisolve_kernel, dim3(nblk), dim3(256), args, 0, st);
+        if (e != cudaSuccess) return ss_fail(SFFT_ERR_CUDA, "sfft_solve_static: trisolve launch: %s", cudaGetErrorString(e));
+    }
+    int hf[2] = {0, 0};
+    e = cudaMemcpyAsync(hf, flag, sizeof hf, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return ss_fail(SFFT_ERR_CUDA, "sfft_solve_static: %s", cudaGetErrorString(e));
+    if (hf[0]) return ss_fail(SFFT_ERR_NOT_SPD, "sfft_solve_static: a pivot of the equilibrated matrix was <= 1e-12 (or a diagonal entry <= 0)");
+    if (hf[1]) return ss_fail(SFFT_ERR_CUDA, "sfft_solve_static: a triangular-solve block never arrived; c is NaN");
+    return SFFT_OK;
+}

@@ -28,7 +28,9 @@ SYMBOLS = (
     "sfft_get_system", "sfft_enable_timings", "sfft_get_timings", "sfft_kernel_timing_count",
     "sfft_kernel_timing_get", "sfft_launch_count",
     "sfft_last_error", "sfft_version", "sfft_debug_read", "sfft_probe_fp64",
+    "sfft_solve_static", "sfft_solve_static_last_error",
 )
+SOLVE_STATIC_MAX_N = 1024  # include/sfft.h: SFFT_SOLVE_STATIC_MAX_N
 
 
 class SfftError(RuntimeError):
@@ -86,6 +88,8 @@ def load_library():
     lib.sfft_version.restype = ctypes.c_char_p
     lib.sfft_debug_read.argtypes = [vp, ci, ci, vp, ctypes.c_size_t]
     lib.sfft_probe_fp64.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
+    lib.sfft_solve_static.argtypes = [dp, dp, dp, ci, vp]
+    lib.sfft_solve_static_last_error.restype = ctypes.c_char_p
     _lib = lib
     return lib
 
@@ -101,6 +105,19 @@ def probe_fp64(kind: int, iters: int = 4096) -> float:
     if rc:
         raise SfftError(rc, "sfft_probe_fp64")
     return out.value
+
+
+def solve_static(G, h, c, stream=None):
+    """sfft_solve_static: G c = h with the library's static scratch array (no allocation); G (n, n), h (n,), c (n,)
+    are the caller's CUDA float64 tensors, c is written and returned.  Blocks until done."""
+    lib = load_library()
+    n = int(h.shape[0])
+    _dev_f64(G, (n, n), "G"); _dev_f64(h, (n,), "h"); _dev_f64(c, (n,), "c")
+    st = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
+    rc = lib.sfft_solve_static(G.data_ptr(), h.data_ptr(), c.data_ptr(), n, st)
+    if rc:
+        raise SfftError(rc, "sfft_solve_static", lib.sfft_solve_static_last_error().decode())
+    return c
 
 
 def _dev_f64(t, shape, name):
