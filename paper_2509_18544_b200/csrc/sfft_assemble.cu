@@ -93,14 +93,10 @@ __global__ void __launch_bounds__(128) delta_kernel(const double *__restrict__ m
 
 __device__ __forceinline__ int pair_index(int t, int tp, int NK) { return t * NK - (t * (t - 1)) / 2 + (tp - t); }
 
-// one thread per entry of G (full matrix, both triangles)
-__global__ void gather_G_kernel(const double *__restrict__ lagO, const double *__restrict__ gam,
-                                const double *__restrict__ phi, double *__restrict__ G, Geom g) {
-    const int n = g.n, L = g.L, w = g.w, LL = L * L, NKLL = g.NK * LL, W2 = 4 * w + 1;
-    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= (long long)n * n) return;
-    const int r = (int)(id / n), c = (int)(id % n);
-    double val;
+// entry (r, c) of G from the lag tables
+__device__ __forceinline__ double g_entry(const double *__restrict__ lagO, const double *__restrict__ gam,
+                                          const double *__restrict__ phi, const Geom &g, int r, int c) {
+    const int L = g.L, w = g.w, LL = L * L, NKLL = g.NK * LL, W2 = 4 * w + 1;
     if (r < NKLL && c < NKLL) {
         const int t = r / LL, v = (r % LL) / L - w, u = (r % LL) % L - w;
         const int tp = c / LL, vp = (c % LL) / L - w, up = (c % LL) % L - w;
@@ -109,15 +105,31 @@ __global__ void gather_G_kernel(const double *__restrict__ lagO, const double *_
         int dv = v - vp, du = u - up;
         const bool flip = t > tp || (t == tp && (dv < 0 || (dv == 0 && du < 0)));
         if (flip) { dv = -dv; du = -du; }
-        val = lagO[(size_t)pair_index(flip ? tp : t, flip ? t : tp, g.NK) * W2 * W2 + (dv + 2 * w) * W2 + (du + 2 * w)];
-    } else if (r < NKLL) {
-        val = gam[((size_t)(r / LL) * g.NB + (c - NKLL)) * LL + r % LL];
-    } else if (c < NKLL) {
-        val = gam[((size_t)(c / LL) * g.NB + (r - NKLL)) * LL + c % LL];
-    } else {
-        val = phi[(r - NKLL) * g.NB + (c - NKLL)];
+        return lagO[(size_t)pair_index(flip ? tp : t, flip ? t : tp, g.NK) * W2 * W2 + (dv + 2 * w) * W2 + (du + 2 * w)];
     }
+    if (r < NKLL) return gam[((size_t)(r / LL) * g.NB + (c - NKLL)) * LL + r % LL];
+    if (c < NKLL) return gam[((size_t)(c / LL) * g.NB + (r - NKLL)) * LL + c % LL];
+    return phi[(r - NKLL) * g.NB + (c - NKLL)];
+}
+
+// one thread per entry of G (full matrix, both triangles).  The Jacobi equilibration of step a4 rides along (the
+// factorisation follows every gather, and two more small launches sat on the critical path of a step): the thread also
+// gathers its two diagonal entries and writes the scaled lower triangle Lf = D^-1/2 G D^-1/2 and D^-1/2 itself, with
+// the same expressions as equil_diag_kernel / equil_scale_kernel (sfft_solve.cu), which remain for a G that arrives
+// some other way.  *flag is raised for a diagonal entry <= 0.
+__global__ void gather_G_kernel(const double *__restrict__ lagO, const double *__restrict__ gam,
+                                const double *__restrict__ phi, double *__restrict__ G, double *__restrict__ Lf,
+                                double *__restrict__ dscale, int *flag, Geom g) {
+    const int n = g.n;
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= (long long)n * n) return;
+    const int r = (int)(id / n), c = (int)(id % n);
+    const double val = g_entry(lagO, gam, phi, g, r, c);
     G[id] = val;
+    const double grr = g_entry(lagO, gam, phi, g, r, r), gcc = g_entry(lagO, gam, phi, g, c, c);
+    const double sr = grr > 0.0 ? 1.0 / sqrt(grr) : 1.0, sc = gcc > 0.0 ? 1.0 / sqrt(gcc) : 1.0;
+    if (c == 0) { dscale[r] = sr; if (!(grr > 0.0)) *flag = 1; }
+    Lf[id] = c <= r ? sr * val * sc : 0.0;
 }
 
 __global__ void gather_h_kernel(const double *__restrict__ lagT, const double *__restrict__ delta, double *__restrict__ h, Geom g) {
@@ -142,7 +154,9 @@ cudaError_t launch_delta(sfft_plan *p, const double *muS, double *delta) {
 
 cudaError_t launch_gather_G(sfft_plan *p) {
     const long long total = (long long)p->g.n * p->g.n;
-    { KLaunch kl(p, "gather_G"); gather_G_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->lagO, p->gam, p->phi, p->G, p->g); }
+    cudaMemsetAsync(p->flag, 0, sizeof(int), p->cur);   // the pivot flag of the factorisation that follows (launch_factor)
+    { KLaunch kl(p, "gather_G"); gather_G_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->lagO, p->gam, p->phi, p->G, p->Lf, p->dscale, p->flag, p->g); }
+    p->lf_ready = true;                                  // Lf and dscale hold the equilibrated matrix of this G
     return cudaGetLastError();
 }
 

@@ -72,6 +72,7 @@ struct sfft_plan {
     sfft::Knobs knob;        // experiment knobs, read once at plan creation
     int sms;                 // multiprocessors of the plan's device
     bool factor_pending;     // factor kernels are enqueued on fstream and not yet joined into `stream`
+    bool lf_ready;           // Lf, dscale hold the equilibrated G already (written by the gather of G): launch_factor skips that step
     // device workspaces
     sfft::cplx *tw;          // [Nt]
     // planes are column-major (sfft_fft.cuh: plane_idx): intermediates [Hx][My] (column 0 packed), spectra [Hx+1][My]

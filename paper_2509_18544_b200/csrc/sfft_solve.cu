@@ -568,10 +568,13 @@ __global__ void __launch_bounds__(256) trisolve_kernel(const double *__restrict_
 cudaError_t launch_factor(sfft_plan *p) {
     const int n = p->g.n;
     cudaStream_t st = p->cur;
-    cudaMemsetAsync(p->flag, 0, sizeof(int), st);
-    { KLaunch kl(p, "equil_diag"); equil_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(p->G, p->dscale, n, p->flag); }
-    const long long total = (long long)n * n;
-    { KLaunch kl(p, "equil_scale"); equil_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p->G, p->dscale, p->Lf, n); }
+    if (!p->lf_ready) {   // (the gather of G normally leaves the equilibrated matrix behind: sfft_assemble.cu)
+        cudaMemsetAsync(p->flag, 0, sizeof(int), st);
+        { KLaunch kl(p, "equil_diag"); equil_diag_kernel<<<(n + 255) / 256, 256, 0, st>>>(p->G, p->dscale, n, p->flag); }
+        const long long total = (long long)n * n;
+        { KLaunch kl(p, "equil_scale"); equil_scale_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(p->G, p->dscale, p->Lf, n); }
+    }
+    p->lf_ready = false;  // the factor overwrites Lf
     const int nblk = (n + CB - 1) / CB;
     const size_t sm_syrk = 2 * CB * CLD * sizeof(double);
     cudaFuncSetAttribute(syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_syrk);
