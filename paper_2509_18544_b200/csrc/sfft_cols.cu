@@ -33,8 +33,10 @@ template <int LOG2N> struct ColCfg {
 };
 
 // forward transform of the canonical registers (three passes, two exchanges); natural order on return
-template <int LOG2N, int DIR>
-__device__ __forceinline__ void col_fft(cplx (&v)[16], cplx *X, int j, int bar_id, const cplx *__restrict__ tw, int Nt, cplx w2, cplx w3) {
+// after_x() is called once the thread has done its last read of X (the forward kernel hands X to the copy engine there)
+template <int LOG2N, int DIR, typename F>
+__device__ __forceinline__ void col_fft(cplx (&v)[16], cplx *X, int j, int bar_id, const cplx *__restrict__ tw, int Nt, cplx w2, cplx w3,
+                                        F &&after_x) {
     using C = ColCfg<LOG2N>;
     constexpr int T = C::T;
     {   // pass 1: radix 16, no twiddles
@@ -58,6 +60,7 @@ __device__ __forceinline__ void col_fft(cplx (&v)[16], cplx *X, int j, int bar_i
     }
     group_sync(bar_id, T);
     load_canonical<4, 1>(v, X, 0, j, T);
+    after_x();
     if (C::R3 == 16) {
         cplx x[16];
 #pragma unroll
@@ -80,65 +83,76 @@ col_fwd_kernel(const cplx *__restrict__ inter, ST *__restrict__ spec, unsigned l
     using C = ColCfg<LOG2N>;
     constexpr int N = C::N, T = C::T, G = C::G, QE = C::QE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ unsigned long long full[G * COL_RING], done[G * COL_RING];
+    __shared__ unsigned long long full[G * 4], done[G * 4];
     const int grp = threadIdx.x / T, j = threadIdx.x - grp * T, bar_id = 1 + grp;
     cplx *X = reinterpret_cast<cplx *>(smem_raw) + (size_t)grp * N;
     cplx *ring = reinterpret_cast<cplx *>(smem_raw) + (size_t)G * N + (size_t)grp * COL_RING * QE;
-    unsigned long long *bar = full + grp * COL_RING, *rel = done + grp * COL_RING;
+    // FOUR landing slots, one per quarter of a column: quarters 0..2 in the ring, quarter 3 in the first quarter of the
+    // exchange buffer X, which is idle from the last read of a transform to the first store of the next.  With three
+    // slots the fourth quarter of a column could only be asked for when its first quarter had been consumed, and every
+    // column waited a full memory latency for it (9-16 % of the kernel's stall samples sat on that wait).
+    unsigned long long *bar = full + grp * 4, *rel = done + grp * 4;
     if (j == 0) {
-        for (int s = 0; s < COL_RING; s++) { mbar_init(&bar[s], 1); mbar_init(&rel[s], T); }
+        for (int s = 0; s < 4; s++) { mbar_init(&bar[s], 1); mbar_init(&rel[s], T); }
         mbar_fence_init();
     }
     __syncthreads();
     const int Hx = g.Hx, ny = g.ny, Nt = g.Nt;
     const int wid = blockIdx.x * G + grp, nw = gridDim.x * G;
     const int ncol = wid < Hx ? (Hx - wid + nw - 1) / nw : 0;
-    const int nitems = ncol * njobs, nsteps = nitems * 4;
+    const int nitems = ncol * njobs;
     const size_t iplane = (size_t)Hx * N, splane = (size_t)(Hx + 1) * N;
     const double inv_ny = 1.0 / (double)ny;
-    auto issue = [&](int s) { // one thread: quarter Q of item n into slot s % RING
-        const int n = s >> 2, Q = s & 3, slot = s % COL_RING;
+    auto slot_ptr = [&](int Q) -> cplx * { return Q < 3 ? ring + (size_t)Q * QE : X; };
+    auto issue = [&](int n, int Q) { // one thread: quarter Q of item n into slot Q
         const int col = wid + (n / njobs) * nw, k = n % njobs;
         const int ii = (int)(jpack >> (4 * k + 2)) & 3;
         int rows = ny - Q * QE; rows = rows < 0 ? 0 : (rows > QE ? QE : rows);
-        mbar_expect(&bar[slot], (unsigned)rows * 16u);
-        if (rows > 0) bulk_g2s(ring + (size_t)slot * QE, inter + (size_t)ii * iplane + (size_t)col * N + Q * QE, (unsigned)rows * 16u, &bar[slot]);
+        mbar_expect(&bar[Q], (unsigned)rows * 16u);
+        if (rows > 0) bulk_g2s(slot_ptr(Q), inter + (size_t)ii * iplane + (size_t)col * N + Q * QE, (unsigned)rows * 16u, &bar[Q]);
     };
-    if (j == 0)
-        for (int s = 0; s < COL_RING && s < nsteps; s++) issue(s);
+    if (j == 0 && nitems > 0)
+        for (int Q = 0; Q < 4; Q++) issue(0, Q);
     const cplx w2 = tw[(size_t)(j & 15) * (Nt >> 8)];
     const cplx w3 = C::R3 == 16 ? tw[(size_t)(j & 255) * (Nt >> 12)] : mk(1.0, 0.0);
-    int s = 0;
     const int j_outer_ = j; // (see the note at opaque_index)
     for (int n = 0; n < nitems; n++) {
         const int j = opaque_index(j_outer_);
         const int col = wid + (n / njobs) * nw, k = n % njobs;
         const int jp = (int)(jpack >> (4 * k)) & 3;
+        const unsigned par = (unsigned)n & 1u;   // every slot is used once per item
+        const bool more = n + 1 < nitems;
         // weight yt^jp as the one-hot cubic c0 + y (c1 + y (c2 + y c3)): three fused multiply-adds per row, no branches on jp
         const double c0 = jp == 0 ? 1.0 : 0.0, c1 = jp == 1 ? 1.0 : 0.0, c2 = jp == 2 ? 1.0 : 0.0, c3 = jp == 3 ? 1.0 : 0.0;
         const double y0 = (2.0 * j + 1.0 - ny) * inv_ny, ystep = 2.0 * T * inv_ny;
         cplx v[16];
 #pragma unroll
-        for (int Q = 0; Q < 4; Q++, s++) {
-            const int slot = s % COL_RING;
-            mbar_wait(&bar[slot], (unsigned)(s / COL_RING) & 1u);
+        for (int Q = 0; Q < 4; Q++) {
+            const cplx *src = Q < 3 ? ring + (size_t)Q * QE : X;
+            mbar_wait(&bar[Q], par);
 #pragma unroll
             for (int qq = 0; qq < 4; qq++) {
                 const int q = 4 * Q + qq, row = j + T * q;
-                cplx a = ring[(size_t)slot * QE + qq * T + j];
+                cplx a = src[qq * T + j];
                 const double yt = fma((double)q, ystep, y0);          // yt of row j + q T
                 const double wgt = fma(yt, fma(yt, fma(yt, c3, c2), c1), c0);
                 v[q] = row < ny ? cscale(a, wgt) : mk(0.0, 0.0);
             }
             // release the slot: every thread arrives (release semantics: its loads of the slot are done) and the issuing
             // thread refills it once all have.  (A bar.sync is not enough here: the copy engine is not ordered behind
-            // it -- a refill could overtake a slow warp's reads.)
-            slot_release(&rel[slot]);
-            if (j == 0 && s + COL_RING < nsteps) { mbar_wait(&rel[slot], (unsigned)(s / COL_RING) & 1u); issue(s + COL_RING); }
+            // it -- a refill could overtake a slow warp's reads.)  Slot 3 is X: it is busy until the transform's last read.
+            if (Q < 3) {
+                slot_release(&rel[Q]);
+                if (j == 0 && more) { mbar_wait(&rel[Q], par); issue(n + 1, Q); }
+            }
         }
-        group_sync(bar_id, T); // the previous item's reads of X are done
-        col_fft<LOG2N, -1>(v, X, j, bar_id, tw, Nt, w2, w3);
+        group_sync(bar_id, T); // quarter 3 has been read out of X by everyone (and so have the previous item's results)
+        auto x_free = [&]() { // X goes to the copy engine: quarter 3 of the next item
+            slot_release(&rel[3]);
+            if (j == 0 && more) { mbar_wait(&rel[3], par); issue(n + 1, 3); }
+        };
         ST *dst = spec + (size_t)k * splane;
+        col_fft<LOG2N, -1>(v, X, j, bar_id, tw, Nt, w2, w3, [&] { if (col != 0) x_free(); });
         if (col != 0) {
 #pragma unroll
             for (int q = 0; q < 16; q++) st_c(&dst[(size_t)col * N + j + q * T], v[q]);
@@ -155,6 +169,7 @@ col_fwd_kernel(const cplx *__restrict__ inter, ST *__restrict__ spec, unsigned l
                 st_c(&dst[row], mk(0.5 * (v[q].x + m.x), 0.5 * (v[q].y - m.y)));
                 st_c(&dst[(size_t)Hx * N + row], mk(0.5 * (v[q].y + m.y), -0.5 * (v[q].x - m.x)));
             }
+            x_free();
         }
     }
 }
@@ -258,7 +273,7 @@ col_inv_kernel(const ST *__restrict__ spec, const cplx *__restrict__ Ep, cplx *_
             }
         }
         group_sync(bar_id, T); // every thread has read its taps from X
-        col_fft<LOG2N, 1>(acc, X, j, bar_id, tw, Nt, w2, w3);
+        col_fft<LOG2N, 1>(acc, X, j, bar_id, tw, Nt, w2, w3, [] {});
         cplx *dst = inter + (size_t)col * N;
 #pragma unroll
         for (int q = 0; q < 16; q++) {

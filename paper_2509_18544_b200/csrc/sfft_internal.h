@@ -75,6 +75,7 @@ struct sfft_plan {
     bool lf_ready;           // Lf, dscale hold the equilibrated G already (written by the gather of G): launch_factor skips that step
     // device workspaces
     sfft::cplx *tw;          // [Nt]
+    sfft::cplx *rtw;         // [3][Hx/16] the row passes' per-thread twiddles, compact (sfft_rows.cu: rowtw_kernel)
     // planes are column-major (sfft_fft.cuh: plane_idx): intermediates [Hx][My] (column 0 packed), spectra [Hx+1][My]
     sfft::cplx *inter;       // [(DK+1)][Hx][My] row-transformed intermediates (a1) / a5 intermediate
     // spectrum elements are complex128, or complex64 in the reduced-memory plan mode (spec32; arithmetic stays FP64)

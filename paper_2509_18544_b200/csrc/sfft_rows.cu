@@ -85,7 +85,7 @@ __device__ __forceinline__ void tangle(cplx XA, cplx XB, cplx u, cplx &Zk, cplx 
 template <int LOG2H, bool BULK, bool MASK>
 __global__ void __launch_bounds__(ROW_THREADS, 2)
 row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask, cplx *__restrict__ inter, int NI,
-               double *__restrict__ mu, int NMOM, Geom g, const cplx *__restrict__ tw) {
+               double *__restrict__ mu, int NMOM, Geom g, const cplx *__restrict__ tw, const cplx *__restrict__ rtw) {
     using C = RowCfg<LOG2H>;
     constexpr int Hx = C::Hx, T = C::T, GT = C::GT, TP = 2 * T, QP = C::QP; // TP = Hx/8: butterflies of the last pass
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -218,8 +218,11 @@ row_fwd_kernel(const double *__restrict__ img, const uint8_t *__restrict__ mask,
         pass_store<C::R2, -1, 4, 2>(v, X, r, j, T, 4, tw, Nt);
         // twiddles of the last pass and of the untangle: fetched here (not kept across the passes: 16 registers), their
         // latency hides behind the barrier
-        const cplx wA = tw[(size_t)A * (Nt >> LOG2H)], wB = tw[(size_t)B * (Nt >> LOG2H)]; // exp(-2 pi i jb/Hx)
-        const cplx uA = tw[(size_t)(j == 0 ? T : A) * (Nt >> (LOG2H + 1))];               // exp(-2 pi i k/Mx), k = A (thread 0: T)
+        // (from the compact table rtw[3][T]: three coalesced loads.  Gathered from the big table they were 16 lines per warp
+        // and load; with the shared-memory carve-out at its maximum the L1 is ~30 KB, every one missed, item after item,
+        // and the butterflies below waited for L2: 16 % of the kernel's stall samples)
+        const cplx wA = rtw[j], wB = rtw[T + j]; // exp(-2 pi i jb/Hx), jb = A, B
+        const cplx uA = rtw[2 * T + j];          // exp(-2 pi i k/Mx), k = A (thread 0: T)
         group_sync(bar_id, GT);
         // last pass: radix 8, Ns = Hx/8, butterflies A and B
         cplx zA[8], zB[8];
@@ -412,6 +415,17 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// rtw[0][j] = exp(-2 pi i j/Hx), rtw[1][j] = exp(-2 pi i B/Hx) (B = Hx/8 - j; j = 0: T), rtw[2][j] = exp(-2 pi i k/Mx)
+// (k = j; j = 0: T), j < T = Hx/16: the last-pass and untangle twiddles of thread j of row_fwd_kernel, taken from tw
+__global__ void rowtw_kernel(cplx *rtw, const cplx *__restrict__ tw, int T, int Nt, int Hx) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= T) return;
+    const int TP = 2 * T, A = j, B = j == 0 ? T : TP - j;
+    rtw[j] = tw[(size_t)A * (Nt / Hx)];
+    rtw[T + j] = tw[(size_t)B * (Nt / Hx)];
+    rtw[2 * T + j] = tw[(size_t)(j == 0 ? T : A) * (Nt / (2 * Hx))];
+}
+
 // per device and plan, at plan creation: kernel attributes and the tensor map of the a5 intermediate
 // (plane [Hx][My] complex = [Hx][2 My] doubles, box {4 doubles = rows y0, y0+1 of one kx; Hx/8 kx})
 cudaError_t rows_init(sfft_plan *p) {
@@ -420,6 +434,13 @@ cudaError_t rows_init(sfft_plan *p) {
     if (e == cudaSuccess) e = rows_attr<10>();
     if (e == cudaSuccess) e = rows_attr<11>();
     if (e != cudaSuccess) return e;
+    {   // after twiddle_kernel (same stream)
+        const int T = g.Hx / 16;
+        e = cudaMalloc(&p->rtw, (size_t)3 * T * sizeof(cplx));
+        if (e != cudaSuccess) return e;
+        p->bytes += (size_t)3 * T * sizeof(cplx);
+        rowtw_kernel<<<(T + 127) / 128, 128>>>(p->rtw, p->tw, T, g.Nt, g.Hx);
+    }
     void *fn = nullptr; cudaDriverEntryPointQueryResult qr;
     e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
     if (e != cudaSuccess) return e;
@@ -433,7 +454,7 @@ cudaError_t rows_init(sfft_plan *p) {
                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
-void rows_free(sfft_plan *p) { delete p->mapI; p->mapI = nullptr; }
+void rows_free(sfft_plan *p) { delete p->mapI; p->mapI = nullptr; if (p->rtw) cudaFree(p->rtw); p->rtw = nullptr; }
 
 template <int LOG2H> static int row_grid(const sfft_plan *p) {
     const int need = ((p->g.ny + 1) / 2 + RowCfg<LOG2H>::RP - 1) / RowCfg<LOG2H>::RP;
@@ -450,10 +471,10 @@ static void run_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cp
     const bool bulk = ((g.nx & 1) == 0) && (((size_t)img & 15) == 0);
     const int grid = row_grid<LOG2H>(p);
     const size_t sm = RowCfg<LOG2H>::SMEM_F;
-    if (bulk && !mask) row_fwd_kernel<LOG2H, true, false><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
-    else if (bulk) row_fwd_kernel<LOG2H, true, true><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
-    else if (!mask) row_fwd_kernel<LOG2H, false, false><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
-    else row_fwd_kernel<LOG2H, false, true><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw);
+    if (bulk && !mask) row_fwd_kernel<LOG2H, true, false><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw, p->rtw);
+    else if (bulk) row_fwd_kernel<LOG2H, true, true><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw, p->rtw);
+    else if (!mask) row_fwd_kernel<LOG2H, false, false><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw, p->rtw);
+    else row_fwd_kernel<LOG2H, false, true><<<grid, ROW_THREADS, sm, p->stream>>>(img, mask, inter, NI, mu, NMOM, g, p->tw, p->rtw);
 }
 
 cudaError_t launch_row_fwd(sfft_plan *p, const double *img, const uint8_t *mask, cplx *inter, int NI, double *mu, int NMOM) {
