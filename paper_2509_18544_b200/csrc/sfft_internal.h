@@ -37,7 +37,7 @@ struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of
 };
 
 // launch shape of stage 1 of a lag pass (sfft_lags.cu), fixed at plan creation
-struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split, nst; size_t smem; };
+struct LagCfg { int WB, KXC, npg, nkb, ngr, nsplit, halves, rows_per_split, nst; bool wide; size_t smem; }; // wide: one CTA of <= 384 threads per SM
 struct LagMaps;             // TMA tensor maps of a lag pass (sfft_lags.cu)
 } // namespace sfft
 struct CUtensorMap_st;      // <cuda.h>: CUtensorMap

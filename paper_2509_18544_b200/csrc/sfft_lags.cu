@@ -164,6 +164,18 @@ lagcol_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, con
     }
 }
 
+// The WIDE form: when the pairs of a pass need more than 192 threads but fit 384 (the Omega pass of DK = 2: 21 pairs x 2 kx
+// x 8 b-lanes = 352 threads at 168 registers), ONE CTA per SM takes them all and one ring feeds them, instead of two CTAs
+// that each bring their own copy of every stage from L2: 0.420 -> 0.372 ms at 4088^2 (a fifth of the warps' stall samples
+// had been waiting for stage data).
+template <int WB, typename ST>
+__global__ void __launch_bounds__(384, 1)
+lagcol_wide_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, const cplx *__restrict__ PH, cplx *__restrict__ Q, Geom g) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ unsigned long long full[4], done[4];
+    lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, blockIdx.z, PH, Q, g, smem_raw, full, done);
+}
+
 // phase table PH[b/8][d-1][b%8] = exp(-2 pi i b d/My), b < My/16, d = 1..W (W = the kernel's compile-time lag bound WB)
 __global__ void lag_phase_kernel(cplx *PH, int W, int My, const cplx *__restrict__ tw, int Nt) {
     const int id = blockIdx.x * blockDim.x + threadIdx.x, Tb = My / LC_NA;
@@ -237,16 +249,18 @@ void lagcol_config(const Geom &g, int np, int ns, int W, LagCfg *c, size_t esz) 
     const int WB = W <= 3 ? 3 : W <= 5 ? 5 : W <= 6 ? 6 : W <= 10 ? 10 : 20;
     const int Tb = g.My / LC_NA;
     const int KXC = ns <= 7 ? 2 : 1;
-    int npg = 192 / (LC_NB * KXC); if (npg > np) npg = np;
+    // wide form (lagcol_wide_kernel): all pairs in one CTA when that takes 193..384 threads and all lags fit one thread
+    const bool wide = WB <= 10 && np * KXC * LC_NB > 192 && ((np * KXC + 3) & ~3) * LC_NB <= 384;
+    int npg = (wide ? 384 : 192) / (LC_NB * KXC); if (npg > np) npg = np;
     int ngr = (np + npg - 1) / npg; npg = (np + ngr - 1) / ngr;   // even groups (21 pairs: 11 + 10)
     while ((npg * KXC) & 3) npg++;                                 // whole warps (inactive pair slots idle)
     const size_t stage = (size_t)ns * KXC * LC_NA * LC_NB * esz + (size_t)WB * LC_NB * sizeof(cplx); // the kernel folds WB lags (>= W)
     int nst = 4;
     while (nst > 2 && nst * stage > (size_t)110 * 1024) nst--;
     c->WB = WB; c->KXC = KXC; c->npg = npg; c->ngr = ngr; c->nkb = (g.Hx + 1 + KXC - 1) / KXC;
-    c->halves = WB > 10 ? 2 : 1;
+    c->halves = WB > 10 ? 2 : 1; c->wide = wide;
     int nsplit = 1;   // few kx blocks (small frames): split the ky range so that the machine still fills
-    while ((long long)c->nkb * ngr * nsplit * c->halves < 296 && Tb / (2 * nsplit) >= 2 * LC_NB) nsplit *= 2;
+    while ((long long)c->nkb * ngr * nsplit * c->halves < (wide ? 148 : 296) && Tb / (2 * nsplit) >= 2 * LC_NB) nsplit *= 2;
     c->nsplit = nsplit; c->rows_per_split = Tb / nsplit; c->nst = nst; c->smem = nst * stage;
 }
 
@@ -275,6 +289,11 @@ static cudaError_t make_lag_map(CUtensorMap *tm, const void *base, bool f32, int
 template <int WB> static cudaError_t lag_attr() {
     cudaError_t e = cudaFuncSetAttribute(lagcol_kernel<WB, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(lagcol_kernel<WB, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    if (WB <= 10) {
+        constexpr int WW = WB <= 10 ? WB : 10;
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lagcol_wide_kernel<WW, cplx>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lagcol_wide_kernel<WW, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    }
     return e;
 }
 
@@ -316,7 +335,10 @@ static cudaError_t run_lagcol(sfft_plan *p, const LagMaps &maps, int ns, int nsc
     la.ns = ns; la.nsci = nsci; la.npg = c.npg; la.KXC = c.KXC; la.W = W; la.nbs = c.rows_per_split; la.nst = c.nst; la.phW = c.WB;
     dim3 grid(c.ngr * c.halves, c.nkb, c.nsplit);
     KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega");
-    if (p->spec32) lagcol_kernel<WB, float2><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
+    constexpr int WW = WB <= 10 ? WB : 10;
+    if (c.wide && p->spec32) lagcol_wide_kernel<WW, float2><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
+    else if (c.wide) lagcol_wide_kernel<WW, cplx><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
+    else if (p->spec32) lagcol_kernel<WB, float2><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
     else lagcol_kernel<WB, cplx><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
     return cudaGetLastError();
 }
