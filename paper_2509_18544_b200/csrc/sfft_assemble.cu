@@ -61,23 +61,45 @@ __device__ __forceinline__ double block_sum2(double v, double *sh) {
     return r;
 }
 
-// grid = (L*L, NB, NK); block 128
-__global__ void __launch_bounds__(128) gamma_cols_kernel(const double *__restrict__ gamA, double *__restrict__ gam, Geom g) {
-    __shared__ double sh[32];
+// grid = (L [v], NB, NK); block 512.  One CTA takes ALL u of its (v, s, t): the weight yt^j yt((y+v) mod ny)^q of a row is
+// formed once and meets the L rows A_{i,p,u}[y] (one CTA per (u, v, s, t) spent 57 us of a machine whose FP64 pipe is
+// the scarce resource on int -> double conversions and powers it repeated 4356 times; this form: 8 x fewer FP64
+// instructions, 11 x fewer CTAs).
+__global__ void __launch_bounds__(512) gamma_cols_kernel(const double *__restrict__ gamA, double *__restrict__ gam, Geom g) {
+    __shared__ double sh[16][MAX_L];
     const int L = g.L, w = g.w, ny = g.ny;
-    const int uv = blockIdx.x, s = blockIdx.y, t = blockIdx.z;
-    const int ui = uv % L, v = uv / L - w;
+    const int vi = blockIdx.x, v = vi - w, s = blockIdx.y, t = blockIdx.z;
     const int i = g.pi[t], j = g.pj[t], pp = g.pi[s], qq = g.pj[s];
-    const double *A = gamA + (((size_t)i * (g.DB + 1) + pp) * L + ui) * ny;
-    double acc = 0.0;
+    const double *A = gamA + (((size_t)i * (g.DB + 1) + pp) * L) * ny; // rows u = 0..L-1, ny apart
+    double acc[MAX_L];
+#pragma unroll
+    for (int u = 0; u < MAX_L; u++) acc[u] = 0.0;
     const double inv_ny = 1.0 / (double)ny;
     for (int y = threadIdx.x; y < ny; y += blockDim.x) {
         int y2 = y + v; if (y2 >= ny) y2 -= ny; if (y2 < 0) y2 += ny;
         const double yt = (2.0 * y + 1.0 - ny) * inv_ny, yt2 = (2.0 * y2 + 1.0 - ny) * inv_ny;
-        acc += ipw(yt, j) * ipw(yt2, qq) * A[y];
+        const double wgt = ipw(yt, j) * ipw(yt2, qq);
+#pragma unroll
+        for (int u = 0; u < MAX_L; u++)
+            if (u < L) acc[u] = fma(wgt, A[(size_t)u * ny + y], acc[u]);
     }
-    acc = block_sum2(acc, sh);
-    if (threadIdx.x == 0) gam[((size_t)t * g.NB + s) * L * L + uv] = acc;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int u = 0; u < MAX_L; u++)
+        if (u < L) {
+            double x = acc[u];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
+            if (lane == 0) sh[wid][u] = x;
+        }
+    __syncthreads();
+    if ((int)threadIdx.x < L) {
+        const int u = threadIdx.x;
+        double x = 0.0;
+#pragma unroll
+        for (int k = 0; k < 16; k++) x += sh[k][u];
+        gam[((size_t)t * g.NB + s) * L * L + vi * L + u] = x;
+    }
 }
 
 // grid = NB; block 128:  Delta_s = sum_y yt^q muS_p[y]
@@ -143,7 +165,7 @@ cudaError_t launch_gamma(sfft_plan *p) {
     const Geom &g = p->g;
     const long long total = (long long)(g.DK + 1) * (g.DB + 1) * g.L * g.ny;
     { KLaunch kl(p, "gamma_rows"); gamma_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->muR, p->R, p->mask, p->gamA, g); }
-    { KLaunch kl(p, "gamma_cols"); gamma_cols_kernel<<<dim3(g.L * g.L, g.NB, g.NK), 128, 0, p->cur>>>(p->gamA, p->gam, g); }
+    { KLaunch kl(p, "gamma_cols"); gamma_cols_kernel<<<dim3(g.L, g.NB, g.NK), 512, 0, p->cur>>>(p->gamA, p->gam, g); }
     return cudaGetLastError();
 }
 

@@ -68,18 +68,19 @@ __device__ __forceinline__ void lag_fold(const cplx *x, const cplx *ph, cplx *ac
 struct LagArgs {
     int ns, nsci;        // spectra per stage (NK + nsci); science spectra among them (0 for Omega)
     int npg, KXC, W, nbs, nst; // pairs per group, kx per CTA, lag bound, b per split, ring stages
+    int nkb;             // kx chunks of the pass (a CTA takes chunks blockIdx.y, blockIdx.y + gridDim.y, ...)
     int phW;             // lag bound of the phase table PH[b/8][d-1][b%8], d = 1..phW
 };
 
 template <int DLO, int DHI, typename ST>
-__device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int group, int zsplit,
+__device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int group, int kb, int zsplit,
                                             const cplx *__restrict__ PH, cplx *__restrict__ Q, const Geom &g,
                                             unsigned char *tile, unsigned long long *full, unsigned long long *done) {
     const int Hx = g.Hx, Tb = g.My / LC_NA, KXC = la.KXC, W = la.W, NK = g.NK;
     const int col_elems = LC_NA * LC_NB;                       // one (spectrum, kx) of a stage: 128 elements of ST
     // a stage: the spectra part in ST elements, then the phase factors (cplx); sized in bytes
     const unsigned spec_bytes = (unsigned)(la.ns * KXC * col_elems * sizeof(ST)), stage_bytes = spec_bytes + (unsigned)(la.phW * LC_NB * sizeof(cplx));
-    const int kx0 = blockIdx.y * KXC;   // (the pair group is the FASTEST grid index: the groups of one kx chunk run side by
+    const int kx0 = kb * KXC;           // (the pair group is the FASTEST grid index: the groups of one kx chunk run side by
                                         //  side and the second reads the chunk's spectra from L2, not from DRAM again)
     const int b0 = zsplit * la.nbs, b1 = min(Tb, b0 + la.nbs);
     const int nIt = max(0, (b1 - b0) / LC_NB);
@@ -155,12 +156,22 @@ lagcol_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, con
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long full[4], done[4];
     unsigned char *tile = smem_raw;
-    if (WB > 10) {
-        const int half = blockIdx.x & 1, grp = blockIdx.x >> 1;   // (the lag halves too: fastest index, shared L2 reads)
-        if (half == 0) lagcol_body<0, WB, ST>(maps, la, pl, grp, blockIdx.z, PH, Q, g, tile, full, done);
-        else lagcol_body<-WB, -1, ST>(maps, la, pl, grp, blockIdx.z, PH, Q, g, tile, full, done);
-    } else {
-        lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, blockIdx.z, PH, Q, g, tile, full, done);
+    // A CTA normally takes one kx chunk (gridDim.y = nkb).  While a factorisation runs beside the pass the grid is capped
+    // (run_lagcol) and the CTAs loop: a grid of 1025 short-lived CTAs would hold every SM for one CTA lifetime (57 us at
+    // 4088^2) before the first slot frees, and the factorisation's next small launch waits exactly that long.
+    for (int kb = blockIdx.y; kb < la.nkb; kb += gridDim.y) {
+        if (WB > 10) {
+            const int half = blockIdx.x & 1, grp = blockIdx.x >> 1;   // (the lag halves too: fastest index, shared L2 reads)
+            if (half == 0) lagcol_body<0, WB, ST>(maps, la, pl, grp, kb, blockIdx.z, PH, Q, g, tile, full, done);
+            else lagcol_body<-WB, -1, ST>(maps, la, pl, grp, kb, blockIdx.z, PH, Q, g, tile, full, done);
+        } else {
+            lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, kb, blockIdx.z, PH, Q, g, tile, full, done);
+        }
+        if (kb + (int)gridDim.y < la.nkb) {   // the barriers start over with the next chunk
+            __syncthreads();
+            if (threadIdx.x == 0)
+                for (int k = 0; k < la.nst; k++) { mbar_inval(&full[k]); mbar_inval(&done[k]); }
+        }
     }
 }
 
@@ -173,7 +184,7 @@ __global__ void __launch_bounds__(384, 1)
 lagcol_wide_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, const cplx *__restrict__ PH, cplx *__restrict__ Q, Geom g) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long full[4], done[4];
-    lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, blockIdx.z, PH, Q, g, smem_raw, full, done);
+    lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, blockIdx.y, blockIdx.z, PH, Q, g, smem_raw, full, done);
 }
 
 // phase table PH[b/8][d-1][b%8] = exp(-2 pi i b d/My), b < My/16, d = 1..W (W = the kernel's compile-time lag bound WB)
@@ -332,8 +343,12 @@ size_t lag_q_elems(const sfft_plan *p) { // Q: the largest of the Omega pass and
 template <int WB>
 static cudaError_t run_lagcol(sfft_plan *p, const LagMaps &maps, int ns, int nsci, const PairList &pl, int W, const LagCfg &c, bool science) {
     LagArgs la;
-    la.ns = ns; la.nsci = nsci; la.npg = c.npg; la.KXC = c.KXC; la.W = W; la.nbs = c.rows_per_split; la.nst = c.nst; la.phW = c.WB;
+    la.ns = ns; la.nsci = nsci; la.npg = c.npg; la.KXC = c.KXC; la.W = W; la.nbs = c.rows_per_split; la.nst = c.nst; la.phW = c.WB; la.nkb = c.nkb;
     dim3 grid(c.ngr * c.halves, c.nkb, c.nsplit);
+    if (science && p->factor_pending && !c.wide) {   // leave SMs to the factorisation running beside the pass (lagcol_kernel)
+        const int per = c.ngr * c.halves * c.nsplit, cap = 2 * (p->sms - p->knob.factor_sms) / (per > 0 ? per : 1);
+        if (cap >= 1 && cap < c.nkb) grid.y = cap;
+    }
     KLaunch kl(p, science ? "lagcol_theta" : "lagcol_omega");
     constexpr int WW = WB <= 10 ? WB : 10;
     if (c.wide && p->spec32) lagcol_wide_kernel<WW, float2><<<grid, c.npg * c.KXC * LC_NB, c.smem, p->cur>>>(maps, la, pl, science ? p->phT : p->phO, p->Q, p->g);
