@@ -145,8 +145,14 @@ sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, 
     for (int t = 0; t < g.NK; t++)
         for (int tp = t; tp < g.NK; tp++) { p->plO.a[p->plO.np] = t; p->plO.b[p->plO.np] = tp; p->plO.np++; }
     p->plT.np = g.NK;
+    for (int q = 0; q < MAX_PAIRS; q++) p->plT.ord[q] = q;
     for (int t = 0; t < g.NK; t++) { p->plT.a[t] = t; p->plT.b[t] = g.NK; }
     p->npairsO = p->plO.np;
+    {   // slot order of the Omega pass: the NK self-pairs first
+        int k = 0;
+        for (int q = 0; q < p->plO.np; q++) if (p->plO.a[q] == p->plO.b[q]) p->plO.ord[k++] = q;
+        for (int q = 0; q < p->plO.np; q++) if (p->plO.a[q] != p->plO.b[q]) p->plO.ord[k++] = q;
+    }
 
     const size_t iplane = (size_t)g.My * g.Hx, splane = (size_t)g.My * (g.Hx + 1);
     const int W2 = 4 * g.w + 1, n = g.n;
@@ -384,6 +390,7 @@ static sfft_status science_sideN(sfft_plan *p, int nimg, const double *const *S,
     }
     p->S = S[0];
     PairList pl; pl.np = nimg * g.NK;
+    for (int q = 0; q < MAX_PAIRS; q++) pl.ord[q] = q;
     for (int i = 0; i < nimg; i++)
         for (int t = 0; t < g.NK; t++) { pl.a[i * g.NK + t] = t; pl.b[i * g.NK + t] = g.NK + i; }
     fork_side(p);

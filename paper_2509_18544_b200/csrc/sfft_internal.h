@@ -34,6 +34,7 @@ struct KRec { const char *name; cudaEvent_t e0, e1; };
 struct PairList {           // spectra pairs (A = spec[a[p]], B = spec[b[p]]) of one lag pass
     int np;
     int a[MAX_PAIRS], b[MAX_PAIRS];
+    int ord[MAX_PAIRS];     // thread slot -> pair: self-pairs (a == b) first, so that they fill whole warps of the lag pass
 };
 
 // launch shape of stage 1 of a lag pass (sfft_lags.cu), fixed at plan creation

@@ -72,7 +72,7 @@ struct LagArgs {
     int phW;             // lag bound of the phase table PH[b/8][d-1][b%8], d = 1..phW
 };
 
-template <int DLO, int DHI, typename ST>
+template <int DLO, int DHI, typename ST, bool SELF = false>
 __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int group, int kb, int zsplit,
                                             const cplx *__restrict__ PH, cplx *__restrict__ Q, const Geom &g,
                                             unsigned char *tile, unsigned long long *full, unsigned long long *done) {
@@ -86,8 +86,9 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
     const int nIt = max(0, (b1 - b0) / LC_NB);
     const int bl = threadIdx.x & (LC_NB - 1), u = threadIdx.x >> 3;
     const int lp = u / KXC, kxl = u - lp * KXC;
-    const int p = group * la.npg + lp;
-    const bool active = (p < pl.np) && (lp < la.npg);
+    const int slot = group * la.npg + lp;
+    const bool active = (slot < pl.np) && (lp < la.npg);
+    const int p = active ? pl.ord[slot] : 0;
     const int sa = active ? pl.a[p] : 0, sb = active ? pl.b[p] : 0;
     constexpr int NACC = DHI - DLO + 1;
     cplx acc[NACC];
@@ -123,8 +124,13 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
             const ST *pa = reinterpret_cast<const ST *>(st) + (size_t)(sa * KXC + kxl) * col_elems + bl;
             const ST *pb = reinterpret_cast<const ST *>(st) + (size_t)(sb * KXC + kxl) * col_elems + bl;
             cplx x[LC_NA];
+            if (SELF && sa == sb) {   // a self-pair (whole warps of them: PairList::ord): |A|^2, one operand read
 #pragma unroll
-            for (int a = 0; a < LC_NA; a++) x[a] = cmulc(ld_c(pa[a * LC_NB]), ld_c(pb[a * LC_NB]));
+                for (int a = 0; a < LC_NA; a++) { const cplx z = ld_c(pa[a * LC_NB]); x[a] = mk(fma(z.x, z.x, z.y * z.y), 0.0); }
+            } else {
+#pragma unroll
+                for (int a = 0; a < LC_NA; a++) x[a] = cmulc(ld_c(pa[a * LC_NB]), ld_c(pb[a * LC_NB]));
+            }
             dft16<1>(x);
             lag_fold<DLO, DHI>(x, reinterpret_cast<const cplx *>(st + spec_bytes) + bl, acc);
         }
@@ -184,7 +190,7 @@ __global__ void __launch_bounds__(384, 1)
 lagcol_wide_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, const cplx *__restrict__ PH, cplx *__restrict__ Q, Geom g) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long full[4], done[4];
-    lagcol_body<-WB, WB, ST>(maps, la, pl, blockIdx.x, blockIdx.y, blockIdx.z, PH, Q, g, smem_raw, full, done);
+    lagcol_body<-WB, WB, ST, true>(maps, la, pl, blockIdx.x, blockIdx.y, blockIdx.z, PH, Q, g, smem_raw, full, done);
 }
 
 // phase table PH[b/8][d-1][b%8] = exp(-2 pi i b d/My), b < My/16, d = 1..W (W = the kernel's compile-time lag bound WB)
