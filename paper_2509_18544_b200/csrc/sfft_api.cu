@@ -79,6 +79,7 @@ static void free_plan(sfft_plan *p) {
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
     for (int i = 1; i < 2 * NSCI; i++) { if (p->hq[i]) cudaFree(p->hq[i]); if (p->cq[i]) cudaFree(p->cq[i]); }
     if (p->flag_host) cudaFreeHost(p->flag_host);
+    if (p->gmeta) cudaFree(p->gmeta);
     lags_free(p); rows_free(p);
     for (int s = 0; s < SFFT_NUM_STAGES; s++) {
         if (p->ev0[s]) cudaEventDestroy(p->ev0[s]);
@@ -203,6 +204,7 @@ sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, 
     AL(p->delta, g.NB);
     for (int i = 1; i < NSCI; i++) AL(p->deltax[i], g.NB);
     AL(p->G, (size_t)n * n);
+    if (e == cudaSuccess) { e = cudaMalloc(&p->gmeta, (size_t)n * sizeof(int)); if (e == cudaSuccess) p->bytes += (size_t)n * sizeof(int); }
     AL(p->h, n);
     AL(p->Lf, (size_t)n * n);
     AL(p->dscale, n);
@@ -250,7 +252,8 @@ sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, 
     cudaEventCreateWithFlags(&p->ev_lookP, cudaEventDisableTiming);
     cudaEventCreateWithFlags(&p->ev_lookB, cudaEventDisableTiming);
     twiddle_kernel<<<(g.Nt + 255) / 256, 256>>>(p->tw, g.Nt);
-    e = rows_init(p);
+    e = assemble_init(p);
+    if (e == cudaSuccess) e = rows_init(p);
     if (e == cudaSuccess) e = cols_init();
     if (e == cudaSuccess) e = lags_init(p);   // tensor maps over the spectra, phase tables (after the twiddles)
     if (e != cudaSuccess) { cudaGetLastError(); free_plan(p); return SFFT_ERR_CUDA; }

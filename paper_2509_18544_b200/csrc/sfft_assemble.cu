@@ -115,13 +115,22 @@ __global__ void __launch_bounds__(128) delta_kernel(const double *__restrict__ m
 
 __device__ __forceinline__ int pair_index(int t, int tp, int NK) { return t * NK - (t * (t - 1)) / 2 + (tp - t); }
 
-// entry (r, c) of G from the lag tables
+// index meta data of an unknown r < NK L^2: t | (v + w) << 8 | (u + w) << 16; r >= NK L^2 (background term s): -1 - s.
+// Geometry only: written once at plan creation (assemble_init), so that the gather of G divides nothing.
+__global__ void gather_meta_kernel(int *meta, Geom g) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= g.n) return;
+    const int L = g.L, LL = L * L, NKLL = g.NK * LL;
+    meta[r] = r < NKLL ? ((r / LL) | (((r % LL) / L) << 8) | (((r % LL) % L) << 16)) : -1 - (r - NKLL);
+}
+
+// entry (r, c) of G from the lag tables; mr, mc: the meta words of r and c
 __device__ __forceinline__ double g_entry(const double *__restrict__ lagO, const double *__restrict__ gam,
-                                          const double *__restrict__ phi, const Geom &g, int r, int c) {
-    const int L = g.L, w = g.w, LL = L * L, NKLL = g.NK * LL, W2 = 4 * w + 1;
-    if (r < NKLL && c < NKLL) {
-        const int t = r / LL, v = (r % LL) / L - w, u = (r % LL) % L - w;
-        const int tp = c / LL, vp = (c % LL) / L - w, up = (c % LL) % L - w;
+                                          const double *__restrict__ phi, const Geom &g, int mr, int mc) {
+    const int L = g.L, w = g.w, LL = L * L, W2 = 4 * w + 1;
+    if (mr >= 0 && mc >= 0) {
+        const int t = mr & 255, v = (mr >> 8) & 255, u = mr >> 16;
+        const int tp = mc & 255, vp = (mc >> 8) & 255, up = mc >> 16;
         // X(b,a)[d] = X(a,b)[-d] (pin P11): every entry and its transpose read the SAME table slot, so G is
         // symmetric bit for bit (for t == t' the slot with the lexicographically non-negative lag is used)
         int dv = v - vp, du = u - up;
@@ -129,26 +138,27 @@ __device__ __forceinline__ double g_entry(const double *__restrict__ lagO, const
         if (flip) { dv = -dv; du = -du; }
         return lagO[(size_t)pair_index(flip ? tp : t, flip ? t : tp, g.NK) * W2 * W2 + (dv + 2 * w) * W2 + (du + 2 * w)];
     }
-    if (r < NKLL) return gam[((size_t)(r / LL) * g.NB + (c - NKLL)) * LL + r % LL];
-    if (c < NKLL) return gam[((size_t)(c / LL) * g.NB + (r - NKLL)) * LL + c % LL];
-    return phi[(r - NKLL) * g.NB + (c - NKLL)];
+    if (mr >= 0) { const int t = mr & 255, v = (mr >> 8) & 255, u = mr >> 16; return gam[((size_t)t * g.NB + (-1 - mc)) * LL + v * L + u]; }
+    if (mc >= 0) { const int t = mc & 255, v = (mc >> 8) & 255, u = mc >> 16; return gam[((size_t)t * g.NB + (-1 - mr)) * LL + v * L + u]; }
+    return phi[(-1 - mr) * g.NB + (-1 - mc)];
 }
 
-// one thread per entry of G (full matrix, both triangles).  The Jacobi equilibration of step a4 rides along (the
-// factorisation follows every gather, and two more small launches sat on the critical path of a step): the thread also
-// gathers its two diagonal entries and writes the scaled lower triangle Lf = D^-1/2 G D^-1/2 and D^-1/2 itself, with
-// the same expressions as equil_diag_kernel / equil_scale_kernel (sfft_solve.cu), which remain for a G that arrives
-// some other way.  *flag is raised for a diagonal entry <= 0.
-__global__ void gather_G_kernel(const double *__restrict__ lagO, const double *__restrict__ gam,
-                                const double *__restrict__ phi, double *__restrict__ G, double *__restrict__ Lf,
-                                double *__restrict__ dscale, int *flag, Geom g) {
-    const int n = g.n;
-    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= (long long)n * n) return;
-    const int r = (int)(id / n), c = (int)(id % n);
-    const double val = g_entry(lagO, gam, phi, g, r, c);
+// grid = (ceil(n / 256), n): one CTA row per row of G, one thread per entry (both triangles).  The Jacobi equilibration
+// of step a4 rides along (the factorisation follows every gather, and two more small launches sat on the critical path
+// of a step): the thread also gathers its two diagonal entries and writes the scaled lower triangle
+// Lf = D^-1/2 G D^-1/2 and D^-1/2 itself, with the same expressions as equil_diag_kernel / equil_scale_kernel
+// (sfft_solve.cu), which remain for a G that arrives some other way.  *flag is raised for a diagonal entry <= 0.
+// (With one thread per linear index and its divisions this kernel took 235 us at n = 4416.)
+__global__ void __launch_bounds__(256) gather_G_kernel(const double *__restrict__ lagO, const double *__restrict__ gam,
+                                const double *__restrict__ phi, const int *__restrict__ meta, double *__restrict__ G,
+                                double *__restrict__ Lf, double *__restrict__ dscale, int *flag, Geom g) {
+    const int n = g.n, r = blockIdx.y, c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n) return;
+    const int mr = meta[r], mc = meta[c];
+    const size_t id = (size_t)r * n + c;
+    const double val = g_entry(lagO, gam, phi, g, mr, mc);
     G[id] = val;
-    const double grr = g_entry(lagO, gam, phi, g, r, r), gcc = g_entry(lagO, gam, phi, g, c, c);
+    const double grr = g_entry(lagO, gam, phi, g, mr, mr), gcc = g_entry(lagO, gam, phi, g, mc, mc);
     const double sr = grr > 0.0 ? 1.0 / sqrt(grr) : 1.0, sc = gcc > 0.0 ? 1.0 / sqrt(gcc) : 1.0;
     if (c == 0) { dscale[r] = sr; if (!(grr > 0.0)) *flag = 1; }
     Lf[id] = c <= r ? sr * val * sc : 0.0;
@@ -174,10 +184,15 @@ cudaError_t launch_delta(sfft_plan *p, const double *muS, double *delta) {
     return cudaGetLastError();
 }
 
+// plan creation: the index meta data of the gather (p->gmeta allocated by the caller)
+cudaError_t assemble_init(sfft_plan *p) {
+    gather_meta_kernel<<<(p->g.n + 255) / 256, 256>>>(p->gmeta, p->g);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_gather_G(sfft_plan *p) {
-    const long long total = (long long)p->g.n * p->g.n;
     cudaMemsetAsync(p->flag, 0, sizeof(int), p->cur);   // the pivot flag of the factorisation that follows (launch_factor)
-    { KLaunch kl(p, "gather_G"); gather_G_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->lagO, p->gam, p->phi, p->G, p->Lf, p->dscale, p->flag, p->g); }
+    { KLaunch kl(p, "gather_G"); gather_G_kernel<<<dim3((p->g.n + 255) / 256, p->g.n), 256, 0, p->cur>>>(p->lagO, p->gam, p->phi, p->gmeta, p->G, p->Lf, p->dscale, p->flag, p->g); }
     p->lf_ready = true;                                  // Lf and dscale hold the equilibrated matrix of this G
     return cudaGetLastError();
 }

@@ -68,35 +68,47 @@ __global__ void __launch_bounds__(256) linpair_kernel(const double *__restrict__
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
     const double inv_n = 1.0 / (double)n;
     const size_t slot = ((((size_t)blockIdx.x * 4 + blockIdx.z) * W + rI) * W + zI) * (2 * W + 1);
+    // c(pos + e) = c(pos) + delta, delta = 2e/n, so c(pos)^ea c(pos+e)^eb = sum_m C(eb, m) delta^(eb-m) c(pos)^(ea+m): the
+    // EA x EB weighted correlations of a lag follow from the EA + EB - 1 moments M_k = sum_pos c(pos)^k a[pos] b[pos+e]
+    // (7 running sums instead of 16 products for DK = 3, 5 instead of 9 for DK = 2: the kernel is FP64-bound).
+    constexpr int NM = EA + EB - 1;
     for (int ei = warp; ei <= 2 * W; ei += nw) {
         const int e = ei - W;
-        double acc[EA][EB];
+        double mom[NM];
 #pragma unroll
-        for (int i = 0; i < EA; i++)
-#pragma unroll
-            for (int j = 0; j < EB; j++) acc[i][j] = 0.0;
+        for (int k = 0; k < NM; k++) mom[k] = 0.0;
         for (int k = lane; k < CH; k += 32) {
-            const double ca = (2.0 * (p0 + k) + 1.0 - n) * inv_n, cb = (2.0 * (p0 + k + e) + 1.0 - n) * inv_n;
-            double pa[EA], pb[EB];
-            pa[0] = sa[k]; pb[0] = sb[k + W + e];
+            const double ca = (2.0 * (p0 + k) + 1.0 - n) * inv_n;
+            double t = sa[k] * sb[k + W + e];
 #pragma unroll
-            for (int i = 1; i < EA; i++) pa[i] = pa[i - 1] * ca;
+            for (int m = 0; m < NM; m++) { mom[m] += t; t *= ca; }
+        }
 #pragma unroll
-            for (int j = 1; j < EB; j++) pb[j] = pb[j - 1] * cb;
+        for (int m = 0; m < NM; m++) {
+            double v = mom[m];
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+            mom[m] = v;
+        }
+        if (lane == 0) {
+            const double delta = 2.0 * e * inv_n;
+            double dp[EB];   // delta^j
+            dp[0] = 1.0;
+#pragma unroll
+            for (int j = 1; j < EB; j++) dp[j] = dp[j - 1] * delta;
 #pragma unroll
             for (int i = 0; i < EA; i++)
 #pragma unroll
-                for (int j = 0; j < EB; j++) acc[i][j] = fma(pa[i], pb[j], acc[i][j]);
+                for (int j = 0; j < EB; j++) {
+                    double v = 0.0, binom = 1.0;   // C(j, m), m = 0..j
+#pragma unroll
+                    for (int m = 0; m <= j; m++) {
+                        v = fma(binom * dp[j - m], mom[i + m], v);
+                        binom = binom * (double)(j - m) / (double)(m + 1);
+                    }
+                    LP[((slot + ei) * EA + i) * EB + j] = v;
+                }
         }
-#pragma unroll
-        for (int i = 0; i < EA; i++)
-#pragma unroll
-            for (int j = 0; j < EB; j++) {
-                double v = acc[i][j];
-#pragma unroll
-                for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
-                if (lane == 0) LP[((slot + ei) * EA + i) * EB + j] = v;
-            }
     }
 }
 

@@ -106,6 +106,7 @@ struct sfft_plan {
     double *phi;             // [NB][NB]
     double *delta;           // [NB]
     double *G;               // [n][n]
+    int *gmeta;              // [n] index meta data of the unknowns for the gather of G (sfft_assemble.cu)
     double *h;               // [n]
     double *h2, *coef2;      // [n] each: second right-hand side / solution (the batched path pipelines two images)
     double *Lf;              // [n][n] Cholesky factor of the equilibrated matrix (lower, row-major)
@@ -173,6 +174,7 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag /*[
 // nsci > 1: pl lists the NK pairs of each image in turn (images p->Sx[i])
 cudaError_t launch_gamma(sfft_plan *p);   // muR, R, mask -> gam
 cudaError_t launch_delta(sfft_plan *p, const double *muS = nullptr, double *delta = nullptr);   // muS -> delta
+cudaError_t assemble_init(sfft_plan *p);
 cudaError_t launch_gather_G(sfft_plan *p);
 cudaError_t launch_gather_h(sfft_plan *p, const double *lagT = nullptr, const double *delta = nullptr, double *h = nullptr);
 

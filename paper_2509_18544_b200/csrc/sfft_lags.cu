@@ -258,6 +258,15 @@ __global__ void __launch_bounds__(256) lagrow_kernel(const cplx *__restrict__ Q,
     }
 }
 
+// lag[i] += sum over chunks of bpart[chunk][i]: the native-grid wrap corrections join the lag tables
+__global__ void lagadd_kernel(double *__restrict__ lag, const double *__restrict__ bpart, int total, int nchunk) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    double v = lag[i];
+    for (int k = 0; k < nchunk; k++) v += bpart[(size_t)k * total + i];
+    lag[i] = v;
+}
+
 // ---------------------------------------------------------------- host side
 // Launch shape of stage 1, fixed at plan creation (it sizes Q and the TMA boxes): 8 b-lanes per (pair, kx),
 // KXC kx per CTA, pairs in even groups, CTAs of <= 192 threads so that two fit an SM with the accumulators in
@@ -400,13 +409,19 @@ cudaError_t launch_lags(sfft_plan *p, const PairList &pl, int W, double *lag, bo
     else if (c.WB == 10) e = run_lagcol<10>(p, maps, ns, science ? nsci : 0, pl, W, c, science);
     else e = run_lagcol<20>(p, maps, ns, science ? nsci : 0, pl, W, c, science);
     if (e != cudaSuccess) return e;
-    join_side(p);
-    {
+    {   // the row reduction does not wait for the wrap corrections (a chain of small kernels on a side stream that only gets
+        // SMs once the column pass has ended -- 0.57 ms of it at L = 21): they are added afterwards (lagadd)
         KLaunch kl(p, science ? "lagrow_theta" : "lagrow_omega");
         const dim3 gr(pl.np, 2 * W + 1);
-        if (W <= 5) lagrow_kernel<5><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
-        else if (W <= 10) lagrow_kernel<10><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
-        else lagrow_kernel<MAX_L - 1><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, nchunk, lag, g, p->tw);
+        if (W <= 5) lagrow_kernel<5><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, 0, lag, g, p->tw);
+        else if (W <= 10) lagrow_kernel<10><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, 0, lag, g, p->tw);
+        else lagrow_kernel<MAX_L - 1><<<gr, 256, 0, p->cur>>>(p->Q, pl.np, W, nsplit, bpart, 0, lag, g, p->tw);
+    }
+    join_side(p);
+    if (nchunk > 0) {
+        const int total = pl.np * (2 * W + 1) * (2 * W + 1);
+        KLaunch kl(p, science ? "lagadd_theta" : "lagadd_omega");
+        lagadd_kernel<<<(total + 255) / 256, 256, 0, p->cur>>>(lag, bpart, total, nchunk);
     }
     return cudaGetLastError();
 }
