@@ -73,7 +73,7 @@ struct StageTimer {
 static void free_plan(sfft_plan *p) {
     if (!p) return;
     void *ptrs[] = {p->tw, p->inter, p->specT, (p->specTo != p->specT) ? p->specTo : nullptr, p->specS, p->muR, p->muS,
-                    p->Q, p->phO, p->phT, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
+                    p->Q, p->phO, p->phT, p->lagO, p->lagT, p->bpart, p->SB, p->LP, p->gamA, p->gam, p->gamP, p->phi, p->delta, p->G, p->h, p->Lf, p->dscale, p->Linv,
                     p->ywork, p->zwork, p->coef, p->ratioEZ, p->ratioW, p->E, p->wcorr, p->flag, p->stS, p->stR, p->stD, p->stM};
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int i = 1; i < NSCI; i++) { if (p->specSx[i]) cudaFree(p->specSx[i]); if (p->muSx[i]) cudaFree(p->muSx[i]); if (p->deltax[i]) cudaFree(p->deltax[i]); }
@@ -200,6 +200,7 @@ sfft_status sfft_plan_create_ex(sfft_plan **out, int nx, int ny, int L, int DK, 
     }
     AL(p->gamA, (size_t)(DK + 1) * (DB + 1) * L * ny);
     AL(p->gam, (size_t)g.NK * g.NB * L * L);
+    AL(p->gamP, (size_t)((ny + 255) / 256) * g.NK * g.NB * L * L);
     AL(p->phi, g.NB * g.NB);
     AL(p->delta, g.NB);
     for (int i = 1; i < NSCI; i++) AL(p->deltax[i], g.NB);

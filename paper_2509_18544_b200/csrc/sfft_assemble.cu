@@ -61,45 +61,52 @@ __device__ __forceinline__ double block_sum2(double v, double *sh) {
     return r;
 }
 
-// grid = (L [v], NB, NK); block 512.  One CTA takes ALL u of its (v, s, t): the weight yt^j yt((y+v) mod ny)^q of a row is
-// formed once and meets the L rows A_{i,p,u}[y] (one CTA per (u, v, s, t) spent 57 us of a machine whose FP64 pipe is
-// the scarce resource on int -> double conversions and powers it repeated 4356 times; this form: 8 x fewer FP64
-// instructions, 11 x fewer CTAs).
-__global__ void __launch_bounds__(512) gamma_cols_kernel(const double *__restrict__ gamA, double *__restrict__ gam, Geom g) {
-    __shared__ double sh[16][MAX_L];
-    const int L = g.L, w = g.w, ny = g.ny;
-    const int vi = blockIdx.x, v = vi - w, s = blockIdx.y, t = blockIdx.z;
+// Gamma_{(i,j),(p,q)}[u,v] = sum_y W_{j,q,v}[y] A_{i,p,u}[y],  W = yt^j yt((y+v) mod ny)^q: per (t, s) an L x L x ny product.
+// gamma_part: grid = (ceil(ny / GC_Y), NB, NK); block = L^2 rounded up to warps.  A CTA brings its GC_Y-row chunk of the L
+// rows A_{i,p,.} into shared memory ONCE, forms the L weight rows there, and thread (v, u) takes one dot product; a second
+// kernel adds the chunk partials in a fixed order.  (One CTA per (u, v, s, t) re-read the 3 MB table A 44 times through L2
+// and repeated the powers 4356 times: 44 us at L = 11, 167-181 us at L = 21, on the tail behind the Omega pass.)
+constexpr int GC_Y = 256;
+__global__ void gamma_part_kernel(const double *__restrict__ gamA, double *__restrict__ part, Geom g) {
+    extern __shared__ __align__(16) double gsm[];
+    const int L = g.L, w = g.w, ny = g.ny, LL = L * L;
+    double (*As)[GC_Y + 1] = reinterpret_cast<double (*)[GC_Y + 1]>(gsm);
+    double (*Ws)[GC_Y + 1] = reinterpret_cast<double (*)[GC_Y + 1]>(gsm + (size_t)L * (GC_Y + 1));
+    const int ch = blockIdx.x, s = blockIdx.y, t = blockIdx.z, y0 = ch * GC_Y;
     const int i = g.pi[t], j = g.pj[t], pp = g.pi[s], qq = g.pj[s];
     const double *A = gamA + (((size_t)i * (g.DB + 1) + pp) * L) * ny; // rows u = 0..L-1, ny apart
-    double acc[MAX_L];
-#pragma unroll
-    for (int u = 0; u < MAX_L; u++) acc[u] = 0.0;
     const double inv_ny = 1.0 / (double)ny;
-    for (int y = threadIdx.x; y < ny; y += blockDim.x) {
-        int y2 = y + v; if (y2 >= ny) y2 -= ny; if (y2 < 0) y2 += ny;
-        const double yt = (2.0 * y + 1.0 - ny) * inv_ny, yt2 = (2.0 * y2 + 1.0 - ny) * inv_ny;
-        const double wgt = ipw(yt, j) * ipw(yt2, qq);
-#pragma unroll
-        for (int u = 0; u < MAX_L; u++)
-            if (u < L) acc[u] = fma(wgt, A[(size_t)u * ny + y], acc[u]);
-    }
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-#pragma unroll
-    for (int u = 0; u < MAX_L; u++)
-        if (u < L) {
-            double x = acc[u];
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) x += __shfl_down_sync(0xffffffffu, x, off);
-            if (lane == 0) sh[wid][u] = x;
+    for (int e = threadIdx.x; e < L * GC_Y; e += blockDim.x) {
+        const int r = e / GC_Y, yy = e - r * GC_Y, y = y0 + yy;
+        double av = 0.0, wv = 0.0;
+        if (y < ny) {
+            av = A[(size_t)r * ny + y];
+            int y2 = y + (r - w); if (y2 >= ny) y2 -= ny; if (y2 < 0) y2 += ny;
+            wv = ipw((2.0 * y + 1.0 - ny) * inv_ny, j) * ipw((2.0 * y2 + 1.0 - ny) * inv_ny, qq);
         }
-    __syncthreads();
-    if ((int)threadIdx.x < L) {
-        const int u = threadIdx.x;
-        double x = 0.0;
-#pragma unroll
-        for (int k = 0; k < 16; k++) x += sh[k][u];
-        gam[((size_t)t * g.NB + s) * L * L + vi * L + u] = x;
+        As[r][yy] = av; Ws[r][yy] = wv;
     }
+    __syncthreads();
+    const int o = threadIdx.x;
+    if (o >= LL) return;
+    const int vi = o / L, u = o - vi * L;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;   // four running sums, added in a fixed order
+#pragma unroll 4
+    for (int yy = 0; yy < GC_Y; yy += 4) {
+        a0 = fma(Ws[vi][yy], As[u][yy], a0);
+        a1 = fma(Ws[vi][yy + 1], As[u][yy + 1], a1);
+        a2 = fma(Ws[vi][yy + 2], As[u][yy + 2], a2);
+        a3 = fma(Ws[vi][yy + 3], As[u][yy + 3], a3);
+    }
+    part[(((size_t)ch * g.NK + t) * g.NB + s) * LL + o] = (a0 + a1) + (a2 + a3);
+}
+// gam[t][s][v][u] = sum over the chunks, in order
+__global__ void gamma_sum_kernel(const double *__restrict__ part, double *__restrict__ gam, int total, int nch) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= total) return;
+    double v = 0.0;
+    for (int c = 0; c < nch; c++) v += part[(size_t)c * total + id];
+    gam[id] = v;
 }
 
 // grid = NB; block 128:  Delta_s = sum_y yt^q muS_p[y]
@@ -175,7 +182,12 @@ cudaError_t launch_gamma(sfft_plan *p) {
     const Geom &g = p->g;
     const long long total = (long long)(g.DK + 1) * (g.DB + 1) * g.L * g.ny;
     { KLaunch kl(p, "gamma_rows"); gamma_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, p->cur>>>(p->muR, p->R, p->mask, p->gamA, g); }
-    { KLaunch kl(p, "gamma_cols"); gamma_cols_kernel<<<dim3(g.L, g.NB, g.NK), 512, 0, p->cur>>>(p->gamA, p->gam, g); }
+    {
+        const int nch = (g.ny + GC_Y - 1) / GC_Y, total = g.NK * g.NB * g.L * g.L, bt = ((g.L * g.L + 31) / 32) * 32;
+        const size_t sm = (size_t)2 * g.L * (GC_Y + 1) * sizeof(double);
+        { KLaunch kl(p, "gamma_cols"); gamma_part_kernel<<<dim3(nch, g.NB, g.NK), bt, sm, p->cur>>>(p->gamA, p->gamP, g); }
+        { KLaunch kl(p, "gamma_sum"); gamma_sum_kernel<<<(total + 255) / 256, 256, 0, p->cur>>>(p->gamP, p->gam, total, nch); }
+    }
     return cudaGetLastError();
 }
 
@@ -184,8 +196,12 @@ cudaError_t launch_delta(sfft_plan *p, const double *muS, double *delta) {
     return cudaGetLastError();
 }
 
-// plan creation: the index meta data of the gather (p->gmeta allocated by the caller)
+// plan creation: the index meta data of the gather (p->gmeta allocated by the caller), kernel attributes
 cudaError_t assemble_init(sfft_plan *p) {
+    {   // gamma_part_kernel: 2 L (GC_Y + 1) doubles of shared memory (86 KB at L = 21)
+        const cudaError_t e = cudaFuncSetAttribute(gamma_part_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)2 * MAX_L * (GC_Y + 1) * sizeof(double)));
+        if (e != cudaSuccess) return e;
+    }
     gather_meta_kernel<<<(p->g.n + 255) / 256, 256>>>(p->gmeta, p->g);
     return cudaGetLastError();
 }

@@ -103,6 +103,7 @@ struct sfft_plan {
     double *LP;              // [chunk][4][W][W][2W+1][DK+1][DK+1|1] line-pair linear correlations
     double *gamA;            // [(DK+1)][(DB+1)][L][ny] row sums for Gamma
     double *gam;             // [NK][NB][L*L]
+    double *gamP;            // [ceil(ny/256)][NK][NB][L*L] chunk partials of Gamma (sfft_assemble.cu)
     double *phi;             // [NB][NB]
     double *delta;           // [NB]
     double *G;               // [n][n]
