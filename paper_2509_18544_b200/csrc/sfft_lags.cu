@@ -25,7 +25,8 @@ namespace sfft {
 
 constexpr int LC_NA = 16;  // decimation factor: ky = b + (My/16) a, a = 0..15
 constexpr int LC_NB = 8;   // consecutive b per stage and per (pair, kx): one 128-byte line of a spectrum column
-constexpr int LC_PRE = 2;  // prefetch distance in stages
+constexpr int LC_PRE = 2;  // prefetch distance in stages; the wide form uses 1 (measured there: 1 -> 0.365, 2 -> 0.374, 3 -> 0.486 ms;
+                           // the two-CTA forms: 2 is 1-1.5 % faster than 1): more loads in flight are slower
 
 struct LagMaps { CUtensorMap t; CUtensorMap s[NSCI]; };
 
@@ -72,7 +73,7 @@ struct LagArgs {
     int phW;             // lag bound of the phase table PH[b/8][d-1][b%8], d = 1..phW
 };
 
-template <int DLO, int DHI, typename ST, bool SELF = false>
+template <int DLO, int DHI, typename ST, bool SELF = false, int PRE = LC_PRE>
 __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &la, const PairList &pl, int group, int kb, int zsplit,
                                             const cplx *__restrict__ PH, cplx *__restrict__ Q, const Geom &g,
                                             unsigned char *tile, unsigned long long *full, unsigned long long *done) {
@@ -110,11 +111,11 @@ __device__ __forceinline__ void lagcol_body(const LagMaps &maps, const LagArgs &
         if (la.phW > 0) bulk_g2s(st + spec_bytes, PH + (size_t)(b / LC_NB) * la.phW * LC_NB, (unsigned)(la.phW * LC_NB * 16), bar);
     };
     if (threadIdx.x == 0)
-        for (int it = 0; it < LC_PRE && it < nIt; it++) issue(it);
+        for (int it = 0; it < PRE && it < nIt; it++) issue(it);
     for (int it = 0; it < nIt; it++) {
         const int st_i = it % la.nst;
-        if (threadIdx.x == 0 && it + LC_PRE < nIt) {
-            const int nx_i = it + LC_PRE;
+        if (threadIdx.x == 0 && it + PRE < nIt) {
+            const int nx_i = it + PRE;
             if (nx_i >= la.nst) mbar_wait(&done[nx_i % la.nst], (unsigned)((nx_i / la.nst) - 1) & 1u); // its previous use has been consumed
             issue(nx_i);
         }
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(384, 1)
 lagcol_wide_kernel(const __grid_constant__ LagMaps maps, LagArgs la, PairList pl, const cplx *__restrict__ PH, cplx *__restrict__ Q, Geom g) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long full[4], done[4];
-    lagcol_body<-WB, WB, ST, true>(maps, la, pl, blockIdx.x, blockIdx.y, blockIdx.z, PH, Q, g, smem_raw, full, done);
+    lagcol_body<-WB, WB, ST, true, 1>(maps, la, pl, blockIdx.x, blockIdx.y, blockIdx.z, PH, Q, g, smem_raw, full, done);
 }
 
 // phase table PH[b/8][d-1][b%8] = exp(-2 pi i b d/My), b < My/16, d = 1..W (W = the kernel's compile-time lag bound WB)
